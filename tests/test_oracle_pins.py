@@ -1,0 +1,335 @@
+"""Pins for the CPU oracle (oracle/sfft_oracle.c) against things OTHER than itself:
+the paper's Eqs. 14 and 19-24 evaluated literally with a library DFT, closed forms,
+library routines (scipy.ndimage wrap-convolution, numpy lstsq, scipy BSpline), exact
+rational arithmetic, and recovery of injected parameters.  CPU only.
+Each test names the plausible mistake it would catch.
+"""
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import scipy.interpolate
+import scipy.ndimage
+
+import oracle
+
+POLY, BSPL = oracle.POLY, oracle.BSPLINE
+
+
+def _u(N):
+    return (2.0 * np.arange(N) + 1.0) / N - 1.0
+
+
+def _poly_terms(D):
+    return [(i, j) for i in range(D + 1) for j in range(D + 1 - i)]
+
+
+def _poly_T(H, W, D):
+    ux, uy = _u(H)[:, None], _u(W)[None, :]
+    return [ux ** i * uy ** j * np.ones((H, W)) for (i, j) in _poly_terms(D)]
+
+
+def _rand_pair(H, W, seed):
+    rng = np.random.default_rng(seed)
+    R = 100.0 + 50.0 * rng.random((H, W)) + 400.0 * (rng.random((H, W)) > 0.97)
+    S = 90.0 + 60.0 * rng.random((H, W))
+    return R, S
+
+
+# --------------------------------------------------------------------------- weights
+
+def test_term_order_and_counts():
+    # i in [0,D], j in [0,D-i]  -> (D+1)(D+2)/2 terms; BASELINE unknown counts
+    assert oracle.terms(POLY, 2) == [(0, 0), (0, 1), (0, 2), (1, 0), (1, 1), (2, 0)]
+    for L, DK, DB, n in [(7, 1, 1, 150), (11, 2, 2, 732), (15, 2, 2, 1356), (17, 2, 2, 1740)]:
+        assert oracle.num_unknowns(L, POLY, DK, DB) == n
+    assert oracle.num_unknowns(11, BSPL, 4, 4) == 7808   # DESIGN g13: 8x8 functions
+    assert oracle.terms(BSPL, 4)[9] == (1, 1)
+
+
+def test_poly_axis_closed_form():
+    for N in (8, 12, 128):
+        tab = oracle.axis_table(POLY, N, 3)
+        u = _u(N)
+        for f in range(4):
+            np.testing.assert_allclose(tab[f], u ** f, rtol=0, atol=2e-16)
+        assert np.all(np.abs(u) < 1.0) and abs(u[0] + u[-1]) < 1e-15   # symmetric, inside (-1,1)
+
+
+@pytest.mark.parametrize("N,m", [(16, 0), (64, 4), (100, 2), (1024, 4)])
+def test_bspline_axis_vs_scipy(N, m):
+    # catches a wrong knot vector, degree, or interval convention
+    tab = oracle.axis_table(BSPL, N, m)
+    knots = np.r_[np.zeros(4), np.arange(1, m + 1) / (m + 1.0), np.ones(4)]
+    v = (np.arange(N) + 0.5) / N
+    ref = scipy.interpolate.BSpline.design_matrix(v, knots, 3).toarray().T
+    assert tab.shape == (m + 4, N)
+    np.testing.assert_allclose(tab, ref, rtol=0, atol=5e-16)
+    np.testing.assert_allclose(tab.sum(axis=0), 1.0, rtol=0, atol=1e-15)   # partition of unity
+    assert tab.min() >= 0.0
+
+
+# --------------------------------------------------------------------------- paper's equations
+
+def test_eqs_14_19_24_literal_dft():
+    """Evaluate Eqs. (14), (19)-(24) exactly as printed with numpy's FFT (forward DFT carrying
+    1/(N0 N1), W = exp(-2 pi i/N)) and compare with the oracle's real-space normal system through
+    A = M_aa/N^3, B = M_ab/N^2, C = M_bb/N, D = rhs_a/N^2, E = rhs_b/N  (N = N0 N1), and check that
+    the paper's solution a = N * a_ring.  Catches: wrong shift sign, a dropped
+    '-delta' term, transposed axes, wrong centre handling, wrong index order."""
+    H, W, L, DK, DB = 12, 10, 3, 1, 1
+    w, N = 1, H * W
+    R, S = _rand_pair(H, W, 1)
+    dft = lambda f: np.fft.fft2(f) / N
+    l, m = np.arange(H)[:, None], np.arange(W)[None, :]
+    W0, W1 = np.exp(-2j * np.pi / H), np.exp(-2j * np.pi / W)
+    Khat = {}
+    for al in range(-w, w + 1):
+        for be in range(-w, w + 1):
+            Khat[(al, be)] = np.full((H, W), 1.0 / N, complex) if (al, be) == (0, 0) \
+                else (W0 ** (l * al) * W1 ** (m * be) - 1.0) / N
+    TK, TB = _poly_T(H, W, DK), _poly_T(H, W, DB)
+    Rhat = [dft(T * R) for T in TK]
+    That = [dft(T) for T in TB]
+    Shat = dft(S)
+    lags = [(al, be) for al in range(-w, w + 1) for be in range(-w, w + 1)]
+    FK, FB, LL = len(TK), len(TB), L * L
+    n = FK * LL + FB
+    Mp, rp = np.zeros((n, n)), np.zeros(n)
+    for tb in range(FK):
+        for ab, lb in enumerate(lags):
+            kb = tb * LL + ab
+            Xb = Rhat[tb] * Khat[lb]
+            for t in range(FK):
+                for a, la in enumerate(lags):
+                    Mp[kb, t * LL + a] = np.sum((Xb * np.conj(Rhat[t]) * np.conj(Khat[la])).real)      # (19)
+            for s in range(FB):
+                Mp[kb, FK * LL + s] = np.sum((Xb * np.conj(That[s])).real)                              # (20)
+                Mp[FK * LL + s, kb] = np.sum((That[s] * np.conj(Rhat[tb]) * np.conj(Khat[lb])).real)    # (21)
+            rp[kb] = np.sum((np.conj(Shat) * Xb).real)                                                  # (23)
+    for sb in range(FB):
+        for s in range(FB):
+            Mp[FK * LL + sb, FK * LL + s] = np.sum((That[sb] * np.conj(That[s])).real)                  # (22)
+        rp[FK * LL + sb] = np.sum((np.conj(Shat) * That[sb]).real)                                      # (24)
+
+    for M, rhs in (oracle.normal_bruteforce(R, S, L, POLY, DK, DB), oracle.normal_from_lags(R, S, L, POLY, DK, DB)):
+        na = FK * LL
+        sc = np.r_[np.full(na, float(N) ** 1.5), np.full(FB, float(N) ** 0.5)]
+        Mo = M / np.outer(sc, sc)
+        ro = rhs / np.r_[np.full(na, float(N) ** 2), np.full(FB, float(N))]
+        scale = np.sqrt(np.outer(np.diag(Mp), np.diag(Mp)))
+        assert np.max(np.abs(Mo - Mp) / scale) < 1e-13
+        assert np.max(np.abs(ro - rp)) < 1e-13 * np.max(np.abs(rp))
+        c = oracle.solve(M, rhs)
+        cp = np.linalg.solve(Mp, rp)
+        np.testing.assert_allclose(cp[:na] / N, c[:na], rtol=0, atol=1e-9 * np.abs(c).max())
+        np.testing.assert_allclose(cp[na:], c[na:], rtol=0, atol=1e-9 * np.abs(c).max())
+
+
+# --------------------------------------------------------------------------- structure of M
+
+@pytest.mark.parametrize("H,W,L,basis,DK,DB", [(16, 12, 3, POLY, 1, 1), (12, 20, 5, POLY, 2, 1),
+                                              (24, 16, 3, BSPL, 0, 0), (16, 16, 5, POLY, 0, 2)])
+def test_tierB_equals_tierA_and_symmetric_psd(H, W, L, basis, DK, DB):
+    R, S = _rand_pair(H, W, 2)
+    MA, rA = oracle.normal_bruteforce(R, S, L, basis, DK, DB)
+    MB, rB = oracle.normal_from_lags(R, S, L, basis, DK, DB)
+    d = np.sqrt(np.diag(MA))
+    assert np.max(np.abs(MA - MB) / np.outer(d, d)) < 1e-13
+    assert np.max(np.abs(rA - rB)) < 1e-13 * np.max(np.abs(rA))
+    assert np.array_equal(MA, MA.T) and np.array_equal(MB, MB.T)
+    assert np.linalg.eigvalsh(MA / np.outer(d, d)).min() > -1e-12
+
+
+def test_tierA_vs_independent_numpy_design_matrix():
+    """Phi rebuilt with np.roll from Eqs. 3-4, 11 (independent of the C loops), M = Phi^T Phi via BLAS."""
+    H, W, L, DK, DB = 16, 20, 5, 2, 1
+    w = 2
+    R, S = _rand_pair(H, W, 3)
+    cols = []
+    for T in _poly_T(H, W, DK):
+        Rt = T * R
+        for al in range(-w, w + 1):
+            for be in range(-w, w + 1):
+                sh = np.roll(Rt, (al, be), axis=(0, 1))          # sh(x,y) = Rt(x-al, y-be)
+                cols.append((sh if (al, be) == (0, 0) else sh - Rt).ravel())
+    cols += [T.ravel() for T in _poly_T(H, W, DB)]
+    Phi = np.array(cols)
+    np.testing.assert_allclose(oracle.design_matrix(R, L, POLY, DK, DB), Phi, rtol=0, atol=1e-12)
+    M, rhs = oracle.normal_bruteforce(R, S, L, POLY, DK, DB)
+    np.testing.assert_allclose(M, Phi @ Phi.T, rtol=1e-12, atol=1e-6)
+    np.testing.assert_allclose(rhs, Phi @ S.ravel(), rtol=1e-12, atol=1e-6)
+
+
+def test_background_block_exact_rational():
+    """M_bb = products of power sums of the normalised coordinates, in exact Fractions;
+    rhs_b = image moments of S.  Catches wrong coordinates or term order in the background block."""
+    H, W, L, DB = 12, 8, 3, 2
+    R, S = _rand_pair(H, W, 4)
+    M, rhs = oracle.normal_from_lags(R, S, L, POLY, 0, DB)
+    ps = lambda N, k: sum((Fraction(2 * x + 1, N) - 1) ** k for x in range(N))
+    tb = _poly_terms(DB)
+    for a, (ib, jb) in enumerate(tb):
+        for b, (i, j) in enumerate(tb):
+            exact = float(ps(H, ib + i) * ps(W, jb + j))
+            assert abs(M[L * L + a, L * L + b] - exact) <= 1e-14 * max(1.0, abs(exact))
+        mom = np.sum(S * _u(H)[:, None] ** ib * _u(W)[None, :] ** jb)
+        assert abs(rhs[L * L + a] - mom) <= 1e-12 * np.abs(S).sum()
+
+
+def test_lag_symmetries():
+    H, W, L = 16, 12, 3
+    R, S = _rand_pair(H, W, 5)
+    t = oracle.lag_tables(R, S, L, POLY, 1, 1)
+    A, B = oracle.weighted_ref(R, POLY, 1, 0), oracle.weighted_ref(R, POLY, 1, 2)
+    for rho, eps in [(1, -2), (-2, 0), (0, 1), (2, 2)]:
+        q, c0 = oracle.corr_diff_one(A, B, rho, eps)
+        qr, c0r = oracle.corr_diff_one(B, A, -rho, -eps)
+        assert abs((q + c0) - (qr + c0r)) < 1e-9 * abs(c0)                       # Omega_ab(r) = Omega_ba(-r)
+        assert abs(q - t["Qom"][0, 2, rho + 2, eps + 2]) < 1e-9 * abs(c0)
+        direct = np.sum(A * np.roll(B, (-rho, -eps), axis=(0, 1)))                 # B(x+rho, y+eps)
+        assert abs((q + c0) - direct) < 1e-12 * abs(direct)
+    q00 = t["Qom"][0, 0]
+    np.testing.assert_allclose(q00, q00[::-1, ::-1], rtol=0, atol=1e-9 * t["Om0"][0, 0])   # Omega_tt even
+
+
+# --------------------------------------------------------------------------- solution
+
+def test_solve_vs_lapack_and_not_spd():
+    rng = np.random.default_rng(6)
+    X = rng.standard_normal((200, 40)) * np.logspace(0, 4, 40)[None, :]
+    M, c_true = X.T @ X, rng.standard_normal(40)
+    c = oracle.solve(M, M @ c_true)
+    np.testing.assert_allclose(c, np.linalg.solve(M, M @ c_true), rtol=1e-9, atol=1e-12)
+    np.testing.assert_allclose(c, c_true, rtol=1e-9, atol=1e-12)
+    M[5, 5] = -1.0
+    with pytest.raises(np.linalg.LinAlgError):
+        oracle.solve(M, M @ c_true)
+
+
+def test_solution_vs_lstsq_qr():
+    """c from the oracle's normal equations == QR/SVD least squares on Phi (never forms M)."""
+    H, W, L, DK, DB = 20, 16, 3, 1, 1
+    R, S = _rand_pair(H, W, 7)
+    Phi = oracle.design_matrix(R, L, POLY, DK, DB)
+    c_ls = np.linalg.lstsq(Phi.T, S.ravel(), rcond=None)[0]
+    c = oracle.solve(*oracle.normal_from_lags(R, S, L, POLY, DK, DB))
+    np.testing.assert_allclose(c, c_ls, rtol=0, atol=1e-10 * np.abs(c_ls).max())
+
+
+def test_identical_images_give_delta_kernel_and_zero_difference():
+    H, W, L = 16, 16, 5
+    R, _ = _rand_pair(H, W, 8)
+    c = oracle.solve(*oracle.normal_from_lags(R, R, L, POLY, 1, 1))
+    e = np.zeros_like(c); e[(L // 2) * L + L // 2] = 1.0
+    np.testing.assert_allclose(c, e, rtol=0, atol=1e-10)
+    assert np.abs(oracle.difference(R, R, c, L, POLY, 1, 1)).max() < 1e-9
+
+
+def test_shift_scale_constant_recovered():
+    """S = lam * R(x-1, y+1) + mu  =>  a_{0,centre} = lam (kernel sum), a_{0,(1,-1)} = lam, b_0 = mu, rest 0."""
+    H, W, L, lam, mu = 16, 20, 3, 1.1, 3.0
+    R, _ = _rand_pair(H, W, 9)
+    S = lam * np.roll(R, (1, -1), axis=(0, 1)) + mu
+    c = oracle.solve(*oracle.normal_from_lags(R, S, L, POLY, 1, 1))
+    expect = np.zeros_like(c)
+    expect[1 * L + 1] = lam                    # centre
+    expect[(1 + 1) * L + (-1 + 1)] = lam       # (alpha,beta) = (1,-1)
+    expect[3 * L * L] = mu
+    np.testing.assert_allclose(c, expect, rtol=0, atol=1e-9)
+
+
+def test_constant_kernel_is_textbook_circular_convolution():
+    """App. A: for DK=0 the model is an exact circular convolution.  S is made by
+    scipy.ndimage.convolve(mode='wrap'); the oracle must return that kernel, and its difference
+    routine must reproduce scipy's convolution."""
+    H, W, L = 24, 20, 5
+    rng = np.random.default_rng(10)
+    R, _ = _rand_pair(H, W, 10)
+    k = rng.random((L, L)); k[0, 3] = 0.9            # asymmetric on purpose
+    S = scipy.ndimage.convolve(R, k, mode="wrap") + 7.0
+    c = oracle.solve(*oracle.normal_from_lags(R, S, L, POLY, 0, 0))
+    kc = c[:L * L].reshape(L, L).copy()
+    ksum = kc[2, 2]
+    kc[2, 2] = ksum - (kc.sum() - ksum)              # Eqs. 3-4: centre coefficient is the kernel SUM
+    np.testing.assert_allclose(kc, k, rtol=0, atol=1e-9)
+    assert abs(ksum - k.sum()) < 1e-9 and abs(c[-1] - 7.0) < 1e-8
+    D = oracle.difference(R, np.zeros_like(R), c, L, POLY, 0, 0)
+    np.testing.assert_allclose(-D, S, rtol=0, atol=1e-9)
+
+
+@pytest.mark.parametrize("basis,DK,DB", [(POLY, 2, 1), (BSPL, 0, 0)])
+def test_injected_spatially_varying_model_recovered(basis, DK, DB):
+    """S = sum_t (T_t R) o k_t + sum_s b_s T'_s  built with scipy's wrap-convolution per term
+    (Eq. 12) from chosen kernels; the fit must return them (noiseless => exact)."""
+    H, W, L = 32, 28, 3
+    rng = np.random.default_rng(11)
+    R, _ = _rand_pair(H, W, 11)
+    if basis == POLY:
+        TK, TB = _poly_T(H, W, DK), _poly_T(H, W, DB)
+    else:
+        fx, gy = oracle.axis_table(BSPL, H, DK), oracle.axis_table(BSPL, W, DK)   # pinned to scipy above
+        TK = [np.outer(fx[i], gy[j]) for (i, j) in oracle.terms(BSPL, DK)]
+        TB = TK
+    ks = [rng.standard_normal((L, L)) * (1.0 if t == 0 else 0.2) for t in range(len(TK))]
+    bs = rng.standard_normal(len(TB))
+    S = sum(scipy.ndimage.convolve(T * R, k, mode="wrap") for T, k in zip(TK, ks)) + sum(b * T for b, T in zip(bs, TB))
+    c = oracle.solve(*oracle.normal_from_lags(R, S, L, basis, DK, DB))
+    LL = L * L
+    for t, k in enumerate(ks):
+        a = k.ravel().copy(); a[LL // 2] = k.sum()
+        np.testing.assert_allclose(c[t * LL:(t + 1) * LL], a, rtol=0, atol=2e-8)
+    np.testing.assert_allclose(c[len(TK) * LL:], bs, rtol=0, atol=1e-6)
+    D = oracle.difference(R, S, c, L, basis, DK, DB)
+    assert np.abs(D).max() < 1e-7
+
+
+def test_kernel_sum_property_with_delta_image():
+    """the kernel sum at a position is the K_00 coefficient field sum_t a_{t,00} T_t.
+    A delta image at (x0,y0) makes the model image equal the local kernel (weights at the source pixel)."""
+    H, W, L, DK = 16, 16, 3, 1
+    rng = np.random.default_rng(12)
+    n = oracle.num_unknowns(L, POLY, DK, 0)
+    c = rng.standard_normal(n); c[-1] = 0.0
+    x0, y0 = 5, 9
+    R = np.zeros((H, W)); R[x0, y0] = 1.0
+    model = -oracle.difference(R, np.zeros((H, W)), c, L, POLY, DK, 0)
+    T = [Tt[x0, y0] for Tt in _poly_T(H, W, DK)]
+    expect_sum = sum(c[t * L * L + L * L // 2] * T[t] for t in range(3))
+    assert abs(model.sum() - expect_sum) < 1e-12
+    a_off = sum(c[t * L * L + (1 + 1) * L + (0 + 1)] * T[t] for t in range(3))   # (alpha,beta) = (1,0)
+    assert abs(model[x0 + 1, y0] - a_off) < 1e-12
+
+
+def test_normal_equation_orthogonality_and_sampled_difference():
+    H, W, L = 20, 24, 5
+    R, S = _rand_pair(H, W, 13)
+    c = oracle.solve(*oracle.normal_from_lags(R, S, L, POLY, 1, 1))
+    D = oracle.difference(R, S, c, L, POLY, 1, 1)
+    Phi = oracle.design_matrix(R, L, POLY, 1, 1)
+    g = Phi @ D.ravel()
+    assert np.max(np.abs(g) / (np.linalg.norm(Phi, axis=1) * np.linalg.norm(D))) < 1e-11
+    px, py = np.array([0, 3, 19, 7]), np.array([0, 23, 11, 2])
+    np.testing.assert_allclose(oracle.difference_at(R, S, c, L, POLY, 1, 1, px, py), D[px, py], rtol=0, atol=1e-10)
+
+
+def test_affine_coordinate_invariance_of_difference():
+    """DESIGN g8: the total-degree polynomial space is affine invariant, so D fitted with raw pixel
+    indices (the paper's T = x^p y^q) equals D fitted with normalised coordinates."""
+    H, W, L, DK, DB = 16, 12, 3, 1, 1
+    R, S = _rand_pair(H, W, 14)
+    c = oracle.solve(*oracle.normal_from_lags(R, S, L, POLY, DK, DB))
+    D = oracle.difference(R, S, c, L, POLY, DK, DB)
+    x, y = np.arange(H)[:, None] * 1.0, np.arange(W)[None, :] * 1.0
+    raw = [x ** i * y ** j * np.ones((H, W)) for (i, j) in _poly_terms(1)]
+    cols = []
+    for T in raw:
+        Rt = T * R
+        for al in (-1, 0, 1):
+            for be in (-1, 0, 1):
+                sh = np.roll(Rt, (al, be), axis=(0, 1))
+                cols.append((sh if (al, be) == (0, 0) else sh - Rt).ravel())
+    cols += [T.ravel() for T in raw]
+    Phi = np.array(cols).T
+    c_raw = np.linalg.lstsq(Phi, S.ravel(), rcond=None)[0]
+    np.testing.assert_allclose(D.ravel(), S.ravel() - Phi @ c_raw, rtol=0, atol=1e-8)
