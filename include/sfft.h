@@ -1,0 +1,128 @@
+/*
+ * sfft.h -- C ABI of libsfft_b200: the data-parallel hot path of SFFT image differencing
+ * (arXiv 2109.09334, "Image Subtraction in Fourier Space") for NVIDIA B200 (sm_100a).
+ *
+ * Citations are "PAPER.md:<line>" (the paper's text) plus the equation; "DESIGN g#" refers
+ * to a reading of a garbled or silent passage listed in DESIGN.md.
+ *
+ * Problem (Eqs. 1-12).  Given a reference image R and a science image S,
+ * both N0 x N1 = H x W, find the coefficients of
+ *     D(x,y) = S(x,y) - sum_{t,(a,b)} a_{t,ab} (R^t o K_ab)(x,y) - sum_s b_s T'_s(x,y)       (Eq. 12)
+ * that minimise sum D^2, where o is circular convolution, R^t = T_t R, K_00 = delta,
+ * K_ab = delta(u-a,v-b) - delta(u,v) for (a,b) != (0,0), |a|,|b| <= w, L = 2w+1 (Eqs. 3-4),
+ * and T_t / T'_s are spatial weight functions of the kernel / background:
+ *   SFFT_BASIS_POLY    monomials u_x^i u_y^j, i+j <= DK (resp. DB)        (Eqs. 2, 6; DESIGN g8)
+ *                      of the normalised coordinates u_x = (2x+1)/H - 1, u_y = (2y+1)/W - 1
+ *   SFFT_BASIS_BSPLINE tensor products B_i(v_x) B_j(v_y) of cubic B-splines on a clamped
+ *                      knot vector with DK (resp. DB) uniform interior knots per axis,
+ *                      v_x = (x+0.5)/H, v_y = (y+0.5)/W                    (Eqs. 8-9; DESIGN g13)
+ *
+ * Layout and indices.  Images are row-major double [x][y], x in [0,H) slow, y in [0,W) fast;
+ * with nbatch > 1 they are [b][x][y] (independent pairs).  Lag index a = (alpha+w)*L + (beta+w),
+ * centre a0 = w*L+w.  Unknown k = t*L*L + a (kernel) or F_K*L*L + s (background);
+ * n = F_K*L*L + F_B.  POLY terms t <-> (i,j): i = 0..D outer, j = 0..D-i inner;
+ * BSPLINE terms t = i*(D+4) + j.  Coefficients are the real-space a-ring of the paper
+ * (the paper's a = N0 N1 a-ring), with the photometric scale free (DESIGN g9).
+ *
+ * All pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The caller owns every
+ * buffer, including the workspace; the plan owns only small constant tables.  Calls enqueue
+ * work on the plan's CUDA stream and return without synchronising unless stated.  Every call
+ * returns an SFFT_* status; nothing throws or aborts.  There is no CPU fallback: without a
+ * CUDA device every compute call returns SFFT_ERR_CUDA.
+ */
+#ifndef SFFT_H_
+#define SFFT_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sfft_plan sfft_plan; /* opaque host-side handle */
+
+enum { SFFT_BASIS_POLY = 0, SFFT_BASIS_BSPLINE = 1 };
+
+enum {
+    SFFT_OK = 0,
+    SFFT_ERR_INVALID_ARG = 1, /* bad size / null pointer / unsupported shape                */
+    SFFT_ERR_STATE = 2,       /* call order violated (e.g. solve before build)              */
+    SFFT_ERR_WORKSPACE = 3,   /* workspace missing or too small                              */
+    SFFT_ERR_CUDA = 4,        /* CUDA runtime error (message via sfft_last_cuda_error)       */
+    SFFT_ERR_NOT_SPD = 5      /* normal matrix not positive definite (rank-deficient input)  */
+};
+
+/* Create a plan for H x W images, L x L kernel (L odd), spatial orders DK / DB, given basis.
+ * POLY: DK, DB = total polynomial degree.  BSPLINE: DK, DB = number of uniform interior knots.
+ * Restrictions (INVALID_ARG otherwise): H, W powers of two with 32 <= H <= 8192, 64 <= W <= 8192; L odd, 1 <= L <= 33, 2L-1 <= min(H, W); DK, DB in [0, 8].
+ * Builds constant tables on the host and uploads them (synchronous). */
+int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int basis);
+
+/* Number of independent pairs processed per call (default 1).  Must precede set_workspace. */
+int sfft_plan_set_batch(sfft_plan *plan, int nbatch);
+
+/* CUDA stream (cudaStream_t cast to void*; NULL = legacy default stream). */
+int sfft_plan_set_stream(sfft_plan *plan, void *cuda_stream);
+
+/* n = F_K*L*L + F_B (Eq. 18's dimension), or -1 for a null plan. */
+int sfft_plan_num_unknowns(const sfft_plan *plan);
+int sfft_plan_num_kernel_terms(const sfft_plan *plan);     /* F_K */
+int sfft_plan_num_background_terms(const sfft_plan *plan); /* F_B */
+
+/* Bytes of device workspace the plan needs for its current batch size. */
+size_t sfft_plan_workspace_bytes(const sfft_plan *plan);
+
+/* Lend a device buffer (>= workspace_bytes, 256-byte aligned) to the plan.  The caller keeps
+ * ownership and must keep it alive until the plan is destroyed or another buffer is set. */
+int sfft_plan_set_workspace(sfft_plan *plan, void *d_ws, size_t bytes);
+
+/* Steps a1-a5: assemble the normal system of Eq. 18 in real-space scaling,
+ * M = Phi^T Phi, rhs = Phi^T S, from the pair (d_R, d_S), each [nbatch][H][W] double.
+ * Every block is a cross-correlation of weighted images evaluated by FFT and read at the
+ * kernel-lag offsets only (App. B).  Inputs are not modified. */
+int sfft_build_system(sfft_plan *plan, const double *d_R, const double *d_S);
+
+/* Device pointers to the assembled system (valid until the next build): M is [nbatch][n][ld]
+ * row-major, FULL symmetric (both triangles), ld = n; rhs is [nbatch][n].  For parity tests. */
+int sfft_get_system(const sfft_plan *plan, const double **d_M, const double **d_rhs, int *ld);
+
+/* Device pointer to the lag tables of the last build, for parity tests.  which: 0 = Omega
+ * [nbatch][npairs][2L-1][2L-1] over pairs (tb <= t) in row-major pair order, 1 = Theta
+ * [nbatch][F_K][L][L], 2 = Lambda [nbatch][F_K][F_B][L][L], 3 = Delta [nbatch][F_B].
+ * count receives the number of doubles per batch entry. */
+int sfft_get_lag_table(const sfft_plan *plan, int which, const double **d_table, size_t *count);
+
+/* Step a6: solve M c = rhs (Jacobi-scaled blocked FP64 Cholesky; DESIGN g11) and write
+ * c to d_coef [nbatch][n].  A non-positive pivot raises a device flag reported by
+ * sfft_plan_status as SFFT_ERR_NOT_SPD; d_coef is then undefined. */
+int sfft_solve(sfft_plan *plan, double *d_coef);
+
+/* Steps a7-a8: D = S - sum_t sum_ab k_{t,ab} R^t((x-a)%H,(y-b)%W) - sum_s b_s T'_s  (Eqs. 1, 12)
+ * with k the delta-basis coefficients folded back to pixel kernels (Eqs. 3-4).  (d_R, d_S)
+ * may differ from the fitted pair (fit on the masked pair, apply to the
+ * original).  d_D [nbatch][H][W] may alias d_S; no other aliasing. */
+int sfft_subtract(sfft_plan *plan, const double *d_coef, const double *d_R, const double *d_S, double *d_D);
+
+/* Synchronise the plan's stream and report numerical status.  On SFFT_ERR_NOT_SPD, *info =
+ * batch*n + index of the first failing pivot; otherwise *info = -1.  info may be NULL. */
+int sfft_plan_status(sfft_plan *plan, int *info);
+
+/* End-to-end convenience with HOST buffers: copies h_R, h_S ([nbatch][H][W]) to the device,
+ * runs build -> solve -> subtract, copies D and the coefficients back, synchronises.
+ * Needs the workspace (sfft_plan_workspace_bytes already includes the image staging area).
+ * h_D [nbatch][H][W], h_coef [nbatch][n] (either may be NULL to skip that copy). */
+int sfft_run_host(sfft_plan *plan, const double *h_R, const double *h_S, double *h_D, double *h_coef);
+
+/* Number of kernels the plan launched since creation (for bench accounting). */
+long sfft_plan_launch_count(const sfft_plan *plan);
+
+void sfft_plan_destroy(sfft_plan *plan);
+
+const char *sfft_strerror(int status);
+const char *sfft_last_cuda_error(const sfft_plan *plan);
+const char *sfft_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SFFT_H_ */

@@ -1,0 +1,269 @@
+"""Thin ctypes binding of libsfft_b200 (include/sfft.h): argument marshalling only.
+
+Functions carry the C names (sfft_plan_create, sfft_build_system, sfft_solve, sfft_subtract,
+sfft_plan_destroy, ...).  `Plan` bundles a handle with a torch-owned workspace; torch is used
+for device memory and the stream only -- every step of the path runs in the library's kernels.
+There is no CPU fallback: a missing library or a missing GPU raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+SFFT_BASIS_POLY, SFFT_BASIS_BSPLINE = 0, 1
+SFFT_OK, SFFT_ERR_INVALID_ARG, SFFT_ERR_STATE, SFFT_ERR_WORKSPACE, SFFT_ERR_CUDA, SFFT_ERR_NOT_SPD = range(6)
+
+# every symbol include/sfft.h declares (checked against the built library by tests/test_abi.py)
+EXPORTS = [
+    "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_num_unknowns",
+    "sfft_plan_num_kernel_terms", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
+    "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
+    "sfft_subtract", "sfft_plan_status", "sfft_run_host", "sfft_plan_launch_count", "sfft_plan_destroy",
+    "sfft_strerror", "sfft_last_cuda_error", "sfft_version",
+]
+
+_lib = None
+
+
+class SfftError(RuntimeError):
+    def __init__(self, status, where, detail=""):
+        self.status = status
+        msg = f"{where}: {sfft_strerror(status)}"
+        super().__init__(msg + (f" [{detail}]" if detail else ""))
+
+
+def library_path():
+    return _build.LIB
+
+
+def load_library(build_if_missing=True):
+    """dlopen libsfft_b200.so (building it with nvcc first if absent).  Raises if unavailable."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_build.LIB):
+        if not build_if_missing:
+            raise FileNotFoundError(f"{_build.LIB} is missing: run __graft_entry__.build()")
+        _build.build_library()
+    L = ctypes.CDLL(_build.LIB)
+    vp, ci, cs = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+    pvp, pci = ctypes.POINTER(ctypes.c_void_p), ctypes.POINTER(ctypes.c_int)
+    sig = {
+        "sfft_plan_create": (ci, [pvp, ci, ci, ci, ci, ci, ci]),
+        "sfft_plan_set_batch": (ci, [vp, ci]),
+        "sfft_plan_set_stream": (ci, [vp, vp]),
+        "sfft_plan_num_unknowns": (ci, [vp]),
+        "sfft_plan_num_kernel_terms": (ci, [vp]),
+        "sfft_plan_num_background_terms": (ci, [vp]),
+        "sfft_plan_workspace_bytes": (cs, [vp]),
+        "sfft_plan_set_workspace": (ci, [vp, vp, cs]),
+        "sfft_build_system": (ci, [vp, vp, vp]),
+        "sfft_get_system": (ci, [vp, pvp, pvp, pci]),
+        "sfft_get_lag_table": (ci, [vp, ci, pvp, ctypes.POINTER(cs)]),
+        "sfft_solve": (ci, [vp, vp]),
+        "sfft_subtract": (ci, [vp, vp, vp, vp, vp]),
+        "sfft_plan_status": (ci, [vp, pci]),
+        "sfft_run_host": (ci, [vp, vp, vp, vp, vp]),
+        "sfft_plan_launch_count": (ctypes.c_long, [vp]),
+        "sfft_plan_destroy": (None, [vp]),
+        "sfft_strerror": (ctypes.c_char_p, [ci]),
+        "sfft_last_cuda_error": (ctypes.c_char_p, [vp]),
+        "sfft_version": (ctypes.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+# ---- one Python function per C entry point (same names, same argument order) ----
+
+def sfft_strerror(status):
+    return load_library().sfft_strerror(int(status)).decode()
+
+
+def sfft_version():
+    return load_library().sfft_version().decode()
+
+
+def sfft_plan_create(H, W, L, DK, DB, basis):
+    h = ctypes.c_void_p()
+    st = load_library().sfft_plan_create(ctypes.byref(h), H, W, L, DK, DB, basis)
+    return st, h
+
+
+def sfft_plan_set_batch(plan, nbatch):
+    return load_library().sfft_plan_set_batch(plan, nbatch)
+
+
+def sfft_plan_set_stream(plan, stream_ptr):
+    return load_library().sfft_plan_set_stream(plan, ctypes.c_void_p(stream_ptr))
+
+
+def sfft_plan_num_unknowns(plan):
+    return load_library().sfft_plan_num_unknowns(plan)
+
+
+def sfft_plan_workspace_bytes(plan):
+    return load_library().sfft_plan_workspace_bytes(plan)
+
+
+def sfft_plan_set_workspace(plan, dptr, nbytes):
+    return load_library().sfft_plan_set_workspace(plan, ctypes.c_void_p(dptr), nbytes)
+
+
+def sfft_build_system(plan, d_R, d_S):
+    return load_library().sfft_build_system(plan, ctypes.c_void_p(d_R), ctypes.c_void_p(d_S))
+
+
+def sfft_get_system(plan):
+    M, r, ld = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_int()
+    st = load_library().sfft_get_system(plan, ctypes.byref(M), ctypes.byref(r), ctypes.byref(ld))
+    return st, M.value, r.value, ld.value
+
+
+def sfft_get_lag_table(plan, which):
+    t, cnt = ctypes.c_void_p(), ctypes.c_size_t()
+    st = load_library().sfft_get_lag_table(plan, which, ctypes.byref(t), ctypes.byref(cnt))
+    return st, t.value, cnt.value
+
+
+def sfft_solve(plan, d_coef):
+    return load_library().sfft_solve(plan, ctypes.c_void_p(d_coef))
+
+
+def sfft_subtract(plan, d_coef, d_R, d_S, d_D):
+    return load_library().sfft_subtract(plan, ctypes.c_void_p(d_coef), ctypes.c_void_p(d_R), ctypes.c_void_p(d_S),
+                                        ctypes.c_void_p(d_D))
+
+
+def sfft_plan_status(plan):
+    info = ctypes.c_int(-1)
+    st = load_library().sfft_plan_status(plan, ctypes.byref(info))
+    return st, info.value
+
+
+def sfft_run_host(plan, h_R, h_S, h_D, h_coef):
+    return load_library().sfft_run_host(plan, ctypes.c_void_p(h_R), ctypes.c_void_p(h_S), ctypes.c_void_p(h_D),
+                                        ctypes.c_void_p(h_coef))
+
+
+def sfft_plan_launch_count(plan):
+    return load_library().sfft_plan_launch_count(plan)
+
+
+def sfft_plan_destroy(plan):
+    load_library().sfft_plan_destroy(plan)
+
+
+def sfft_last_cuda_error(plan):
+    return load_library().sfft_last_cuda_error(plan).decode()
+
+
+# ---- convenience: a plan plus its torch-owned workspace ----
+
+def _basis_id(basis):
+    if isinstance(basis, str):
+        return {"poly": SFFT_BASIS_POLY, "bspline": SFFT_BASIS_BSPLINE}[basis]
+    return int(basis)
+
+
+class Plan:
+    """sfft_plan handle + workspace tensor on the current CUDA device and stream."""
+
+    def __init__(self, H, W, L, DK, DB, basis="poly", nbatch=1, device="cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise SfftError(SFFT_ERR_CUDA, "Plan", "no CUDA device: libsfft_b200 has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        st, self.h = sfft_plan_create(H, W, L, DK, DB, _basis_id(basis))
+        if st != SFFT_OK:
+            raise SfftError(st, "sfft_plan_create")
+        self.H, self.W, self.L, self.nbatch = H, W, L, nbatch
+        self._check(sfft_plan_set_batch(self.h, nbatch), "sfft_plan_set_batch")
+        self.n = sfft_plan_num_unknowns(self.h)
+        self.ws_bytes = sfft_plan_workspace_bytes(self.h)
+        self.ws = torch.empty(self.ws_bytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self.ws.data_ptr() + 255) & ~255
+        self._check(sfft_plan_set_workspace(self.h, ptr, self.ws_bytes), "sfft_plan_set_workspace")
+        self.stream = torch.cuda.current_stream(self.device)
+        self._check(sfft_plan_set_stream(self.h, self.stream.cuda_stream), "sfft_plan_set_stream")
+
+    def _check(self, st, where):
+        if st != SFFT_OK:
+            raise SfftError(st, where, sfft_last_cuda_error(self.h) if st == SFFT_ERR_CUDA else "")
+
+    def _img(self, t):
+        torch = self.torch
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+        assert t.numel() == self.nbatch * self.H * self.W
+        return t.data_ptr()
+
+    def _ws_view(self, ptr, shape):
+        """Clone of `shape` doubles at device pointer `ptr`, which lies inside the torch-owned workspace."""
+        off, nbytes = ptr - self.ws.data_ptr(), int(np.prod(shape)) * 8
+        assert 0 <= off and off + nbytes <= self.ws.numel()
+        return self.ws[off:off + nbytes].view(self.torch.float64).reshape(shape).clone()
+
+    def build_system(self, R, S):
+        self._check(sfft_build_system(self.h, self._img(R), self._img(S)), "sfft_build_system")
+
+    def solve(self, coef=None):
+        torch = self.torch
+        if coef is None:
+            coef = torch.empty((self.nbatch, self.n), dtype=torch.float64, device=self.device)
+        self._check(sfft_solve(self.h, coef.data_ptr()), "sfft_solve")
+        return coef
+
+    def subtract(self, coef, R, S, D=None):
+        torch = self.torch
+        if D is None:
+            D = torch.empty_like(S)
+        self._check(sfft_subtract(self.h, coef.data_ptr(), self._img(R), self._img(S), self._img(D)), "sfft_subtract")
+        return D
+
+    def status(self, check=True):
+        st, info = sfft_plan_status(self.h)
+        if check and st != SFFT_OK:
+            raise SfftError(st, "sfft_plan_status", f"info={info}")
+        return st, info
+
+    def system(self):
+        """Copies of (M [b][n][n], rhs [b][n]) as torch tensors (parity tests)."""
+        st, pM, pr, ld = sfft_get_system(self.h)
+        self._check(st, "sfft_get_system")
+        self.status()
+        return self._ws_view(pM, (self.nbatch, self.n, ld)), self._ws_view(pr, (self.nbatch, self.n))
+
+    def lag_table(self, which):
+        st, pt, cnt = sfft_get_lag_table(self.h, which)
+        self._check(st, "sfft_get_lag_table")
+        self.status()
+        return self._ws_view(pt, (cnt,))
+
+    def run_host(self, R_host, S_host):
+        """End to end with host (numpy) buffers through sfft_run_host.  Returns (D, coef) numpy arrays."""
+        D = np.empty_like(R_host)
+        coef = np.empty((self.nbatch, self.n))
+        st = sfft_run_host(self.h, R_host.ctypes.data, S_host.ctypes.data, D.ctypes.data, coef.ctypes.data)
+        self._check(st, "sfft_run_host")
+        return D, coef
+
+    def launch_count(self):
+        return sfft_plan_launch_count(self.h)
+
+    def close(self):
+        if getattr(self, "h", None):
+            sfft_plan_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,150 @@
+// Step a1+a2 (row half): fused y-weighting + real-to-complex FFT along the fast axis.
+//
+// For every image row x the kernel forms the nKa y-weighted rows g_j(y) R(x,y) (the y-factor
+// of the weight T_t = f_i(x) g_j(y); the x-factor f_i(x) is constant along the
+// row and is applied later, in the x-direction correlation) plus the row of S, and writes
+// their length-W DFTs  r(x,m) = sum_y a(y) exp(-2 pi i m y / W),  m = 0..W/2.
+// Layout of the spectrum stack: rhat[b][img][x][m], m in [0, W/2) complex double, with the
+// (real) DC and Nyquist bins packed into slot m = 0 as (X[0], X[W/2]).
+//
+// A real row of length W is transformed as a complex FFT of length W/2 (Stockham autosort,
+// radix-4 passes plus one radix-2 pass when log2 is odd, ping-pong in shared memory)
+// followed by the even/odd split.  HBM-bound: one 16-byte load and one 16-byte store per
+// complex point, both fully coalesced.
+#include "sfft_internal.h"
+
+namespace sfft {
+namespace {
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+
+// One Stockham pass of radix R over N points held in shared memory (forward transform).
+// tw[k] = exp(-2 pi i k / (2N)) (the plan's W-point table, W = 2N), so exp(-2 pi i q / N) = tw[2q].
+template <int N, int T, int R>
+__device__ __forceinline__ void stockham_pass(const double2 *__restrict__ in, double2 *__restrict__ out, int Ns,
+                                              const double2 *__restrict__ tw) {
+    for (int j = threadIdx.x; j < N / R; j += T) {
+        const int k = j & (Ns - 1);
+        double2 v[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) v[r] = in[j + r * (N / R)];
+        if (Ns > 1) {
+            const int step = 2 * (N / (Ns * R)) * k;   // index of exp(-2 pi i k /(Ns R)) in the W-point table
+#pragma unroll
+            for (int r = 1; r < R; ++r) v[r] = cmul(v[r], __ldg(&tw[r * step]));
+        }
+        const int j0 = (j - k) * R + k;
+        if (R == 4) {
+            double2 t0 = make_double2(v[0].x + v[2].x, v[0].y + v[2].y);
+            double2 t1 = make_double2(v[0].x - v[2].x, v[0].y - v[2].y);
+            double2 t2 = make_double2(v[1].x + v[3].x, v[1].y + v[3].y);
+            double2 d = make_double2(v[1].x - v[3].x, v[1].y - v[3].y);
+            double2 t3 = make_double2(d.y, -d.x);   // -i * (v1 - v3)
+            out[j0] = make_double2(t0.x + t2.x, t0.y + t2.y);
+            out[j0 + Ns] = make_double2(t1.x + t3.x, t1.y + t3.y);
+            out[j0 + 2 * Ns] = make_double2(t0.x - t2.x, t0.y - t2.y);
+            out[j0 + 3 * Ns] = make_double2(t1.x - t3.x, t1.y - t3.y);
+        } else {
+            out[j0] = make_double2(v[0].x + v[1].x, v[0].y + v[1].y);
+            out[j0 + Ns] = make_double2(v[0].x - v[1].x, v[0].y - v[1].y);
+        }
+    }
+}
+
+template <int N>
+struct Log2 { static constexpr int value = 1 + Log2<N / 2>::value; };
+template <>
+struct Log2<1> { static constexpr int value = 0; };
+
+// Forward complex FFT of N points in shared memory; returns the buffer holding the result.
+template <int N, int T>
+__device__ __forceinline__ double2 *fft_smem_forward(double2 *a, double2 *b, const double2 *__restrict__ tw) {
+    constexpr int LOG = Log2<N>::value;
+    int Ns = 1;
+    double2 *in = a, *out = b;
+#pragma unroll
+    for (int s = 0; s < LOG / 2; ++s) {
+        stockham_pass<N, T, 4>(in, out, Ns, tw);
+        __syncthreads();
+        Ns *= 4;
+        double2 *t = in; in = out; out = t;
+    }
+    if (LOG & 1) {
+        stockham_pass<N, T, 2>(in, out, Ns, tw);
+        __syncthreads();
+        double2 *t = in; in = out; out = t;
+    }
+    return in;
+}
+
+// grid: x = image slot (0..nKa-1: weighted R rows, nKa: S), y = row, z = batch entry
+template <int NH, int T>
+__global__ void __launch_bounds__(T) k_rowfft_forward(const double *__restrict__ R, const double *__restrict__ S,
+                                                      const double *__restrict__ gK, const double2 *__restrict__ twW,
+                                                      double2 *__restrict__ rhat, int H, int nKa) {
+    extern __shared__ double2 sm[];
+    double2 *a = sm, *b = sm + NH;
+    constexpr int W = 2 * NH;
+    const int img = blockIdx.x, x = blockIdx.y, bz = blockIdx.z;
+    const double2 *src = reinterpret_cast<const double2 *>((img < nKa ? R : S) + ((size_t)bz * H + x) * W);
+    if (img < nKa) {
+        const double2 *g = reinterpret_cast<const double2 *>(gK + (size_t)img * W);
+        for (int i = threadIdx.x; i < NH; i += T) {
+            double2 v = __ldg(&src[i]), gg = __ldg(&g[i]);
+            a[i] = make_double2(v.x * gg.x, v.y * gg.y);    // z[n] = a[2n] + i a[2n+1]
+        }
+    } else {
+        for (int i = threadIdx.x; i < NH; i += T) a[i] = __ldg(&src[i]);
+    }
+    __syncthreads();
+    const double2 *Z = fft_smem_forward<NH, T>(a, b, twW);
+    double2 *dst = rhat + (((size_t)bz * (nKa + 1) + img) * H + x) * NH;
+    // even/odd split: E = (Z[k] + conj Z[NH-k])/2, O = (Z[k] - conj Z[NH-k])/(2i), X[k] = E + w^k O,
+    // X[NH-k] = conj(E - w^k O), w = exp(-2 pi i / W)
+    for (int k = threadIdx.x; k <= NH / 2; k += T) {
+        if (k == 0) {
+            double2 z0 = Z[0];
+            dst[0] = make_double2(z0.x + z0.y, z0.x - z0.y);   // (X[0], X[W/2]) packed
+        } else {
+            double2 zk = Z[k], zn = Z[NH - k];
+            double2 E = make_double2(0.5 * (zk.x + zn.x), 0.5 * (zk.y - zn.y));
+            double2 O = make_double2(0.5 * (zk.y + zn.y), -0.5 * (zk.x - zn.x));
+            double2 wO = cmul(__ldg(&twW[k]), O);
+            dst[k] = make_double2(E.x + wO.x, E.y + wO.y);
+            if (k != NH - k) dst[NH - k] = make_double2(E.x - wO.x, -(E.y - wO.y));
+        }
+    }
+}
+
+template <int NH>
+cudaError_t launch_fwd(sfft_plan *p, const double *dR, const double *dS) {
+    constexpr int T = NH >= 1024 ? 256 : (NH >= 256 ? 128 : 64);
+    size_t smem = 2 * (size_t)NH * sizeof(double2);
+    auto kern = k_rowfft_forward<NH, T>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid(p->nimg, p->H, p->nbatch);
+    kern<<<grid, T, smem, p->stream>>>(dR, dS, p->dt.gK, p->dt.twW, p->rhat, p->H, p->nKa);
+    p->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_rowfft_forward(sfft_plan *p, const double *dR, const double *dS) {
+    switch (p->Nh) {
+        case 32: return launch_fwd<32>(p, dR, dS);
+        case 64: return launch_fwd<64>(p, dR, dS);
+        case 128: return launch_fwd<128>(p, dR, dS);
+        case 256: return launch_fwd<256>(p, dR, dS);
+        case 512: return launch_fwd<512>(p, dR, dS);
+        case 1024: return launch_fwd<1024>(p, dR, dS);
+        case 2048: return launch_fwd<2048>(p, dR, dS);
+        case 4096: return launch_fwd<4096>(p, dR, dS);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace sfft
