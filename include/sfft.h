@@ -54,7 +54,8 @@ enum {
 
 /* Create a plan for H x W images, L x L kernel (L odd), spatial orders DK / DB, given basis.
  * POLY: DK, DB = total polynomial degree.  BSPLINE: DK, DB = number of uniform interior knots.
- * Restrictions (INVALID_ARG otherwise): H, W powers of two with 32 <= H <= 8192, 64 <= W <= 8192; L odd, 1 <= L <= 33, 2L-1 <= min(H, W); DK, DB in [0, 8].
+ * Restrictions (INVALID_ARG otherwise): H, W powers of two with 32 <= H <= 8192 and
+ * 64 <= W <= 8192; L odd, 1 <= L <= 33, 2L-1 <= min(H, W); DK, DB in [0, 8].
  * Builds constant tables on the host and uploads them (synchronous). */
 int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int basis);
 
@@ -112,6 +113,17 @@ int sfft_plan_status(sfft_plan *plan, int *info);
  * Needs the workspace (sfft_plan_workspace_bytes already includes the image staging area).
  * h_D [nbatch][H][W], h_coef [nbatch][n] (either may be NULL to skip that copy). */
 int sfft_run_host(sfft_plan *plan, const double *h_R, const double *h_S, double *h_D, double *h_coef);
+
+/* Per-stage device timing.  sfft_plan_profile(plan, nsteps) with nsteps > 0 makes the next nsteps
+ * build/solve/subtract rounds record CUDA events on the plan's stream around each stage (no host
+ * synchronisation; 0 disables).  sfft_plan_profile_read synchronises the stream and writes
+ * ms[step][SFFT_NUM_STAGES] (row-major; -1 where a stage did not run) for the *nrecorded steps seen.
+ * Stage order: 0 row FFT (a1+a2), 1 lag correlation (a3+a4), 2 column reduction to lag tables (a4),
+ * 3 lag gather (a5), 4 solve (a6), 5 kernel folding + per-row coefficient table (a7), 6 convolve-and-
+ * subtract (a7+a8). */
+#define SFFT_NUM_STAGES 7
+int sfft_plan_profile(sfft_plan *plan, int nsteps);
+int sfft_plan_profile_read(sfft_plan *plan, double *ms, int *nrecorded);
 
 /* Number of kernels the plan launched since creation (for bench accounting). */
 long sfft_plan_launch_count(const sfft_plan *plan);

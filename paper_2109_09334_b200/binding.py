@@ -21,8 +21,10 @@ EXPORTS = [
     "sfft_plan_num_kernel_terms", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
     "sfft_subtract", "sfft_plan_status", "sfft_run_host", "sfft_plan_launch_count", "sfft_plan_destroy",
-    "sfft_strerror", "sfft_last_cuda_error", "sfft_version",
+    "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
 ]
+SFFT_NUM_STAGES = 7
+STAGE_NAMES = ["rowfft", "corr", "lagsum", "gather", "solve", "subtract_prep", "subtract"]
 
 _lib = None
 
@@ -71,6 +73,8 @@ def load_library(build_if_missing=True):
         "sfft_strerror": (ctypes.c_char_p, [ci]),
         "sfft_last_cuda_error": (ctypes.c_char_p, [vp]),
         "sfft_version": (ctypes.c_char_p, []),
+        "sfft_plan_profile": (ci, [vp, ci]),
+        "sfft_plan_profile_read": (ci, [vp, vp, pci]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -153,6 +157,17 @@ def sfft_run_host(plan, h_R, h_S, h_D, h_coef):
 
 def sfft_plan_launch_count(plan):
     return load_library().sfft_plan_launch_count(plan)
+
+
+def sfft_plan_profile(plan, nsteps):
+    return load_library().sfft_plan_profile(plan, nsteps)
+
+
+def sfft_plan_profile_read(plan, nsteps):
+    ms = np.zeros((nsteps, SFFT_NUM_STAGES))
+    nrec = ctypes.c_int(0)
+    st = load_library().sfft_plan_profile_read(plan, ms.ctypes.data, ctypes.byref(nrec))
+    return st, ms[:nrec.value]
 
 
 def sfft_plan_destroy(plan):
@@ -253,6 +268,14 @@ class Plan:
         st = sfft_run_host(self.h, R_host.ctypes.data, S_host.ctypes.data, D.ctypes.data, coef.ctypes.data)
         self._check(st, "sfft_run_host")
         return D, coef
+
+    def profile(self, nsteps):
+        self._check(sfft_plan_profile(self.h, nsteps), "sfft_plan_profile")
+
+    def profile_read(self, nsteps):
+        st, ms = sfft_plan_profile_read(self.h, nsteps)
+        self._check(st, "sfft_plan_profile_read")
+        return ms
 
     def launch_count(self):
         return sfft_plan_launch_count(self.h)

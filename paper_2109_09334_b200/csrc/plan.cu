@@ -10,6 +10,14 @@
 
 using namespace sfft;
 
+namespace sfft {
+// record profiling mark `m` of the current step on the plan's stream (no-op unless profiling)
+void prof_mark(sfft_plan *p, int m) {
+    if (p->prof_steps <= 0 || p->prof_cur < 0 || p->prof_cur >= p->prof_steps) return;
+    cudaEventRecord(p->prof_events[(size_t)p->prof_cur * kProfMarks + m], p->stream);
+}
+}  // namespace sfft
+
 namespace {
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
@@ -314,12 +322,50 @@ int sfft_build_system(sfft_plan *p, const double *d_R, const double *d_S) {
     if (!p->ws) return SFFT_ERR_WORKSPACE;
     p->built = p->solved = false;
     cudaError_t e = cudaMemsetAsync(p->flag, 0xff, sizeof(int) * 2 * p->nbatch, p->stream);  // -1 = no failure
+    if (p->prof_steps > 0) p->prof_cur = p->prof_cur + 1;   // a build opens the next profiled step
+    prof_mark(p, 0);
     if (e == cudaSuccess) e = launch_rowfft_forward(p, d_R, d_S);
+    prof_mark(p, 1);
     if (e == cudaSuccess) e = launch_corr(p);
+    prof_mark(p, 2);
     if (e == cudaSuccess) e = launch_lagsum(p);
+    prof_mark(p, 3);
     if (e == cudaSuccess) e = launch_gather(p);
+    prof_mark(p, 4);
     if (e != cudaSuccess) return fail_cuda(p, e);
     p->built = true;
+    return SFFT_OK;
+}
+
+int sfft_plan_profile(sfft_plan *p, int nsteps) {
+    if (!p || nsteps < 0 || nsteps > 4096) return SFFT_ERR_INVALID_ARG;
+    for (cudaEvent_t ev : p->prof_events) cudaEventDestroy(ev);
+    p->prof_events.clear();
+    p->prof_steps = nsteps; p->prof_cur = -1;
+    for (int i = 0; i < nsteps * kProfMarks; ++i) {
+        cudaEvent_t ev;
+        if (cudaEventCreate(&ev) != cudaSuccess) return fail_cuda(p, cudaGetLastError());
+        p->prof_events.push_back(ev);
+    }
+    return SFFT_OK;
+}
+
+int sfft_plan_profile_read(sfft_plan *p, double *ms, int *nrecorded) {
+    if (!p || !ms) return SFFT_ERR_INVALID_ARG;
+    cudaError_t e = cudaStreamSynchronize(p->stream);
+    if (e != cudaSuccess) return fail_cuda(p, e);
+    int nrec = std::min(p->prof_cur + 1, p->prof_steps);
+    if (nrecorded) *nrecorded = nrec;
+    // stages: 0 rowfft, 1 corr, 2 lagsum, 3 gather, 4 solve, 5 subtract-prep, 6 subtract
+    static const int from[SFFT_NUM_STAGES] = {0, 1, 2, 3, 5, 7, 8}, to[SFFT_NUM_STAGES] = {1, 2, 3, 4, 6, 8, 9};
+    for (int s = 0; s < nrec; ++s)
+        for (int g = 0; g < SFFT_NUM_STAGES; ++g) {
+            float t = 0.f;
+            cudaError_t q = cudaEventElapsedTime(&t, p->prof_events[(size_t)s * kProfMarks + from[g]],
+                                                 p->prof_events[(size_t)s * kProfMarks + to[g]]);
+            ms[(size_t)s * SFFT_NUM_STAGES + g] = (q == cudaSuccess) ? (double)t : -1.0;
+            if (q != cudaSuccess) cudaGetLastError();
+        }
     return SFFT_OK;
 }
 
@@ -345,7 +391,9 @@ int sfft_get_lag_table(const sfft_plan *p, int which, const double **d_table, si
 int sfft_solve(sfft_plan *p, double *d_coef) {
     if (!p || !d_coef) return SFFT_ERR_INVALID_ARG;
     if (!p->built) return SFFT_ERR_STATE;
+    prof_mark(p, 5);
     cudaError_t e = launch_solve(p, d_coef);
+    prof_mark(p, 6);
     if (e != cudaSuccess) return fail_cuda(p, e);
     p->solved = true;
     return SFFT_OK;
@@ -354,7 +402,9 @@ int sfft_solve(sfft_plan *p, double *d_coef) {
 int sfft_subtract(sfft_plan *p, const double *d_coef, const double *d_R, const double *d_S, double *d_D) {
     if (!p || !d_coef || !d_R || !d_S || !d_D) return SFFT_ERR_INVALID_ARG;
     if (!p->ws) return SFFT_ERR_WORKSPACE;
+    prof_mark(p, 7);
     cudaError_t e = launch_subtract(p, d_coef, d_R, d_S, d_D);
+    prof_mark(p, 9);
     if (e != cudaSuccess) return fail_cuda(p, e);
     return SFFT_OK;
 }
@@ -398,6 +448,7 @@ long sfft_plan_launch_count(const sfft_plan *p) { return p ? p->launches : -1; }
 
 void sfft_plan_destroy(sfft_plan *p) {
     if (!p) return;
+    for (cudaEvent_t ev : p->prof_events) cudaEventDestroy(ev);
     free_tables(p);
     delete p;
 }

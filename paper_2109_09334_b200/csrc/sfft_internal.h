@@ -10,6 +10,7 @@
 
 namespace sfft {
 
+constexpr int kProfMarks = 10;   // event marks per profiled step (see sfft_plan_profile_read)
 constexpr int kMaxTile = 4;     // sequences per side of a correlation job tile
 constexpr int kColsPerCta = 8;  // spectrum columns (m) per CTA in the correlation kernel
 
@@ -68,6 +69,8 @@ struct sfft_plan {
     cudaStream_t stream = nullptr;
     bool built = false, solved = false;
     long launches = 0;
+    int prof_steps = 0, prof_cur = -1;          // stage profiling (sfft_plan_profile)
+    std::vector<cudaEvent_t> prof_events;       // [prof_steps][kProfMarks]
     std::string cuda_err;
 };
 
@@ -79,5 +82,6 @@ cudaError_t launch_lagsum(sfft_plan *p);
 cudaError_t launch_gather(sfft_plan *p);
 cudaError_t launch_solve(sfft_plan *p, double *d_coef);
 int subtract_tap_width(int L);
+void prof_mark(sfft_plan *p, int mark);
 cudaError_t launch_subtract(sfft_plan *p, const double *d_coef, const double *dR, const double *dS, double *dD);
 }  // namespace sfft

@@ -1,0 +1,203 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json's, in the DESIGN g16 reading:
+  matrix   |dM_kk'| <= 1e-10 sqrt(M_kk M_k'k')      rhs |d rhs_k| <= 1e-10 sqrt(M_kk sum S^2)
+  solution max|dc| <= 1e-8 max|c| per block (kernel, background)
+  D        max|dD| <= 1e-6 sigma,  sigma = sqrt(sky + read^2) = sqrt(125) ADU
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2109_09334_b200 import binding as B
+from paper_2109_09334_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_M, TOL_C, TOL_D = 1e-10, 1e-8, 1e-6
+
+
+def _bid(basis):
+    return oracle.POLY if basis == "poly" else oracle.BSPLINE
+
+
+def _oracle_all(R, S, L, basis, DK, DB):
+    bid = _bid(basis)
+    M, rhs = oracle.normal_from_lags(R, S, L, bid, DK, DB)
+    c = oracle.solve(M, rhs)
+    D = oracle.difference(R, S, c, L, bid, DK, DB)
+    return M, rhs, c, D
+
+
+def _check_system(M, rhs, Mo, ro, S):
+    d = np.sqrt(np.diag(Mo))
+    assert np.max(np.abs(M - Mo) / np.outer(d, d)) <= TOL_M
+    assert np.max(np.abs(rhs - ro) / (d * np.sqrt(np.sum(S * S)))) <= TOL_M
+    assert np.array_equal(M, M.T)
+
+
+def _check_coef(c, co, na):
+    assert np.max(np.abs(c[:na] - co[:na])) <= TOL_C * np.max(np.abs(co[:na]))
+    assert np.max(np.abs(c[na:] - co[na:])) <= TOL_C * np.max(np.abs(co[na:]))
+
+
+def _gpu_all(torch, p, L, basis, DK, DB, R=None, S=None):
+    R = p.R if R is None else R
+    S = p.S if S is None else S
+    nb = 1 if R.ndim == 2 else R.shape[0]
+    H, W = R.shape[-2:]
+    plan = B.Plan(H, W, L, DK, DB, basis, nbatch=nb)
+    dR, dS = torch.from_numpy(np.ascontiguousarray(R)).cuda(), torch.from_numpy(np.ascontiguousarray(S)).cuda()
+    plan.build_system(dR, dS)
+    coef = plan.solve()
+    D = plan.subtract(coef, dR, dS)
+    plan.status()
+    M, rhs = plan.system()
+    out = M.cpu().numpy(), rhs.cpu().numpy(), coef.cpu().numpy(), D.cpu().numpy()
+    plan.close()
+    return out
+
+
+CASES = [
+    # (config, H, W, L, basis, DK, DB)  -- None = the config's own value
+    (1, None, None, None, None, None, None),          # config 1 as specified
+    (2, 256, 256, None, None, None, None),            # config-2 recipe, several row tiles, L=11
+    (2, 128, 512, 5, None, None, None),               # non-square
+    (3, 64, 256, 15, None, None, None),               # 2L-1 = 29 lags on a small frame (wrap-heavy)
+    (4, 256, 128, 17, None, None, None),              # L=17 taps
+    (2, 64, 64, 1, None, 2, 1),                       # L=1: no kernel lags, only scale + background
+    (2, 64, 8192, 3, None, 0, 0),                     # longest row FFT (W=8192), constant kernel
+    (2, 128, 128, 9, None, 1, 2),                     # L without an exact subtract instantiation (padded taps)
+    (5, 128, 128, 5, "bspline", 1, 0),                # B-spline weights
+    (5, 256, 256, 5, "bspline", 4, 4),                # config-5 basis (8x8 functions), n = 1664
+]
+
+
+@pytest.mark.parametrize("cfg,H,W,L,basis,DK,DB", CASES)
+def test_parity_small(cuda_device, cfg, H, W, L, basis, DK, DB):
+    import torch
+    p = synth.make_pair(cfg, H=H, W=W)
+    L = p.L if L is None else L
+    basis = p.basis if basis is None else basis
+    DK = p.DK if DK is None else DK
+    DB = p.DB if DB is None else DB
+    Mo, ro, co, Do = _oracle_all(p.R, p.S, L, basis, DK, DB)
+    M, rhs, c, D = _gpu_all(torch, p, L, basis, DK, DB)
+    _check_system(M[0], rhs[0], Mo, ro, p.S)
+    _check_coef(c[0], co, Mo.shape[0] - oracle.num_terms(_bid(basis), DB))
+    assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
+
+
+def test_parity_config2_full(cuda_device):
+    import torch
+    p = synth.make_pair(2)
+    Mo, ro, co, Do = _oracle_all(p.R, p.S, p.L, p.basis, p.DK, p.DB)
+    M, rhs, c, D = _gpu_all(torch, p, p.L, p.basis, p.DK, p.DB)
+    _check_system(M[0], rhs[0], Mo, ro, p.S)
+    _check_coef(c[0], co, 6 * p.L * p.L)
+    assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_parity_full_size(cuda_device, cfg):
+    """Configs 3 and 4 at BASELINE.json's full size, in the launch configuration bench.py times.
+    The oracle's full direct-sum system takes about a minute or two of host time per config."""
+    import torch
+    p = synth.make_pair(cfg)
+    bid = oracle.POLY
+    Mo, ro = oracle.normal_from_lags(p.R, p.S, p.L, bid, p.DK, p.DB)
+    co = oracle.solve(Mo, ro)
+    M, rhs, c, D = _gpu_all(torch, p, p.L, p.basis, p.DK, p.DB)
+    _check_system(M[0], rhs[0], Mo, ro, p.S)
+    _check_coef(c[0], co, 6 * p.L * p.L)
+    rng = np.random.default_rng(cfg)
+    px = np.r_[rng.integers(0, p.H, 4000), [0, 0, p.H - 1, p.H - 1, 3, p.H - 2]]       # random + corners/borders
+    py = np.r_[rng.integers(0, p.W, 4000), [0, p.W - 1, 0, p.W - 1, p.W - 4, 5]]
+    Dref = oracle.difference_at(p.R, p.S, co, p.L, bid, p.DK, p.DB, px, py)
+    assert np.max(np.abs(D[px, py] - Dref)) <= TOL_D * p.sigma
+
+
+def test_batch_matches_single(cuda_device):
+    """nbatch = 3 independent pairs in one call: each entry equals the oracle on that pair."""
+    import torch
+    pb = synth.make_batch(5, nbatch=3, H=128, W=128)
+    L, DK, DB = 5, 1, 1
+    M, rhs, c, D = _gpu_all(torch, pb, L, "bspline", DK, DB)
+    for e in range(3):
+        Mo, ro, co, Do = _oracle_all(pb.R[e], pb.S[e], L, "bspline", DK, DB)
+        _check_system(M[e], rhs[e], Mo, ro, pb.S[e])
+        _check_coef(c[e], co, Mo.shape[0] - 25)
+        assert np.max(np.abs(D[e] - Do)) <= TOL_D * pb.sigma
+
+
+def test_identical_images(cuda_device):
+    """S = R  =>  a_{0,centre} = 1, everything else 0, D = 0 (degenerate but full-rank case)."""
+    import torch
+    p = synth.make_pair(1)
+    M, rhs, c, D = _gpu_all(torch, p, 5, "poly", 1, 1, R=p.R, S=p.R.copy())
+    e = np.zeros_like(c[0]); e[12] = 1.0
+    assert np.max(np.abs(c[0] - e)) <= 1e-9
+    assert np.max(np.abs(D)) <= TOL_D * p.sigma
+
+
+def test_fit_on_one_pair_apply_to_another_and_inplace(cuda_device):
+    """solve on the masked pair, apply to the original pair; D may alias S."""
+    import torch
+    p = synth.make_pair(1)
+    mask = np.ones_like(p.R); mask[40:60, 30:50] = 0.0
+    Rm, Sm = p.R * mask + 100.0 * (1 - mask), p.S * mask + 100.0 * (1 - mask)
+    Mo, ro = oracle.normal_from_lags(Rm, Sm, p.L, oracle.POLY, p.DK, p.DB)
+    co = oracle.solve(Mo, ro)
+    Do = oracle.difference(p.R, p.S, co, p.L, oracle.POLY, p.DK, p.DB)
+    plan = B.Plan(p.H, p.W, p.L, p.DK, p.DB, "poly")
+    plan.build_system(torch.from_numpy(Rm).cuda(), torch.from_numpy(Sm).cuda())
+    coef = plan.solve()
+    dR, dS = torch.from_numpy(p.R).cuda(), torch.from_numpy(p.S).cuda()
+    out = plan.subtract(coef, dR, dS, D=dS)      # in place
+    plan.status()
+    assert out.data_ptr() == dS.data_ptr()
+    assert np.max(np.abs(dS.cpu().numpy() - Do)) <= TOL_D * p.sigma
+    plan.close()
+
+
+def test_run_host_end_to_end(cuda_device):
+    p = synth.make_pair(1)
+    _, _, co, Do = _oracle_all(p.R, p.S, p.L, p.basis, p.DK, p.DB)
+    plan = B.Plan(p.H, p.W, p.L, p.DK, p.DB, p.basis)
+    D, c = plan.run_host(p.R, p.S)
+    _check_coef(c[0], co, 3 * p.L * p.L)
+    assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
+    assert plan.launch_count() > 0
+    plan.close()
+
+
+def test_rank_deficient_input_reports_not_spd(cuda_device):
+    """DESIGN g11: a constant reference makes the shifted-difference columns vanish -> M singular."""
+    import torch
+    plan = B.Plan(64, 64, 3, 0, 0, "poly")
+    R = torch.full((64, 64), 100.0, dtype=torch.float64, device="cuda")
+    S = torch.rand((64, 64), dtype=torch.float64, device="cuda")
+    plan.build_system(R, S)
+    plan.solve()
+    st, info = plan.status(check=False)
+    assert st == B.SFFT_ERR_NOT_SPD and 0 <= info < plan.n
+    plan.close()
+
+
+def test_argument_and_state_errors(cuda_device):
+    import torch
+    for bad in [(100, 128, 7, 1, 1, 0), (128, 128, 6, 1, 1, 0), (128, 128, 7, -1, 1, 0), (128, 128, 7, 1, 1, 2),
+                (64, 64, 33, 1, 1, 0), (16, 128, 3, 1, 1, 0)]:
+        st, _ = B.sfft_plan_create(*bad)
+        assert st == B.SFFT_ERR_INVALID_ARG, bad
+    st, h = B.sfft_plan_create(128, 128, 7, 1, 1, 0)
+    assert st == B.SFFT_OK and B.sfft_plan_num_unknowns(h) == 150
+    x = torch.zeros(128 * 128, dtype=torch.float64, device="cuda")
+    assert B.sfft_build_system(h, x.data_ptr(), x.data_ptr()) == B.SFFT_ERR_WORKSPACE
+    ws = torch.empty(B.sfft_plan_workspace_bytes(h) + 256, dtype=torch.uint8, device="cuda")
+    ptr = (ws.data_ptr() + 255) & ~255
+    assert B.sfft_plan_set_workspace(h, ptr, 1024) == B.SFFT_ERR_WORKSPACE
+    assert B.sfft_plan_set_workspace(h, ptr, B.sfft_plan_workspace_bytes(h)) == B.SFFT_OK
+    assert B.sfft_solve(h, x.data_ptr()) == B.SFFT_ERR_STATE
+    assert B.sfft_build_system(h, 0, x.data_ptr()) == B.SFFT_ERR_INVALID_ARG
+    B.sfft_plan_destroy(h)
