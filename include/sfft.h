@@ -118,10 +118,10 @@ int sfft_run_host(sfft_plan *plan, const double *h_R, const double *h_S, double 
  * build/solve/subtract rounds record CUDA events on the plan's stream around each stage (no host
  * synchronisation; 0 disables).  sfft_plan_profile_read synchronises the stream and writes
  * ms[step][SFFT_NUM_STAGES] (row-major; -1 where a stage did not run) for the *nrecorded steps seen.
- * Stage order: 0 row FFT (a1+a2), 1 lag correlation (a3+a4), 2 column reduction to lag tables (a4),
- * 3 lag gather (a5), 4 solve (a6), 5 kernel folding + per-row coefficient table (a7), 6 convolve-and-
- * subtract (a7+a8). */
-#define SFFT_NUM_STAGES 7
+ * Stage order: 0 row FFT (a1+a2), 1 x-direction lag correlation on the FP64 tensor cores (a3+a4), 2 y-direction
+ * pruned inverse DFT to the lag tables (a4), 3 basis-function moments Lambda/Delta (a4'), 4 lag gather (a5),
+ * 5 solve (a6), 6 kernel folding + per-row coefficient table (a7), 7 convolve-and-subtract (a7+a8). */
+#define SFFT_NUM_STAGES 8
 int sfft_plan_profile(sfft_plan *plan, int nsteps);
 int sfft_plan_profile_read(sfft_plan *plan, double *ms, int *nrecorded);
 

@@ -23,8 +23,8 @@ EXPORTS = [
     "sfft_subtract", "sfft_plan_status", "sfft_run_host", "sfft_plan_launch_count", "sfft_plan_destroy",
     "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
 ]
-SFFT_NUM_STAGES = 7
-STAGE_NAMES = ["rowfft", "corr", "lagsum", "gather", "solve", "subtract_prep", "subtract"]
+SFFT_NUM_STAGES = 8
+STAGE_NAMES = ["rowfft", "corr", "lagsum", "moments", "gather", "solve", "subtract_prep", "subtract"]
 
 _lib = None
 

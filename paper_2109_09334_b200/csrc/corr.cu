@@ -1,160 +1,183 @@
-// Steps a3+a4: cross-spectra and the "saccadic" restriction to the kernel lags.
+// Steps a3+a4 (x-direction): cross-spectra and the "saccadic" restriction to the kernel lags,
+// on the FP64 tensor cores.
 //
 // After the row transform (rowfft.cu) every correlation array of App. B
 // factorises over the spectrum columns m:
 //   Omega_{tb,t}(rho,eps) = sum_{x,y} R^tb(x,y) R^t(x+rho,y+eps)                              (B6, DESIGN g2)
 //     = (1/W) sum_m w_m Re[ G_{tb,t}(rho; m) exp(+2 pi i m eps / W) ],   w_0 = w_{W/2} = 1, else 2
-//   G_{tb,t}(rho; m) = sum_x conj(A_tb(x,m)) B_t((x+rho) mod H, m),     A_t(x,m) = f_i(x) r_j(x,m)
-// and likewise Theta (B = S, B14), Lambda (B = background function, whose row transform is the
-// rank-1 product f'_i(x) ghat'_j(m), B8) and Delta (B16).  Only |rho| <= L-1 (Omega) or <= w
-// (the others) is ever read by the normal matrix (B5-B15), so the x-direction is evaluated at
-// those lags only and the full-size correlation arrays of the paper are never materialised.
+//   G_{p,q}(rho; m) = sum_x conj(z_p(x,m)) z_q((x+rho) mod H, m),        z_t(x,m) = f_i(x) r_j(x,m)
+// and likewise Theta (q = S, B14).  The normal matrix reads Omega only at |rho| <= L-1 and Theta at
+// |rho| <= w (B5-B15), so the x-direction is evaluated at those lags only: the paper's full-size
+// correlation arrays (and the column transforms that would produce them) are never formed.
+// Negative lags come from  G_{p,q}(-rho) = conj(G_{q,p}(rho)),  so only rho = 0..L-1 is computed,
+// for all ordered pairs.
 //
-// k_corr_lags : G[b][entry][m]  (this file's hot kernel; FP64-FMA bound)
-// k_lagsum    : the m-sum above -> lag tables Omega / Theta / Lambda / Delta
+// For one column m this is a small dense contraction over x with a Hankel right operand:
+//   rows    : Re z_p, Im z_p of four sequences p                       (8 real rows)
+//   columns : z_q(x + rho) for eight consecutive lags rho              (8 columns, Re and Im apart)
+// i.e. two mma.sync.m8n8k4.f64 (DMMA) per 4 x-values give 4 x 8 complex lag sums with no wasted
+// multiply:  Re G = Cr[p] + Ci[p+4],  Im G = Ci[p] - Cr[p+4]   (Cr = A Br, Ci = A Bi).
+// The Hankel operand needs no data movement: lane (k, n) of the B fragment reads z_q(x0 + k + n + rho0)
+// straight from the x-contiguous shared-memory plane.  Lag 0 uses one extra block whose columns are the
+// eight N-side sequences at rho = 0.  The packed DC/Nyquist slot (column 0 holds (X[0], X[W/2]), both
+// real) falls out of the same arithmetic: Cr[p] is the DC sum and Ci[p+4] the Nyquist sum.
+//
+// CTA = 8 warps = 2 columns x 2 row blocks x 2 halves of the N side; two CTAs per SM overlap one
+// CTA's staging with the other's MMAs.  FP64-MMA bound.
 #include "sfft_internal.h"
 
 namespace sfft {
 namespace {
 
-constexpr int XT = 32;   // rows of x per shared-memory tile
-
-// value of sequence `sq` at (x, column m): xw[x] * img[x][m] with the packed DC/Nyquist slot undone
-__device__ __forceinline__ double2 load_seq(const double2 *__restrict__ rhat_b, const double *__restrict__ xwt, Seq sq,
-                                            int x, int m, int H, int Nh) {
-    double wgt = sq.xw >= 0 ? __ldg(&xwt[(size_t)sq.xw * H + x]) : 1.0;
-    if (sq.img < 0) return make_double2(wgt, 0.0);
-    if (m > Nh) return make_double2(0.0, 0.0);
-    const double2 *col = rhat_b + ((size_t)sq.img * H + x) * Nh;
-    double2 v;
-    if (m == 0) v = make_double2(__ldg(&col[0]).x, 0.0);
-    else if (m == Nh) v = make_double2(__ldg(&col[0]).y, 0.0);
-    else v = __ldg(&col[m]);
-    return make_double2(v.x * wgt, v.y * wgt);
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c[0]), "+d"(c[1])
+        : "d"(a), "d"(b));
 }
 
-// grid: x = column chunk (kColsPerCta columns), y = job, z = batch.  block: (kColsPerCta, 2*hwmax+1)
-__global__ void k_corr_lags(const double2 *__restrict__ rhat, const double *__restrict__ xwt,
-                            const Seq *__restrict__ seqs, const Job *__restrict__ jobs, double2 *__restrict__ G,
-                            int H, int Nh, int nimg, int nentries, int gcols, int hwmax) {
-    extern __shared__ double2 sm[];
-    const Job job = jobs[blockIdx.y];
-    const int c = threadIdx.x, ri = threadIdx.y, MC = kColsPerCta;
-    const int m0 = blockIdx.x * MC, hw = job.hw, nlag = 2 * hw + 1;
-    const int brows = XT + 2 * hwmax;
-    double2 *As = sm;                          // [kMaxTile][XT][MC]
-    double2 *Bs = sm + kMaxTile * XT * MC;     // [kMaxTile][brows][MC]
-    const double2 *rhat_b = rhat + (size_t)blockIdx.z * nimg * H * Nh;
-    const int tid = threadIdx.y * MC + threadIdx.x, nthr = blockDim.x * blockDim.y;
+template <int XT, int NLB>
+struct CorrCfg {
+    static constexpr int NTH = NLB <= 2 ? 4 : 2;           // N-side sequences per warp half
+    static constexpr int KNT = 2 * NTH - 1;                // N-side sequences per job
+    static constexpr int ROWS = XT + 8 * NLB;              // staged x-rows per tile
+    static constexpr int XS = ((ROWS + 7) / 16) * 16 + 8;  // plane stride, = 8 mod 16 (conflict-free staging stores)
+    static constexpr int SS = 4 * XS + 4;                  // slot stride [part 2][col 2][XS] + 4 (conflict-free A loads)
+    static constexpr int LBA = NLB > 0 ? NLB : 1;
+    static constexpr size_t SMEM = (size_t)kCorrSlots * SS * sizeof(double);
+};
 
-    double2 acc[kMaxTile][kMaxTile];
-#pragma unroll
-    for (int i = 0; i < kMaxTile; ++i)
-#pragma unroll
-        for (int j = 0; j < kMaxTile; ++j) acc[i][j] = make_double2(0.0, 0.0);
+// grid: x = column pair, y = job * Sx + xs, z = batch.  block: 256.
+template <int XT, int NLB>
+__global__ void __launch_bounds__(256, 2)
+k_corr_mma(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const Seq *__restrict__ seqs,
+           const CorrJob *__restrict__ jobs, double2 *__restrict__ G, int H, int Nh, int nimg, int nseq, int L, int E,
+           int Sx) {
+    using C = CorrCfg<XT, NLB>;
+    constexpr int NTH = C::NTH, KNT = C::KNT, ROWS = C::ROWS, XS = C::XS, SS = C::SS, LBA = C::LBA;
+    extern __shared__ double sm[];
+    __shared__ CorrJob job;
+    __shared__ Seq sseq[kCorrSlots];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int col = warp & 1, mb = (warp >> 1) & 1, nh = warp >> 2;
+    const int jb = blockIdx.y / Sx, xs = blockIdx.y - jb * Sx, bz = blockIdx.z;
+    const int m0 = blockIdx.x * kCorrCols;
 
-    for (int x0 = 0; x0 < H; x0 += XT) {
+    if (tid < (int)(sizeof(CorrJob) / sizeof(int))) reinterpret_cast<int *>(&job)[tid] = reinterpret_cast<const int *>(&jobs[jb])[tid];
+    for (int i = tid; i < kCorrSlots * SS; i += 256) sm[i] = 0.0;
+    __syncthreads();
+    if (tid < job.nstage) sseq[tid] = seqs[job.stage_seq[tid]];
+
+    const double2 *rhat_b = rhat + (size_t)bz * nimg * H * Nh;
+    const int row = lane >> 2, kq = lane & 3;
+    // per-lane fragment bases (doubles)
+    const double *sA = sm + job.mslot[mb][row & 3] * SS + ((row >> 2) * 2 + col) * XS + kq;
+    const double *sB = sm + (nh * NTH) * SS + col * XS + 1 + kq + row;
+    const double *s0 = sm + (row < KNT ? row : kCorrNSeq) * SS + col * XS + kq;
+
+    double acc[NTH][LBA][2][2];
+#pragma unroll
+    for (int q = 0; q < NTH; ++q)
+#pragma unroll
+        for (int lb = 0; lb < LBA; ++lb)
+#pragma unroll
+            for (int pt = 0; pt < 2; ++pt) acc[q][lb][pt][0] = acc[q][lb][pt][1] = 0.0;
+
+    const int xlen = H / Sx, xbeg = xs * xlen;
+    const int nitems = job.nstage * ROWS * kCorrCols;
+    for (int x0 = xbeg; x0 < xbeg + xlen; x0 += XT) {
         __syncthreads();
-        for (int i = tid; i < job.na * XT * MC; i += nthr) {
-            int cc = i % MC, r = (i / MC) % XT, s = i / (MC * XT);
-            As[(s * XT + r) * MC + cc] = load_seq(rhat_b, xwt, seqs[job.a[s]], x0 + r, m0 + cc, H, Nh);
-        }
-        const int nbr = XT + 2 * hw;
-        for (int i = tid; i < job.nb * nbr * MC; i += nthr) {
-            int cc = i % MC, r = (i / MC) % nbr, s = i / (MC * nbr);
-            int x = (x0 + r - hw) & (H - 1);
-            Bs[(s * brows + r) * MC + cc] = load_seq(rhat_b, xwt, seqs[job.b[s]], x, m0 + cc, H, Nh);
+        // ---- stage the tile: weighted sequences, split into Re / Im planes, x-contiguous ----
+        for (int i = tid; i < nitems; i += 256) {
+            const int c = i & 1, r = (i >> 1) % ROWS, si = (i >> 1) / ROWS;
+            const int x = (x0 + r) & (H - 1);
+            const Seq sq = sseq[si];
+            double2 v = __ldg(&rhat_b[((size_t)sq.img * H + x) * Nh + m0 + c]);
+            if (sq.xw >= 0) { const double wgt = __ldg(&xwt[(size_t)sq.xw * H + x]); v.x *= wgt; v.y *= wgt; }
+            double *pl = sm + job.stage_slot[si] * SS + c * XS + r;
+            pl[0] = v.x;
+            pl[2 * XS] = v.y;
         }
         __syncthreads();
-        if (ri < nlag) {
-#pragma unroll 4
-            for (int r = 0; r < XT; ++r) {
-                double2 a[kMaxTile], b[kMaxTile];
+        // ---- MMAs ----
+#pragma unroll 2
+        for (int kk = 0; kk < XT; kk += 4) {
+            const double a = sA[kk];
 #pragma unroll
-                for (int i = 0; i < kMaxTile; ++i) a[i] = As[(i * XT + r) * MC + c];
+            for (int q = 0; q < NTH; ++q) {
+                if (q == NTH - 1 && nh == 1) {      // warp-uniform: the lag-0 block takes this slot
 #pragma unroll
-                for (int j = 0; j < kMaxTile; ++j) b[j] = Bs[(j * brows + r + ri) * MC + c];
+                    for (int pt = 0; pt < 2; ++pt) dmma884(acc[q][0][pt], a, s0[pt * 2 * XS + kk]);
+                } else {
 #pragma unroll
-                for (int i = 0; i < kMaxTile; ++i)
+                    for (int lb = 0; lb < NLB; ++lb)
 #pragma unroll
-                    for (int j = 0; j < kMaxTile; ++j) {   // acc += conj(a) * b
-                        acc[i][j].x = fma(a[i].x, b[j].x, fma(a[i].y, b[j].y, acc[i][j].x));
-                        acc[i][j].y = fma(a[i].x, b[j].y, fma(-a[i].y, b[j].x, acc[i][j].y));
-                    }
+                        for (int pt = 0; pt < 2; ++pt) dmma884(acc[q][lb][pt], a, sB[q * SS + pt * 2 * XS + lb * 8 + kk]);
+                }
             }
         }
     }
-    if (ri < nlag && m0 + c <= Nh) {
-        double2 *Gb = G + (size_t)blockIdx.z * nentries * gcols;
+
+    // ---- epilogue: combine the Re/Im row halves and store G[b][xs][m][e] ----
+    const int mcol = m0 + col;
+    double2 *Gm = G + (((size_t)bz * Sx + xs) * (Nh + 1) + mcol) * E;
+    double2 *Gn = G + (((size_t)bz * Sx + xs) * (Nh + 1) + Nh) * E;     // Nyquist row (used by column 0 only)
+    const int p = job.mseq[mb][row & 3];
 #pragma unroll
-        for (int i = 0; i < kMaxTile; ++i)
+    for (int q = 0; q < NTH; ++q)
 #pragma unroll
-            for (int j = 0; j < kMaxTile; ++j)
-                if (i < job.na && j < job.nb)
-                    Gb[(size_t)(job.out_off + (i * job.nb + j) * nlag + ri) * gcols + m0 + c] = acc[i][j];
-    }
+        for (int lb = 0; lb < LBA; ++lb) {
+            const bool zero_blk = (q == NTH - 1 && nh == 1);
+            if (zero_blk ? (lb > 0) : (lb >= NLB)) continue;
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const double cr = acc[q][lb][0][i], ci = acc[q][lb][1][i];
+                const double ocr = __shfl_xor_sync(0xffffffffu, cr, 16), oci = __shfl_xor_sync(0xffffffffu, ci, 16);
+                if (row >= 4) continue;
+                const int nn = 2 * kq + i;
+                int rho, qs;
+                if (zero_blk) { rho = 0; qs = nn < KNT ? job.nseq[nn] : -1; }
+                else { rho = 1 + 8 * lb + nn; qs = job.nseq[nh * NTH + q]; }
+                if (p < 0 || qs < 0 || rho >= L) continue;
+                const int e = (p * nseq + qs) * L + rho;
+                if (mcol == 0) {
+                    Gm[e] = make_double2(cr, 0.0);
+                    Gn[e] = make_double2(oci, 0.0);
+                } else {
+                    Gm[e] = make_double2(cr + oci, ci - ocr);
+                }
+            }
+        }
 }
 
-// One CTA per (unit, batch): dst[e] = (1/W) sum_m w_m Re[G[m] ghat[m] exp(+2 pi i m (e-hw)/W)]
-__global__ void k_lagsum(const double2 *__restrict__ G, const Unit *__restrict__ units,
-                         const double2 *__restrict__ ghatB, const double2 *__restrict__ twW, double *__restrict__ tab,
-                         int Nh, int W, int nentries, int gcols, size_t tab_size) {
-    extern __shared__ double2 row[];   // [Nh+1]
-    const Unit u = units[blockIdx.x];
-    const double2 *g = G + ((size_t)blockIdx.y * nentries + u.g_entry) * gcols;
-    const int Wh1 = Nh + 1;
-    const double inv = 1.0 / (double)W;
-    for (int m = threadIdx.x; m < Wh1; m += blockDim.x) {
-        double2 v = g[m];
-        if (u.gj >= 0) {
-            double2 h = __ldg(&ghatB[(size_t)u.gj * Wh1 + m]);
-            v = make_double2(v.x * h.x - v.y * h.y, v.x * h.y + v.y * h.x);
-        }
-        double wm = (m == 0 || m == Nh) ? inv : 2.0 * inv;
-        row[m] = make_double2(v.x * wm, v.y * wm);
-    }
-    __syncthreads();
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-    const int neps = 2 * u.hw + 1;
-    double *dst = tab + (size_t)blockIdx.y * tab_size + u.dst_off;
-    for (int e = warp; e < neps; e += nwarp) {
-        const int eps = e - u.hw;
-        double s = 0.0;
-        for (int m = lane; m < Wh1; m += 32) {
-            // exp(+2 pi i m eps / W) = conj(twW[(m*eps) mod W])
-            double2 t = __ldg(&twW[(m * eps) & (W - 1)]);
-            double2 v = row[m];
-            s += v.x * t.x + v.y * t.y;     // Re[v * conj(t)]
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (lane == 0) dst[e] = s;
+template <int XT, int NLB>
+cudaError_t launch_t(sfft_plan *p) {
+    using C = CorrCfg<XT, NLB>;
+    auto kern = k_corr_mma<XT, NLB>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
+    dim3 grid(p->Nh / kCorrCols, (unsigned)p->jobs.size() * p->Sx, p->nbatch);
+    kern<<<grid, 256, C::SMEM, p->stream>>>(p->rhat, p->dt.xwt, p->dt.seqs, p->dt.jobs, p->G, p->H, p->Nh, p->nimg,
+                                            p->nseq, p->L, p->E, p->Sx);
+    p->launches++;
+    return cudaGetLastError();
+}
+
+template <int XT>
+cudaError_t launch_x(sfft_plan *p) {
+    switch (p->nlb) {
+        case 0: return launch_t<XT, 0>(p);
+        case 1: return launch_t<XT, 1>(p);
+        case 2: return launch_t<XT, 2>(p);
+        case 3: return launch_t<XT, 3>(p);
+        case 4: return launch_t<XT, 4>(p);
+        default: return cudaErrorInvalidValue;
     }
 }
 
 }  // namespace
 
 cudaError_t launch_corr(sfft_plan *p) {
-    const int hwmax = p->L - 1, MC = kColsPerCta;
-    size_t smem = (size_t)(kMaxTile * XT * MC + kMaxTile * (XT + 2 * hwmax) * MC) * sizeof(double2);
-    cudaError_t e = cudaFuncSetAttribute(k_corr_lags, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    dim3 grid((p->Nh + 1 + MC - 1) / MC, (unsigned)p->jobs.size(), p->nbatch), block(MC, 2 * hwmax + 1);
-    k_corr_lags<<<grid, block, smem, p->stream>>>(p->rhat, p->dt.xwt, p->dt.seqs, p->dt.jobs, p->G, p->H, p->Nh,
-                                                  p->nimg, p->nentries, p->gcols, hwmax);
-    p->launches++;
-    return cudaGetLastError();
-}
-
-cudaError_t launch_lagsum(sfft_plan *p) {
-    size_t smem = (size_t)(p->Nh + 1) * sizeof(double2);
-    cudaError_t e = cudaFuncSetAttribute(k_lagsum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    dim3 grid((unsigned)p->units.size(), p->nbatch);
-    k_lagsum<<<grid, 128, smem, p->stream>>>(p->G, p->dt.units, p->dt.ghatB, p->dt.twW, p->tab, p->Nh, p->W,
-                                             p->nentries, p->gcols, p->tab_size);
-    p->launches++;
-    return cudaGetLastError();
+    return (p->H / p->Sx) >= 64 ? launch_x<64>(p) : launch_x<32>(p);
 }
 
 }  // namespace sfft

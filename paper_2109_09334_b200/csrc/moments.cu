@@ -1,0 +1,163 @@
+// Step a4' : the correlation terms whose second factor is a basis function rather than an image.
+//   Lambda_{tb,s}(alpha,beta) = sum_{x,y} R^tb(x,y) T'_s((x+alpha) mod H, (y+beta) mod W)        (B8)
+//   Delta_s                   = sum_{x,y} S(x,y) T'_s(x,y)                                        (B16, DESIGN g2)
+// With T_tb = f_ib(x) g_jb(y) and T'_s = f'_i(x) g'_j(y) both are separable, so instead of the paper's
+// full-size DFT products they are two small real dense contractions (FP64 tensor cores):
+//   Q [x][(jb,j,beta)]  = sum_y R(x,y) * cy[(jb,j,beta)][y],     cy = g_jb(y) g'_j((y+beta) mod W)   (plan constant)
+//   C [(ib,i,alpha)][(jb,j,beta)] = sum_x fx[(ib,i,alpha)][x] * Q[x][(jb,j,beta)],  fx = f_ib(x) f'_i((x+alpha) mod H)
+//   Lambda_{(ib,jb),(i,j)}(alpha,beta) = C[(ib,i,alpha)][(jb,j,beta)]
+//   QS[x][j] = sum_y S(x,y) g'_j(y),   Delta_(i,j) = sum_x f'_i(x) QS[x][j]
+// Phi(0,0) = M_bb does not depend on the images and is a plan constant (plan.cu).
+//
+// k_dgemm : generic C = alpha A B(^T) + beta C, 64x64 CTA tile, mma.sync.m8n8k4.f64; also used by solve.cu.
+#include "sfft_internal.h"
+
+namespace sfft {
+namespace {
+
+constexpr int BM = 64, BN = 64, BK = 16, LDS_ = BK + 4;   // smem row stride = 4 mod 16 doubles: conflict-free fragments
+
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c[0]), "+d"(c[1])
+        : "d"(a), "d"(b));
+}
+
+// grid: x = N tile, y = M tile, z = problem * ksplit + kpart.  block: 128 (2x2 warps of 32x32).
+template <bool BT>
+__global__ void __launch_bounds__(128) k_dgemm(GemmArgs g) {
+    __shared__ double As[BM][LDS_];
+    __shared__ double Bs[BN][LDS_];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int zi = blockIdx.z / g.ksplit, kp = blockIdx.z - zi * g.ksplit;
+    const int i0 = blockIdx.y * BM, j0 = blockIdx.x * BN;
+    if (g.lower && j0 > i0 + BM - 1) return;
+    const double *A = g.A + (size_t)zi * g.sA, *B = g.B + (size_t)zi * g.sB;
+    double *C = g.C + (size_t)zi * g.sC + (size_t)kp * g.sCk;
+    const int klen = (g.K + g.ksplit - 1) / g.ksplit, kbeg = kp * klen, kend = min(g.K, kbeg + klen);
+    const int wm = (warp >> 1) * 32, wn = (warp & 1) * 32, r = lane >> 2, kq = lane & 3;
+
+    double acc[4][4][2];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+
+    for (int k0 = kbeg; k0 < kend; k0 += BK) {
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < BM * BK / 128; ++q) {
+            const int i = tid + 128 * q, rr = i >> 4, kk = i & 15;
+            As[rr][kk] = (i0 + rr < g.M && k0 + kk < kend) ? __ldg(&A[(size_t)(i0 + rr) * g.lda + k0 + kk]) : 0.0;
+        }
+        if (BT) {
+#pragma unroll
+            for (int q = 0; q < BN * BK / 128; ++q) {
+                const int i = tid + 128 * q, rr = i >> 4, kk = i & 15;
+                Bs[rr][kk] = (j0 + rr < g.N && k0 + kk < kend) ? __ldg(&B[(size_t)(j0 + rr) * g.ldb + k0 + kk]) : 0.0;
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < BN * BK / 128; ++q) {
+                const int i = tid + 128 * q, kk = i >> 6, nn = i & 63;
+                Bs[nn][kk] = (j0 + nn < g.N && k0 + kk < kend) ? __ldg(&B[(size_t)(k0 + kk) * g.ldb + j0 + nn]) : 0.0;
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int ks = 0; ks < BK; ks += 4) {
+            double af[4], bf[4];
+#pragma unroll
+            for (int a = 0; a < 4; ++a) af[a] = As[wm + 8 * a + r][ks + kq];
+#pragma unroll
+            for (int b = 0; b < 4; ++b) bf[b] = Bs[wn + 8 * b + r][ks + kq];
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) dmma884(acc[a][b], af[a], bf[b]);
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b)
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const int i = i0 + wm + 8 * a + r, j = j0 + wn + 8 * b + 2 * kq + q;
+                if (i < g.M && j < g.N && (!g.lower || j <= i)) {
+                    double *c = &C[(size_t)i * g.ldc + j];
+                    *c = (g.beta == 0.0) ? g.alpha * acc[a][b][q] : fma(g.alpha, acc[a][b][q], g.beta * *c);
+                }
+            }
+}
+
+// Lambda table  la[((tb*FB + s)*L + ai)*L + bi] = sum_kpart C[kpart][(ib,i,ai)][(jb,j,bi)]
+__global__ void k_lambda_pick(const double *__restrict__ C, double *__restrict__ tab, const int *__restrict__ kti,
+                              const int *__restrict__ ktj, const int *__restrict__ bti, const int *__restrict__ btj, int FK,
+                              int FB, int L, int nBa, int NC, int ksplit, size_t off_la, size_t tab_size) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, bz = blockIdx.y, LL = L * L;
+    if (i >= FK * FB * LL) return;
+    const int bi = i % L, ai = (i / L) % L, s = (i / LL) % FB, tb = i / (LL * FB);
+    const int rowc = (kti[tb] * nBa + bti[s]) * L + ai, colc = (ktj[tb] * nBa + btj[s]) * L + bi;
+    const double *c = C + (size_t)bz * ksplit * NC * NC + (size_t)rowc * NC + colc;
+    double v = 0.0;
+    for (int q = 0; q < ksplit; ++q) v += c[(size_t)q * NC * NC];
+    tab[(size_t)bz * tab_size + off_la + i] = v;
+}
+
+// Delta_s = sum_x f'_i(x) QS[x][j]   (one warp per s)
+__global__ void k_delta(const double *__restrict__ QS, const double *__restrict__ xwt, const int *__restrict__ bti,
+                        const int *__restrict__ btj, double *__restrict__ tab, int H, int nKa, int nBa, int FB,
+                        size_t off_de, size_t tab_size) {
+    const int s = blockIdx.x, bz = blockIdx.y, lane = threadIdx.x;
+    const double *f = xwt + (size_t)(nKa + bti[s]) * H;
+    const double *q = QS + (size_t)bz * H * nBa + btj[s];
+    double v = 0.0;
+    for (int x = lane; x < H; x += 32) v = fma(f[x], q[(size_t)x * nBa], v);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) tab[(size_t)bz * tab_size + off_de + s] = v;
+}
+
+}  // namespace
+
+cudaError_t launch_dgemm(sfft_plan *p, const GemmArgs &g) {
+    dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM, g.nz * g.ksplit);
+    if (g.bT) k_dgemm<true><<<grid, 128, 0, p->stream>>>(g);
+    else k_dgemm<false><<<grid, 128, 0, p->stream>>>(g);
+    p->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS) {
+    const int H = p->H, W = p->W, NC = p->NC;
+    const long long P = (long long)H * W;
+    // Q = R * cy^T
+    GemmArgs g{};
+    g.A = dR; g.B = p->dt.cy; g.C = p->Q; g.M = H; g.N = NC; g.K = W; g.lda = W; g.ldb = W; g.ldc = NC;
+    g.sA = P; g.sB = 0; g.sC = (long long)H * NC; g.sCk = 0; g.nz = p->nbatch; g.ksplit = 1; g.alpha = 1.0; g.beta = 0.0;
+    g.bT = true; g.lower = false;
+    cudaError_t e = launch_dgemm(p, g);
+    if (e != cudaSuccess) return e;
+    // QS = S * gB^T
+    g.A = dS; g.B = p->dt.gB; g.C = p->QS; g.N = p->nBa; g.ldc = p->nBa; g.sC = (long long)H * p->nBa;
+    e = launch_dgemm(p, g);
+    if (e != cudaSuccess) return e;
+    // C = fx * Q   (split over K = H)
+    GemmArgs h{};
+    h.A = p->dt.fx; h.B = p->Q; h.C = p->LamC; h.M = NC; h.N = NC; h.K = H; h.lda = H; h.ldb = NC; h.ldc = NC;
+    h.sA = 0; h.sB = (long long)H * NC; h.sC = (long long)p->ksplit * NC * NC; h.sCk = (long long)NC * NC;
+    h.nz = p->nbatch; h.ksplit = p->ksplit; h.alpha = 1.0; h.beta = 0.0; h.bT = false; h.lower = false;
+    e = launch_dgemm(p, h);
+    if (e != cudaSuccess) return e;
+    const int tot = p->FK * p->FB * p->L * p->L;
+    k_lambda_pick<<<dim3((tot + 255) / 256, p->nbatch), 256, 0, p->stream>>>(
+        p->LamC, p->tab, p->dt.kti, p->dt.ktj, p->dt.bti, p->dt.btj, p->FK, p->FB, p->L, p->nBa, NC, p->ksplit, p->off_la,
+        p->tab_size);
+    k_delta<<<dim3(p->FB, p->nbatch), 32, 0, p->stream>>>(p->QS, p->dt.xwt, p->dt.bti, p->dt.btj, p->tab, H, p->nKa, p->nBa,
+                                                         p->FB, p->off_de, p->tab_size);
+    p->launches += 2;
+    return cudaGetLastError();
+}
+
+}  // namespace sfft

@@ -86,79 +86,79 @@ cudaError_t upload(T **dst, const T *src, size_t count) {
 
 int pair_index(int FK, int t1, int t2) { return t1 * FK - t1 * (t1 - 1) / 2 + (t2 - t1); }  // t1 <= t2
 
+// x-range splits of the correlation kernel: fill the 2 x 148 CTA slots evenly (partials are added in lagsum)
+void choose_split(sfft_plan *p) {
+    p->Sx = 1;
+    const double slots = 2.0 * 148.0;
+    double best = 1e300;
+    for (int sx = 1; sx <= 8; sx *= 2) {
+        if (p->H / sx < 32) break;
+        double T = (double)(p->Nh / kCorrCols) * p->jobs.size() * p->nbatch * sx;
+        double cost = ceil(T / slots) / sx * (1.0 + 0.02 * sx);     // mild penalty: G traffic grows with sx
+        if (cost < best) { best = cost; p->Sx = sx; }
+    }
+}
+
 void build_jobs(sfft_plan *p) {
     const int FK = p->FK, FB = p->FB, L = p->L, w = p->w, nO = 2 * L - 1;
     p->seqs.clear(); p->jobs.clear(); p->units.clear();
+    // column sequences: kernel terms z_t = f_i(x) r_j(x,m), then S
     for (int t = 0; t < FK; ++t) p->seqs.push_back({p->ktj[t], p->kti[t]});
     const int seqS = FK;
     p->seqs.push_back({p->nKa, -1});
-    for (int i = 0; i < p->nBa; ++i) p->seqs.push_back({-1, p->nKa + i});
+    p->nseq = FK + 1;
+    p->E = p->nseq * p->nseq * L;
+    p->nlb = (L - 1 + 7) / 8;
     p->npairs = FK * (FK + 1) / 2;
     p->off_om = 0;
     p->off_th = p->off_om + (size_t)p->npairs * nO * nO;
     p->off_la = p->off_th + (size_t)FK * L * L;
     p->off_de = p->off_la + (size_t)FK * FB * L * L;
     p->tab_size = p->off_de + FB;
-    int entry = 0;
-    // Omega: kernel terms x kernel terms, lags +-(L-1); only cells with tb <= t are reduced
-    for (int a0 = 0; a0 < FK; a0 += kMaxTile)
-        for (int b0 = 0; b0 < FK; b0 += kMaxTile) {
-            int na = std::min(kMaxTile, FK - a0), nb = std::min(kMaxTile, FK - b0);
-            if (b0 + nb - 1 < a0) continue;
-            Job j{}; j.na = na; j.nb = nb; j.hw = L - 1; j.out_off = entry;
-            for (int q = 0; q < na; ++q) j.a[q] = a0 + q;
-            for (int q = 0; q < nb; ++q) j.b[q] = b0 + q;
-            for (int ai = 0; ai < na; ++ai)
-                for (int bi = 0; bi < nb; ++bi) {
-                    int tb = a0 + ai, t = b0 + bi;
-                    if (tb > t) continue;
-                    for (int r = 0; r < nO; ++r)
-                        p->units.push_back({entry + (ai * nb + bi) * nO + r, -1, L - 1,
-                                            (int)(p->off_om + ((size_t)pair_index(FK, tb, t) * nO + r) * nO)});
+    // correlation jobs: (group of 8 M-side sequences) x (tile of knt N-side sequences)
+    const int knt = p->nlb <= 2 ? 7 : 3;
+    for (int m0 = 0; m0 < p->nseq; m0 += 8)
+        for (int n0 = 0; n0 < p->nseq; n0 += knt) {
+            CorrJob j{};
+            j.nstage = 0;
+            for (int q = 0; q < 8; ++q) {
+                j.nseq[q] = (q < knt && n0 + q < p->nseq) ? n0 + q : -1;
+                if (j.nseq[q] >= 0) { j.stage_slot[j.nstage] = q; j.stage_seq[j.nstage] = j.nseq[q]; ++j.nstage; }
+            }
+            int extra = kCorrNSeq + 1;
+            for (int h = 0; h < 2; ++h)
+                for (int r = 0; r < 4; ++r) {
+                    int sq = m0 + 4 * h + r;
+                    if (sq >= p->nseq) { j.mseq[h][r] = -1; j.mslot[h][r] = kCorrNSeq; continue; }
+                    j.mseq[h][r] = sq;
+                    int slot = -1;
+                    for (int q = 0; q < 8; ++q) if (j.nseq[q] == sq) slot = q;
+                    if (slot < 0) { slot = extra++; j.stage_slot[j.nstage] = slot; j.stage_seq[j.nstage] = sq; ++j.nstage; }
+                    j.mslot[h][r] = slot;
                 }
-            entry += na * nb * nO;
             p->jobs.push_back(j);
         }
-    // Theta (B = S) and Lambda (B = background x-functions), lags +-w
-    std::vector<int> bl; bl.push_back(seqS);
-    for (int i = 0; i < p->nBa; ++i) bl.push_back(FK + 1 + i);
-    for (int a0 = 0; a0 < FK; a0 += kMaxTile)
-        for (size_t b0 = 0; b0 < bl.size(); b0 += kMaxTile) {
-            int na = std::min(kMaxTile, FK - a0), nb = (int)std::min<size_t>(kMaxTile, bl.size() - b0);
-            Job j{}; j.na = na; j.nb = nb; j.hw = w; j.out_off = entry;
-            for (int q = 0; q < na; ++q) j.a[q] = a0 + q;
-            for (int q = 0; q < nb; ++q) j.b[q] = bl[b0 + q];
-            for (int ai = 0; ai < na; ++ai)
-                for (int bi = 0; bi < nb; ++bi) {
-                    int tb = a0 + ai, sq = j.b[bi];
-                    for (int r = 0; r < L; ++r) {
-                        int ge = entry + (ai * nb + bi) * L + r;
-                        if (sq == seqS) {
-                            p->units.push_back({ge, -1, w, (int)(p->off_th + ((size_t)tb * L + r) * L)});
-                        } else {
-                            int ib = sq - (FK + 1);
-                            for (int s = 0; s < FB; ++s)
-                                if (p->bti[s] == ib)
-                                    p->units.push_back({ge, p->btj[s], w,
-                                                        (int)(p->off_la + (((size_t)tb * FB + s) * L + r) * L)});
-                        }
-                    }
-                }
-            entry += na * nb * L;
-            p->jobs.push_back(j);
+    // lag-table rows.  Negative x-lags use G_{p,q}(-rho) = conj G_{q,p}(rho): entry (q,p,|rho|) with eps negated.
+    auto entry = [&](int pp, int qq, int rho) { return (pp * p->nseq + qq) * L + rho; };
+    for (int tb = 0; tb < FK; ++tb)
+        for (int t = tb; t < FK; ++t)
+            for (int r = 0; r < nO; ++r) {
+                int rho = r - (L - 1);
+                int dst = (int)(p->off_om + ((size_t)pair_index(FK, tb, t) * nO + r) * nO);
+                if (rho >= 0) p->units.push_back({entry(tb, t, rho), +1, L - 1, dst});
+                else p->units.push_back({entry(t, tb, -rho), -1, L - 1, dst});
+            }
+    for (int tb = 0; tb < FK; ++tb)
+        for (int r = 0; r < L; ++r) {
+            int rho = r - w;
+            int dst = (int)(p->off_th + ((size_t)tb * L + r) * L);
+            if (rho >= 0) p->units.push_back({entry(tb, seqS, rho), +1, w, dst});
+            else p->units.push_back({entry(seqS, tb, -rho), -1, w, dst});
         }
-    // Delta: A = S, B = background x-functions, lag 0
-    for (int b0 = 0; b0 < p->nBa; b0 += kMaxTile) {
-        int nb = std::min(kMaxTile, p->nBa - b0);
-        Job j{}; j.na = 1; j.nb = nb; j.hw = 0; j.out_off = entry; j.a[0] = seqS;
-        for (int q = 0; q < nb; ++q) j.b[q] = FK + 1 + b0 + q;
-        for (int bi = 0; bi < nb; ++bi)
-            for (int s = 0; s < FB; ++s)
-                if (p->bti[s] == b0 + bi) p->units.push_back({entry + bi, p->btj[s], 0, (int)(p->off_de + s)});
-        entry += nb;
-        p->jobs.push_back(j);
-    }
-    p->nentries = entry;
+    choose_split(p);
+    p->nch = (p->Nh + 1 + kLagChunk - 1) / kLagChunk;
+    p->NC = p->nKa * p->nBa * L;
+    p->ksplit = std::max(1, std::min(16, p->H / 128));
 }
 
 int fail_cuda(sfft_plan *p, cudaError_t e) {
@@ -168,14 +168,15 @@ int fail_cuda(sfft_plan *p, cudaError_t e) {
 
 void free_tables(sfft_plan *p) {
     DeviceTables &d = p->dt;
-    cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.ghatB); cudaFree(d.phi0);
+    cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.lagtw); cudaFree(d.cy); cudaFree(d.fx);
+    cudaFree(d.phi0);
     cudaFree(d.seqs); cudaFree(d.jobs); cudaFree(d.units);
     cudaFree(d.kti); cudaFree(d.ktj); cudaFree(d.bti); cudaFree(d.btj);
     d = DeviceTables();
 }
 
 struct WsLayout {
-    size_t rhat, G, tab, M, rhs, Lf, dscale, kfold, ctab, flag, stR, stS, stD, stC, total;
+    size_t rhat, G, lagpart, tab, Q, QS, LamC, M, rhs, Lf, dscale, kfold, ctab, flag, stR, stS, stD, stC, total;
 };
 
 WsLayout ws_layout(const sfft_plan *p) {
@@ -183,8 +184,12 @@ WsLayout ws_layout(const sfft_plan *p) {
     size_t nb = p->nbatch, P = (size_t)p->H * p->W, n = p->n, off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
     l.rhat = take(nb * p->nimg * (size_t)p->H * p->Nh * sizeof(double2));
-    l.G = take(nb * (size_t)p->nentries * p->gcols * sizeof(double2));
+    l.G = take(nb * p->Sx * (size_t)(p->Nh + 1) * p->E * sizeof(double2));
+    l.lagpart = take(nb * p->nch * (size_t)p->L * 2 * p->E * sizeof(double));
     l.tab = take(nb * p->tab_size * sizeof(double));
+    l.Q = take(nb * (size_t)p->H * p->NC * sizeof(double));
+    l.QS = take(nb * (size_t)p->H * p->nBa * sizeof(double));
+    l.LamC = take(nb * p->ksplit * (size_t)p->NC * p->NC * sizeof(double));
     l.M = take(nb * n * n * sizeof(double));
     l.rhs = take(nb * n * sizeof(double));
     l.Lf = take(nb * (n + 1) * (size_t)p->ldl * sizeof(double));
@@ -224,7 +229,6 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     p->FK = (int)p->kti.size(); p->FB = (int)p->bti.size();
     p->n = p->FK * L * L + p->FB;
     p->nimg = p->nKa + 1;
-    p->gcols = p->Nh + 8;
     p->ldl = (p->n + 1 + 7) & ~7;
     p->LT = subtract_tap_width(L);
     build_jobs(p);
@@ -243,18 +247,29 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
         cw[k] = cosl(twopi * k / W); sw[k] = -sinl(twopi * k / W);
         twW[k] = make_double2((double)cw[k], (double)sw[k]);
     }
-    const int Wh1 = p->Nh + 1;
-    std::vector<double2> ghat((size_t)p->nBa * Wh1);
-    for (int j = 0; j < p->nBa; ++j)
-        for (int m = 0; m < Wh1; ++m) {
-            long double re = 0.0L, im = 0.0L;
-            for (int y = 0; y < W; ++y) {
-                int k = (int)(((long long)m * y) & (W - 1));
-                long double g = gB[(size_t)j * W + y];
-                re += g * cw[k]; im += g * sw[k];
-            }
-            ghat[(size_t)j * Wh1 + m] = make_double2((double)re, (double)im);
+    // y-direction pruned inverse DFT weights (lagsum.cu): (w_m cos, w_m sin)(2 pi m k / W) / W
+    std::vector<double2> lagtw((size_t)(p->Nh + 1) * L);
+    for (int m = 0; m <= p->Nh; ++m)
+        for (int k = 0; k < L; ++k) {
+            int idx = (int)(((long long)m * k) & (W - 1));
+            long double wm = (m == 0 || m == p->Nh) ? 1.0L : 2.0L;
+            lagtw[(size_t)m * L + k] = make_double2((double)(wm * cw[idx] / W), (double)(wm * -sw[idx] / W));
         }
+    // moment-GEMM operands (moments.cu): products of a kernel and a shifted background basis function
+    const int wl = p->w;
+    std::vector<double> cy((size_t)p->NC * W), fx((size_t)p->NC * H);
+    for (int jb = 0; jb < p->nKa; ++jb)
+        for (int j = 0; j < p->nBa; ++j)
+            for (int b = 0; b < L; ++b) {
+                double *row = &cy[((size_t)(jb * p->nBa + j) * L + b) * W];
+                for (int y = 0; y < W; ++y) row[y] = gK[(size_t)jb * W + y] * gB[(size_t)j * W + ((y + b - wl + W) & (W - 1))];
+            }
+    for (int ib = 0; ib < p->nKa; ++ib)
+        for (int i = 0; i < p->nBa; ++i)
+            for (int a = 0; a < L; ++a) {
+                double *row = &fx[((size_t)(ib * p->nBa + i) * L + a) * H];
+                for (int x = 0; x < H; ++x) row[x] = fK[(size_t)ib * H + x] * fB[(size_t)i * H + ((x + a - wl + H) & (H - 1))];
+            }
     // M_bb = sum_x f_ib f_i * sum_y g_jb g_j  (Eq. 22 / B11 at lag 0; separable, plan constant)
     std::vector<double> phi0((size_t)p->FB * p->FB);
     {
@@ -275,7 +290,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     cudaError_t e = cudaSuccess;
     DeviceTables &d = p->dt;
 #define UP(dst, vec) if (e == cudaSuccess) e = upload(&d.dst, vec.data(), vec.size())
-    UP(xwt, xwt); UP(gK, gK); UP(gB, gB); UP(twW, twW); UP(ghatB, ghat); UP(phi0, phi0);
+    UP(xwt, xwt); UP(gK, gK); UP(gB, gB); UP(twW, twW); UP(lagtw, lagtw); UP(cy, cy); UP(fx, fx); UP(phi0, phi0);
     UP(seqs, p->seqs); UP(jobs, p->jobs); UP(units, p->units);
     UP(kti, p->kti); UP(ktj, p->ktj); UP(bti, p->bti); UP(btj, p->btj);
 #undef UP
@@ -287,6 +302,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
 int sfft_plan_set_batch(sfft_plan *p, int nbatch) {
     if (!p || nbatch < 1 || nbatch > 65535) return SFFT_ERR_INVALID_ARG;
     p->nbatch = nbatch; p->ws = nullptr; p->ws_bytes = 0; p->built = p->solved = false;
+    choose_split(p);
     return SFFT_OK;
 }
 
@@ -308,7 +324,8 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     if (bytes < l.total || ((uintptr_t)d_ws & 255)) return SFFT_ERR_WORKSPACE;
     char *b = (char *)d_ws;
     p->ws = d_ws; p->ws_bytes = bytes;
-    p->rhat = (double2 *)(b + l.rhat); p->G = (double2 *)(b + l.G); p->tab = (double *)(b + l.tab);
+    p->rhat = (double2 *)(b + l.rhat); p->G = (double2 *)(b + l.G); p->lagpart = (double *)(b + l.lagpart); p->tab = (double *)(b + l.tab);
+    p->Q = (double *)(b + l.Q); p->QS = (double *)(b + l.QS); p->LamC = (double *)(b + l.LamC);
     p->M = (double *)(b + l.M); p->rhs = (double *)(b + l.rhs); p->Lf = (double *)(b + l.Lf);
     p->dscale = (double *)(b + l.dscale); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->flag = (int *)(b + l.flag);
     p->stageR = (double *)(b + l.stR); p->stageS = (double *)(b + l.stS); p->stageD = (double *)(b + l.stD);
@@ -330,8 +347,10 @@ int sfft_build_system(sfft_plan *p, const double *d_R, const double *d_S) {
     prof_mark(p, 2);
     if (e == cudaSuccess) e = launch_lagsum(p);
     prof_mark(p, 3);
-    if (e == cudaSuccess) e = launch_gather(p);
+    if (e == cudaSuccess) e = launch_moments(p, d_R, d_S);
     prof_mark(p, 4);
+    if (e == cudaSuccess) e = launch_gather(p);
+    prof_mark(p, 5);
     if (e != cudaSuccess) return fail_cuda(p, e);
     p->built = true;
     return SFFT_OK;
@@ -356,8 +375,8 @@ int sfft_plan_profile_read(sfft_plan *p, double *ms, int *nrecorded) {
     if (e != cudaSuccess) return fail_cuda(p, e);
     int nrec = std::min(p->prof_cur + 1, p->prof_steps);
     if (nrecorded) *nrecorded = nrec;
-    // stages: 0 rowfft, 1 corr, 2 lagsum, 3 gather, 4 solve, 5 subtract-prep, 6 subtract
-    static const int from[SFFT_NUM_STAGES] = {0, 1, 2, 3, 5, 7, 8}, to[SFFT_NUM_STAGES] = {1, 2, 3, 4, 6, 8, 9};
+    // stages: 0 rowfft, 1 corr, 2 lagsum, 3 moments, 4 gather, 5 solve, 6 subtract-prep, 7 subtract
+    static const int from[SFFT_NUM_STAGES] = {0, 1, 2, 3, 4, 6, 8, 9}, to[SFFT_NUM_STAGES] = {1, 2, 3, 4, 5, 7, 9, 10};
     for (int s = 0; s < nrec; ++s)
         for (int g = 0; g < SFFT_NUM_STAGES; ++g) {
             float t = 0.f;
@@ -391,9 +410,9 @@ int sfft_get_lag_table(const sfft_plan *p, int which, const double **d_table, si
 int sfft_solve(sfft_plan *p, double *d_coef) {
     if (!p || !d_coef) return SFFT_ERR_INVALID_ARG;
     if (!p->built) return SFFT_ERR_STATE;
-    prof_mark(p, 5);
-    cudaError_t e = launch_solve(p, d_coef);
     prof_mark(p, 6);
+    cudaError_t e = launch_solve(p, d_coef);
+    prof_mark(p, 7);
     if (e != cudaSuccess) return fail_cuda(p, e);
     p->solved = true;
     return SFFT_OK;
@@ -402,9 +421,9 @@ int sfft_solve(sfft_plan *p, double *d_coef) {
 int sfft_subtract(sfft_plan *p, const double *d_coef, const double *d_R, const double *d_S, double *d_D) {
     if (!p || !d_coef || !d_R || !d_S || !d_D) return SFFT_ERR_INVALID_ARG;
     if (!p->ws) return SFFT_ERR_WORKSPACE;
-    prof_mark(p, 7);
+    prof_mark(p, 8);
     cudaError_t e = launch_subtract(p, d_coef, d_R, d_S, d_D);
-    prof_mark(p, 9);
+    prof_mark(p, 10);
     if (e != cudaSuccess) return fail_cuda(p, e);
     return SFFT_OK;
 }

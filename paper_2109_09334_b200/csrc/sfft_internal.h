@@ -10,35 +10,44 @@
 
 namespace sfft {
 
-constexpr int kProfMarks = 10;   // event marks per profiled step (see sfft_plan_profile_read)
-constexpr int kMaxTile = 4;     // sequences per side of a correlation job tile
-constexpr int kColsPerCta = 8;  // spectrum columns (m) per CTA in the correlation kernel
+constexpr int kProfMarks = 11;     // event marks per profiled step (see sfft_plan_profile_read)
+constexpr int kCorrCols = 2;       // spectrum columns (m) per CTA of the correlation kernel
+constexpr int kCorrNSeq = 7;       // N-side (shifted) sequences per correlation job (max)
+constexpr int kCorrSlots = 16;     // shared-memory sequence planes per CTA: 0..6 N side, 7 zero, 8..15 extra M side
+constexpr int kLagChunk = 32;      // spectrum columns per partial sum of the y-direction inverse DFT
 
-// One column-sequence fed to the x-direction correlation:  value(x, m) = xw[x] * img[x][m]
-//   img >= 0 : row-transformed image `img` of the spectrum stack (0..nKy-1: g_j(y) R, nKy: S)
-//   img <  0 : the constant-in-m real sequence xw[x] (a background x-basis function)
-//   xw  <  0 : no x-weight (1)
+// One column-sequence of the x-direction correlation:  z_s(x, m) = xw[x] * rhat[img][x][m]
+//   img : row-transformed image of the spectrum stack (0..nKa-1: g_j(y) R, nKa: S)
+//   xw  : row of the x-weight table (kernel x-basis function f_i), < 0 = no weight
 struct Seq { int img; int xw; };
 
-// A tile of (A x B) sequence pairs correlated at lags |rho| <= hw; output entries
-// out_off + (ai*nb + bi)*(2hw+1) + (rho+hw)
-struct Job { int na, nb, hw, out_off; int a[kMaxTile]; int b[kMaxTile]; };
+// One job of k_corr_mma: all ordered pairs (p in mseq) x (q in nseq) at lags 0..L-1,
+//   G_{p,q}(rho; m) = sum_x conj(z_p(x,m)) z_q((x+rho) mod H, m).
+struct CorrJob {
+    int nseq[8];        // N-side sequence ids (slot q = nseq[q]); -1 = none (zero plane)
+    int mseq[2][4];     // M-side sequence ids of the two 4-row blocks; -1 = none
+    int mslot[2][4];    // shared-memory slot of each M-side sequence (kCorrNSeq = the zero plane)
+    int nstage;         // number of staged slots
+    int stage_slot[kCorrSlots];   // slot index of each staged sequence
+    int stage_seq[kCorrSlots];    // its sequence id
+};
 
-// One (G entry row -> lag table row) reduction over the spectrum columns m:
-//   dst[e] = (1/W) sum_m w_m Re[ G[g_entry][m] * ghat[gj][m] * exp(+2 pi i m eps / W) ],  eps = e - hw
-// (ghat factor skipped when gj < 0).
-struct Unit { int g_entry; int gj; int hw; int dst_off; };
+// One row of a lag table produced by the y-direction pruned inverse DFT:
+//   dst[eps + hw] = (1/W) sum_m w_m Re[ G[e][m] exp(+2 pi i m (sgn*eps) / W) ],  |eps| <= hw
+struct LagUnit { int e; int sgn; int hw; int dst_off; };
 
 struct DeviceTables {
     double *xwt = nullptr;      // [nKa + nBa][H]   x-axis basis tables (kernel rows first)
     double *gK = nullptr;       // [nKa][W]         kernel y-axis basis
     double *gB = nullptr;       // [nBa][W]         background y-axis basis
     double2 *twW = nullptr;     // [W]              exp(-2 pi i k / W)
-    double2 *ghatB = nullptr;   // [nBa][W/2+1]     DFT_y of gB rows (half spectrum)
+    double2 *lagtw = nullptr;   // [Nh+1][L]        (w_m cos, w_m sin)(2 pi m k / W) / W
+    double *cy = nullptr;       // [NC][W]          g_jb(y) g'_j((y+beta) mod W),  c = (jb*nBa + j)*L + beta+w
+    double *fx = nullptr;       // [NC][H]          f_ib(x) f'_i((x+alpha) mod H), c = (ib*nBa + i)*L + alpha+w
     double *phi0 = nullptr;     // [FB][FB]         M_bb (plan constant)
     Seq *seqs = nullptr;
-    Job *jobs = nullptr;
-    Unit *units = nullptr;
+    CorrJob *jobs = nullptr;
+    LagUnit *units = nullptr;
     int *kti = nullptr, *ktj = nullptr, *bti = nullptr, *btj = nullptr;
 };
 
@@ -48,21 +57,27 @@ struct sfft_plan {
     int H = 0, W = 0, L = 0, w = 0, DK = 0, DB = 0, basis = 0, nbatch = 1;
     int FK = 0, FB = 0, nKa = 0, nBa = 0, n = 0, Nh = 0;
     int nimg = 0;        // spectrum stack depth per batch entry: nKa weighted-y images + S
-    int gcols = 0;       // padded column count of G rows (>= W/2+1)
-    int nentries = 0;    // G rows per batch entry
+    int nseq = 0;        // FK + 1 column sequences (kernel terms, then S)
+    int E = 0;           // G entries per spectrum column: nseq*nseq*L
+    int Sx = 1;          // x-range splits of the correlation kernel (partial sums added by lagsum)
+    int nlb = 0;         // 8-lag blocks: ceil((L-1)/8)
+    int nch = 0;         // column chunks of the lagsum partials
+    int NC = 0;          // nKa*nBa*L columns of the moment GEMMs
+    int ksplit = 1;      // K splits of the second moment GEMM
     int npairs = 0;      // FK(FK+1)/2
     int ldl = 0;         // leading dimension of the Cholesky factor buffer (>= n+1)
     int LT = 0;          // padded tap width of the subtract kernel instantiation (>= L)
     std::vector<int> kti, ktj, bti, btj;
     std::vector<sfft::Seq> seqs;
-    std::vector<sfft::Job> jobs;
-    std::vector<sfft::Unit> units;
+    std::vector<sfft::CorrJob> jobs;
+    std::vector<sfft::LagUnit> units;
     sfft::DeviceTables dt;
     // lag-table layout (doubles per batch entry)
     size_t off_om = 0, off_th = 0, off_la = 0, off_de = 0, tab_size = 0;
     // workspace partition (device pointers into the caller's buffer)
     void *ws = nullptr; size_t ws_bytes = 0;
-    double2 *rhat = nullptr; double2 *G = nullptr; double *tab = nullptr;
+    double2 *rhat = nullptr; double2 *G = nullptr; double *lagpart = nullptr; double *tab = nullptr;
+    double *Q = nullptr, *QS = nullptr, *LamC = nullptr;
     double *M = nullptr, *rhs = nullptr, *Lf = nullptr, *dscale = nullptr, *kfold = nullptr, *ctab = nullptr;
     double *stageR = nullptr, *stageS = nullptr, *stageD = nullptr, *stageC = nullptr;
     int *flag = nullptr;
@@ -79,9 +94,24 @@ namespace sfft {
 cudaError_t launch_rowfft_forward(sfft_plan *p, const double *dR, const double *dS);
 cudaError_t launch_corr(sfft_plan *p);
 cudaError_t launch_lagsum(sfft_plan *p);
+cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS);
 cudaError_t launch_gather(sfft_plan *p);
 cudaError_t launch_solve(sfft_plan *p, double *d_coef);
 int subtract_tap_width(int L);
 void prof_mark(sfft_plan *p, int mark);
 cudaError_t launch_subtract(sfft_plan *p, const double *d_coef, const double *dR, const double *dS, double *dD);
+
+// C[M x N] (ldc) = alpha * A[M x K] (lda, row-major) * B + beta * C  on the FP64 tensor cores.
+// bT = true : B given as [N x K] row-major (ldb)  ("A B^T");  false : B is [K x N] row-major.
+// grid.z = nz problems with element strides sA, sB, sC; K may be split in `ksplit` parts, part q
+// writing C + q*sCk (beta must then be 0).  lower = true : only tiles touching j <= i are computed.
+struct GemmArgs {
+    const double *A; const double *B; double *C;
+    int M, N, K, lda, ldb, ldc;
+    long long sA, sB, sC, sCk;
+    int nz, ksplit;
+    double alpha, beta;
+    bool bT, lower;
+};
+cudaError_t launch_dgemm(sfft_plan *p, const GemmArgs &g);
 }  // namespace sfft

@@ -171,7 +171,7 @@ cudaError_t launch_subtract(sfft_plan *p, const double *d_coef, const double *dR
     k_coef_rows<<<dim3(p->H, p->nbatch), 256, 0, p->stream>>>(p->kfold, p->dt.xwt, p->dt.kti, p->dt.ktj, p->ctab, p->H,
                                                              p->nKa, p->FK, p->L, LT, LTP);
     p->launches += 2;
-    prof_mark(p, 8);
+    prof_mark(p, 9);
     switch (LT) {
         case 3: return launch_sub<3>(p, d_coef, dR, dS, dD);
         case 7: return launch_sub<7>(p, d_coef, dR, dS, dD);
