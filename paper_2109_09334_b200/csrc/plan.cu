@@ -195,7 +195,7 @@ WsLayout ws_layout(const sfft_plan *p) {
     l.Lf = take(nb * (n + 1) * (size_t)p->ldl * sizeof(double));
     l.dscale = take(nb * n * sizeof(double));
     l.kfold = take(nb * (size_t)p->FK * p->L * p->L * sizeof(double));
-    l.ctab = take(nb * (size_t)p->H * p->nKa * p->LT * (p->LT + 1) * sizeof(double));
+    l.ctab = take(nb * (size_t)p->H * p->L * p->LT * sizeof(double));
     l.flag = take(nb * sizeof(int) * 2);
     l.stR = take(nb * P * sizeof(double));
     l.stS = take(nb * P * sizeof(double));
@@ -230,7 +230,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     p->n = p->FK * L * L + p->FB;
     p->nimg = p->nKa + 1;
     p->ldl = (p->n + 1 + 7) & ~7;
-    p->LT = subtract_tap_width(L);
+    p->LT = subtract_kpad(p->nKa, L);
     build_jobs(p);
 
     // ---- constant tables (host, long double where it matters) ----

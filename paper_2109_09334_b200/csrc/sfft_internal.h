@@ -66,7 +66,7 @@ struct sfft_plan {
     int ksplit = 1;      // K splits of the second moment GEMM
     int npairs = 0;      // FK(FK+1)/2
     int ldl = 0;         // leading dimension of the Cholesky factor buffer (>= n+1)
-    int LT = 0;          // padded tap width of the subtract kernel instantiation (>= L)
+    int LT = 0;          // K extent per source row of the subtract contraction (nKa*L padded to 4)
     std::vector<int> kti, ktj, bti, btj;
     std::vector<sfft::Seq> seqs;
     std::vector<sfft::CorrJob> jobs;
@@ -97,7 +97,7 @@ cudaError_t launch_lagsum(sfft_plan *p);
 cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS);
 cudaError_t launch_gather(sfft_plan *p);
 cudaError_t launch_solve(sfft_plan *p, double *d_coef);
-int subtract_tap_width(int L);
+int subtract_kpad(int nKa, int L);
 void prof_mark(sfft_plan *p, int mark);
 cudaError_t launch_subtract(sfft_plan *p, const double *d_coef, const double *dR, const double *dS, double *dD);
 
