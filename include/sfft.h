@@ -134,6 +134,11 @@ const char *sfft_strerror(int status);
 const char *sfft_last_cuda_error(const sfft_plan *plan);
 const char *sfft_version(void);
 
+/* Measurement support (not on the hot path): achieved FP64 throughput of the current device in TFLOP/s from a
+ * register-resident probe kernel, kind 0 = plain FMA pipe (DFMA), kind 1 = FP64 tensor cores (mma.sync.m8n8k4.f64).
+ * These are the denominators of the "alu" rooflines in DESIGN.md / bench.py.  Synchronous; best of 3 timed runs. */
+int sfft_measure_fp64_peak(int kind, double *tflops);
+
 #ifdef __cplusplus
 }
 #endif

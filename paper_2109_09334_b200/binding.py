@@ -22,6 +22,7 @@ EXPORTS = [
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
     "sfft_subtract", "sfft_plan_status", "sfft_run_host", "sfft_plan_launch_count", "sfft_plan_destroy",
     "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
+    "sfft_measure_fp64_peak",
 ]
 SFFT_NUM_STAGES = 8
 STAGE_NAMES = ["rowfft", "corr", "lagsum", "moments", "gather", "solve", "subtract_prep", "subtract"]
@@ -75,6 +76,7 @@ def load_library(build_if_missing=True):
         "sfft_version": (ctypes.c_char_p, []),
         "sfft_plan_profile": (ci, [vp, ci]),
         "sfft_plan_profile_read": (ci, [vp, vp, pci]),
+        "sfft_measure_fp64_peak": (ci, [ci, ctypes.POINTER(ctypes.c_double)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -91,6 +93,12 @@ def sfft_strerror(status):
 
 def sfft_version():
     return load_library().sfft_version().decode()
+
+
+def sfft_measure_fp64_peak(kind):
+    v = ctypes.c_double(0.0)
+    st = load_library().sfft_measure_fp64_peak(int(kind), ctypes.byref(v))
+    return st, v.value
 
 
 def sfft_plan_create(H, W, L, DK, DB, basis):

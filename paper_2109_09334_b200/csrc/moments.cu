@@ -43,27 +43,45 @@ __global__ void __launch_bounds__(128) k_dgemm(GemmArgs g) {
 #pragma unroll
         for (int b = 0; b < 4; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
 
-    for (int k0 = kbeg; k0 < kend; k0 += BK) {
-        __syncthreads();
+    // global -> register prefetch of the next K tile overlaps the MMAs of the current one
+    double ra[BM * BK / 128], rb[BN * BK / 128];
+    auto fetch = [&](int k0) {
+        const int ka0 = g.kmodA > 0 ? k0 % g.kmodA : k0;
 #pragma unroll
         for (int q = 0; q < BM * BK / 128; ++q) {
             const int i = tid + 128 * q, rr = i >> 4, kk = i & 15;
-            As[rr][kk] = (i0 + rr < g.M && k0 + kk < kend) ? __ldg(&A[(size_t)(i0 + rr) * g.lda + k0 + kk]) : 0.0;
+            ra[q] = (i0 + rr < g.M && k0 + kk < kend) ? __ldg(&A[(size_t)(i0 + rr) * g.lda + ka0 + kk]) : 0.0;
         }
         if (BT) {
 #pragma unroll
             for (int q = 0; q < BN * BK / 128; ++q) {
                 const int i = tid + 128 * q, rr = i >> 4, kk = i & 15;
-                Bs[rr][kk] = (j0 + rr < g.N && k0 + kk < kend) ? __ldg(&B[(size_t)(j0 + rr) * g.ldb + k0 + kk]) : 0.0;
+                rb[q] = (j0 + rr < g.N && k0 + kk < kend) ? __ldg(&B[(size_t)(j0 + rr) * g.ldb + k0 + kk]) : 0.0;
             }
         } else {
 #pragma unroll
             for (int q = 0; q < BN * BK / 128; ++q) {
                 const int i = tid + 128 * q, kk = i >> 6, nn = i & 63;
-                Bs[nn][kk] = (j0 + nn < g.N && k0 + kk < kend) ? __ldg(&B[(size_t)(k0 + kk) * g.ldb + j0 + nn]) : 0.0;
+                rb[q] = (j0 + nn < g.N && k0 + kk < kend) ? __ldg(&B[(size_t)(k0 + kk) * g.ldb + j0 + nn]) : 0.0;
             }
         }
+    };
+    if (kbeg < kend) fetch(kbeg);
+    for (int k0 = kbeg; k0 < kend; k0 += BK) {
         __syncthreads();
+#pragma unroll
+        for (int q = 0; q < BM * BK / 128; ++q) {
+            const int i = tid + 128 * q;
+            As[i >> 4][i & 15] = ra[q];
+        }
+#pragma unroll
+        for (int q = 0; q < BN * BK / 128; ++q) {
+            const int i = tid + 128 * q;
+            if (BT) Bs[i >> 4][i & 15] = rb[q];
+            else Bs[i & 63][i >> 6] = rb[q];
+        }
+        __syncthreads();
+        if (k0 + BK < kend) fetch(k0 + BK);
 #pragma unroll
         for (int ks = 0; ks < BK; ks += 4) {
             double af[4], bf[4];
@@ -105,6 +123,34 @@ __global__ void k_lambda_pick(const double *__restrict__ C, double *__restrict__
     tab[(size_t)bz * tab_size + off_la + i] = v;
 }
 
+// QS[x][j] = sum_y S(x,y) g'_j(y): one warp per image row, S streamed once (HBM-bound), NJ >= nBa accumulators per lane
+template <int NJ>
+__global__ void __launch_bounds__(256) k_rowdot(const double *__restrict__ S, const double *__restrict__ gB,
+                                                double *__restrict__ QS, int H, int W, int nBa) {
+    const int lane = threadIdx.x & 31, x = blockIdx.x * 8 + (threadIdx.x >> 5), bz = blockIdx.y;
+    if (x >= H) return;
+    const double2 *src = reinterpret_cast<const double2 *>(S + ((size_t)bz * H + x) * W);
+    double acc[NJ];
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) acc[j] = 0.0;
+    for (int y2 = lane; y2 < W / 2; y2 += 32) {
+        const double2 v = __ldg(&src[y2]);
+#pragma unroll
+        for (int j = 0; j < NJ; ++j)
+            if (j < nBa) {
+                const double2 gg = __ldg(reinterpret_cast<const double2 *>(gB + (size_t)j * W) + y2);
+                acc[j] = fma(v.x, gg.x, fma(v.y, gg.y, acc[j]));
+            }
+    }
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+        double v = acc[j];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0 && j < nBa) QS[((size_t)bz * H + x) * nBa + j] = v;
+    }
+}
+
 // Delta_s = sum_x f'_i(x) QS[x][j]   (one warp per s)
 __global__ void k_delta(const double *__restrict__ QS, const double *__restrict__ xwt, const int *__restrict__ bti,
                         const int *__restrict__ btj, double *__restrict__ tab, int H, int nKa, int nBa, int FB,
@@ -135,24 +181,29 @@ cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS) {
     // Q = R * cy^T
     GemmArgs g{};
     g.A = dR; g.B = p->dt.cy; g.C = p->Q; g.M = H; g.N = NC; g.K = W; g.lda = W; g.ldb = W; g.ldc = NC;
-    g.sA = P; g.sB = 0; g.sC = (long long)H * NC; g.sCk = 0; g.nz = p->nbatch; g.ksplit = 1; g.alpha = 1.0; g.beta = 0.0;
-    g.bT = true; g.lower = false;
+    g.sA = P; g.sB = 0; g.sC = (long long)p->ksq * H * NC; g.sCk = (long long)H * NC; g.nz = p->nbatch; g.ksplit = p->ksq;
+    g.alpha = 1.0; g.beta = 0.0; g.bT = true; g.lower = false; g.kmodA = 0;
     cudaError_t e = launch_dgemm(p, g);
     if (e != cudaSuccess) return e;
     // QS = S * gB^T
-    g.A = dS; g.B = p->dt.gB; g.C = p->QS; g.N = p->nBa; g.ldc = p->nBa; g.sC = (long long)H * p->nBa;
-    e = launch_dgemm(p, g);
-    if (e != cudaSuccess) return e;
-    // C = fx * Q   (split over K = H)
+    {
+        dim3 grid((H + 7) / 8, p->nbatch);
+        if (p->nBa <= 4) k_rowdot<4><<<grid, 256, 0, p->stream>>>(dS, p->dt.gB, p->QS, H, W, p->nBa);
+        else if (p->nBa <= 8) k_rowdot<8><<<grid, 256, 0, p->stream>>>(dS, p->dt.gB, p->QS, H, W, p->nBa);
+        else k_rowdot<12><<<grid, 256, 0, p->stream>>>(dS, p->dt.gB, p->QS, H, W, p->nBa);
+        p->launches++;
+    }
+    // C = fx * (sum of the ksq partial Q's): K = ksq stacked copies of the x axis, split in ksq*ksplit parts
+    const int parts = p->ksq * p->ksplit;
     GemmArgs h{};
-    h.A = p->dt.fx; h.B = p->Q; h.C = p->LamC; h.M = NC; h.N = NC; h.K = H; h.lda = H; h.ldb = NC; h.ldc = NC;
-    h.sA = 0; h.sB = (long long)H * NC; h.sC = (long long)p->ksplit * NC * NC; h.sCk = (long long)NC * NC;
-    h.nz = p->nbatch; h.ksplit = p->ksplit; h.alpha = 1.0; h.beta = 0.0; h.bT = false; h.lower = false;
+    h.A = p->dt.fx; h.B = p->Q; h.C = p->LamC; h.M = NC; h.N = NC; h.K = p->ksq * H; h.lda = H; h.ldb = NC; h.ldc = NC;
+    h.sA = 0; h.sB = (long long)p->ksq * H * NC; h.sC = (long long)parts * NC * NC; h.sCk = (long long)NC * NC;
+    h.nz = p->nbatch; h.ksplit = parts; h.alpha = 1.0; h.beta = 0.0; h.bT = false; h.lower = false; h.kmodA = H;
     e = launch_dgemm(p, h);
     if (e != cudaSuccess) return e;
     const int tot = p->FK * p->FB * p->L * p->L;
     k_lambda_pick<<<dim3((tot + 255) / 256, p->nbatch), 256, 0, p->stream>>>(
-        p->LamC, p->tab, p->dt.kti, p->dt.ktj, p->dt.bti, p->dt.btj, p->FK, p->FB, p->L, p->nBa, NC, p->ksplit, p->off_la,
+        p->LamC, p->tab, p->dt.kti, p->dt.ktj, p->dt.bti, p->dt.btj, p->FK, p->FB, p->L, p->nBa, NC, parts, p->off_la,
         p->tab_size);
     k_delta<<<dim3(p->FB, p->nbatch), 32, 0, p->stream>>>(p->QS, p->dt.xwt, p->dt.bti, p->dt.btj, p->tab, H, p->nKa, p->nBa,
                                                          p->FB, p->off_de, p->tab_size);

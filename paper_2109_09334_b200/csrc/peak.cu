@@ -1,0 +1,74 @@
+// FP64 throughput probes (measurement support for bench.py, not on the hot path): the peak of the plain
+// FP64 FMA pipe (DFMA) and of the FP64 tensor-core path (mma.sync.m8n8k4.f64 -> DMMA) on this device,
+// the denominators of the "alu" rooflines in DESIGN.md.  Register-resident operands, 8 independent
+// accumulator chains per thread / warp, no memory traffic.
+#include "sfft_internal.h"
+
+namespace sfft {
+namespace {
+
+__global__ void __launch_bounds__(256) k_peak_dfma(double *out, int iters, double a, double b) {
+    double c[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) c[q] = threadIdx.x * 1e-9 + q;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) c[q] = fma(c[q], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) s += c[q];
+    if (s == 123.456) out[0] = s;
+}
+
+__global__ void __launch_bounds__(256) k_peak_dmma(double *out, int iters, double a, double b) {
+    double c[8][2];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) c[q][0] = c[q][1] = threadIdx.x * 1e-9 + q;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                         : "+d"(c[q][0]), "+d"(c[q][1])
+                         : "d"(a), "d"(b));
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) s += c[q][0] + c[q][1];
+    if (s == 123.456) out[0] = s;
+}
+
+}  // namespace
+}  // namespace sfft
+
+extern "C" int sfft_measure_fp64_peak(int kind, double *tflops) {
+    if (!tflops || (kind != 0 && kind != 1)) return SFFT_ERR_INVALID_ARG;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return SFFT_ERR_CUDA;
+    }
+    double *d = nullptr;
+    if (cudaMalloc((void **)&d, 8) != cudaSuccess) { cudaGetLastError(); return SFFT_ERR_CUDA; }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 20000, blocks = sms * 8;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0);
+        if (kind == 0) sfft::k_peak_dfma<<<blocks, 256>>>(d, iters, 1.0000001, 1e-9);
+        else sfft::k_peak_dmma<<<blocks, 256>>>(d, iters, 1.0000001, 1e-9);
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        // DFMA: 2 flop per thread-op; DMMA m8n8k4: 2*8*8*4 = 512 flop per warp-op
+        const double flop = kind == 0 ? 2.0 * 8 * iters * 256.0 * blocks : 512.0 * 8 * iters * 8.0 * blocks;
+        if (rep > 0) best = best > flop / (ms * 1e-3) / 1e12 ? best : flop / (ms * 1e-3) / 1e12;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaError_t e = cudaGetLastError();
+    cudaFree(d);
+    *tflops = best;
+    return e == cudaSuccess ? SFFT_OK : SFFT_ERR_CUDA;
+}

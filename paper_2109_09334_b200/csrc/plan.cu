@@ -97,6 +97,10 @@ void choose_split(sfft_plan *p) {
         double cost = ceil(T / slots) / sx * (1.0 + 0.02 * sx);     // mild penalty: G traffic grows with sx
         if (cost < best) { best = cost; p->Sx = sx; }
     }
+    // y-range splits of the first moment GEMM (moments.cu): enough CTAs to fill the machine
+    const long tiles = (long)((p->H + 63) / 64) * ((p->NC + 63) / 64) * p->nbatch;
+    p->ksq = 1;
+    while (p->ksq < 8 && tiles * p->ksq < 4 * 148 && p->W / (2 * p->ksq) >= 256) p->ksq *= 2;
 }
 
 void build_jobs(sfft_plan *p) {
@@ -155,9 +159,9 @@ void build_jobs(sfft_plan *p) {
             if (rho >= 0) p->units.push_back({entry(tb, seqS, rho), +1, w, dst});
             else p->units.push_back({entry(seqS, tb, -rho), -1, w, dst});
         }
+    p->NC = p->nKa * p->nBa * L;
     choose_split(p);
     p->nch = (p->Nh + 1 + kLagChunk - 1) / kLagChunk;
-    p->NC = p->nKa * p->nBa * L;
     p->ksplit = std::max(1, std::min(16, p->H / 128));
 }
 
@@ -176,7 +180,7 @@ void free_tables(sfft_plan *p) {
 }
 
 struct WsLayout {
-    size_t rhat, G, lagpart, tab, Q, QS, LamC, M, rhs, Lf, dscale, kfold, ctab, flag, stR, stS, stD, stC, total;
+    size_t rhat, G, lagpart, tab, Q, QS, LamC, M, rhs, Lf, Winv, dscale, kfold, ctab, flag, stR, stS, stD, stC, total;
 };
 
 WsLayout ws_layout(const sfft_plan *p) {
@@ -187,12 +191,13 @@ WsLayout ws_layout(const sfft_plan *p) {
     l.G = take(nb * p->Sx * (size_t)(p->Nh + 1) * p->E * sizeof(double2));
     l.lagpart = take(nb * p->nch * (size_t)p->L * 2 * p->E * sizeof(double));
     l.tab = take(nb * p->tab_size * sizeof(double));
-    l.Q = take(nb * (size_t)p->H * p->NC * sizeof(double));
+    l.Q = take(nb * p->ksq * (size_t)p->H * p->NC * sizeof(double));
     l.QS = take(nb * (size_t)p->H * p->nBa * sizeof(double));
-    l.LamC = take(nb * p->ksplit * (size_t)p->NC * p->NC * sizeof(double));
+    l.LamC = take(nb * p->ksq * p->ksplit * (size_t)p->NC * p->NC * sizeof(double));
     l.M = take(nb * n * n * sizeof(double));
     l.rhs = take(nb * n * sizeof(double));
     l.Lf = take(nb * (n + 1) * (size_t)p->ldl * sizeof(double));
+    l.Winv = take(nb * (size_t)solve_num_blocks(p->n) * 64 * 64 * sizeof(double));
     l.dscale = take(nb * n * sizeof(double));
     l.kfold = take(nb * (size_t)p->FK * p->L * p->L * sizeof(double));
     l.ctab = take(nb * (size_t)p->H * p->L * p->LT * sizeof(double));
@@ -326,7 +331,7 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     p->ws = d_ws; p->ws_bytes = bytes;
     p->rhat = (double2 *)(b + l.rhat); p->G = (double2 *)(b + l.G); p->lagpart = (double *)(b + l.lagpart); p->tab = (double *)(b + l.tab);
     p->Q = (double *)(b + l.Q); p->QS = (double *)(b + l.QS); p->LamC = (double *)(b + l.LamC);
-    p->M = (double *)(b + l.M); p->rhs = (double *)(b + l.rhs); p->Lf = (double *)(b + l.Lf);
+    p->M = (double *)(b + l.M); p->rhs = (double *)(b + l.rhs); p->Lf = (double *)(b + l.Lf); p->Winv = (double *)(b + l.Winv);
     p->dscale = (double *)(b + l.dscale); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->flag = (int *)(b + l.flag);
     p->stageR = (double *)(b + l.stR); p->stageS = (double *)(b + l.stS); p->stageD = (double *)(b + l.stD);
     p->stageC = (double *)(b + l.stC);

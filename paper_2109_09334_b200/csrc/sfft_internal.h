@@ -63,7 +63,8 @@ struct sfft_plan {
     int nlb = 0;         // 8-lag blocks: ceil((L-1)/8)
     int nch = 0;         // column chunks of the lagsum partials
     int NC = 0;          // nKa*nBa*L columns of the moment GEMMs
-    int ksplit = 1;      // K splits of the second moment GEMM
+    int ksplit = 1;      // K (x-range) splits of the second moment GEMM
+    int ksq = 1;         // K (y-range) splits of the first moment GEMM; its partial Q's are summed by the second
     int npairs = 0;      // FK(FK+1)/2
     int ldl = 0;         // leading dimension of the Cholesky factor buffer (>= n+1)
     int LT = 0;          // K extent per source row of the subtract contraction (nKa*L padded to 4)
@@ -78,7 +79,7 @@ struct sfft_plan {
     void *ws = nullptr; size_t ws_bytes = 0;
     double2 *rhat = nullptr; double2 *G = nullptr; double *lagpart = nullptr; double *tab = nullptr;
     double *Q = nullptr, *QS = nullptr, *LamC = nullptr;
-    double *M = nullptr, *rhs = nullptr, *Lf = nullptr, *dscale = nullptr, *kfold = nullptr, *ctab = nullptr;
+    double *M = nullptr, *rhs = nullptr, *Lf = nullptr, *Winv = nullptr, *dscale = nullptr, *kfold = nullptr, *ctab = nullptr;
     double *stageR = nullptr, *stageS = nullptr, *stageD = nullptr, *stageC = nullptr;
     int *flag = nullptr;
     cudaStream_t stream = nullptr;
@@ -97,6 +98,7 @@ cudaError_t launch_lagsum(sfft_plan *p);
 cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS);
 cudaError_t launch_gather(sfft_plan *p);
 cudaError_t launch_solve(sfft_plan *p, double *d_coef);
+int solve_num_blocks(int n);     // 64-column panels of the Cholesky factorisation
 int subtract_kpad(int nKa, int L);
 void prof_mark(sfft_plan *p, int mark);
 cudaError_t launch_subtract(sfft_plan *p, const double *d_coef, const double *dR, const double *dS, double *dD);
@@ -110,6 +112,7 @@ struct GemmArgs {
     int M, N, K, lda, ldb, ldc;
     long long sA, sB, sC, sCk;
     int nz, ksplit;
+    int kmodA;      // > 0: A's column index is k mod kmodA (B's K axis is kmodA-periodic stacks of partial operands)
     double alpha, beta;
     bool bT, lower;
 };
