@@ -5,18 +5,17 @@
 //      factoring [[A, .],[r^T D, .]] leaves z = L^-1 D r in that row, so the forward
 //      substitution comes for free with the panel solves.
 //   2. Right-looking blocked Cholesky with one look-ahead step, panel width NB = 64, ONE launch
-//      per panel (k_chol_step).  Launch k holds three kinds of CTA:
+//      per panel (k_chol_step).  Launch k holds two kinds of CTA:
 //        P  (one per 64-row slab below the diagonal block of panel k): applies panel k-1 to its
 //           rows of column strip k and to the diagonal block (FP64 tensor cores), factors the
-//           64x64 diagonal block (every P CTA redundantly - that is cheaper than another launch),
-//           and solves its slab against it;
+//           64x64 diagonal block together with the inverse W of its factor (every P CTA redundantly -
+//           cheaper than another launch), and solves its slab as the dense contraction X = S W^T;
 //        U  (one per 64x64 tile of the lower triangle right of strip k): rank-64 update with
-//           panel k-1 on the FP64 tensor cores (mma.sync.m8n8k4.f64: a dense contraction);
-//        I  (one): inverse of the diagonal block of panel k-1, used by the back substitution.
+//           panel k-1 on the FP64 tensor cores (mma.sync.m8n8k4.f64: a dense contraction).
 //      P(k) needs only panel k-1 and the U updates of launch k-1, so the latency-bound panel
 //      chain (factor + triangular solve) overlaps the throughput-bound trailing update.
 //   3. Backward substitution L^T y = z by a thread-block cluster of 8 CTAs per system: the owner
-//      of diagonal block b forms y_b = W_b^T z_b (W_b = L_bb^-1 from the I CTAs), broadcasts it
+//      of diagonal block b forms y_b = W_b^T z_b (W_b = L_bb^-1 from the factorisation), broadcasts it
 //      through distributed shared memory, and every CTA updates the columns it owns.  c = D y.
 // A non-positive pivot writes its index to flag[2*b] (reported as SFFT_ERR_NOT_SPD).
 #include <cooperative_groups.h>
@@ -26,6 +25,14 @@
 #include "sfft_internal.h"
 
 namespace cg = cooperative_groups;
+
+// In-kernel phase timestamps for the development probe (compiled out of the library).
+#ifdef SFFT_PROBE
+__device__ long long g_probe[64 * 8];
+#define PROBE(k, i) do { if (blockIdx.x == 0 && threadIdx.x == 0) g_probe[(k) * 8 + (i)] = clock64(); } while (0)
+#else
+#define PROBE(k, i) do { } while (0)
+#endif
 
 namespace sfft {
 namespace {
@@ -59,15 +66,34 @@ __global__ void k_scale_copy(const double *__restrict__ M, const double *__restr
     Lf[((size_t)b * (n + 1) + i) * ldl + j] = v;
 }
 
-// T[r][c] = L[row0 + r][col0 + c] for r < nr (else 0), 64 columns, into an MMA operand tile (stride LDT)
-__device__ __forceinline__ void load_tile(double *T, const double *__restrict__ L, int ldl, int row0, int col0, int nr) {
-    for (int i = threadIdx.x; i < NB * NB / 2; i += 256) {
-        const int r = i >> 5, c = (i & 31) * 2;
-        double2 v = make_double2(0.0, 0.0);
-        if (r < nr) v = *reinterpret_cast<const double2 *>(&L[(size_t)(row0 + r) * ldl + col0 + c]);
-        T[r * LDT + c] = v.x;
-        T[r * LDT + c + 1] = v.y;
+// T[r][c] = L[row0 + r][col0 + c] for r < nr (else 0), 64 columns, into an MMA operand tile (stride LDT).
+// Split in an issue half (all global loads in flight at once) and a store half.
+struct TileRegs { double2 v[NB * NB / 2 / 256]; };
+__device__ __forceinline__ void tile_fetch(TileRegs &t, const double *L, int ldl, int row0, int col0, int nr) {
+#pragma unroll
+    for (int q = 0; q < NB * NB / 2 / 256; ++q) {
+        const int i = threadIdx.x + 256 * q, r = i >> 5, c = (i & 31) * 2;
+        t.v[q] = make_double2(0.0, 0.0);
+        if (r < nr) t.v[q] = *reinterpret_cast<const double2 *>(&L[(size_t)(row0 + r) * ldl + col0 + c]);
     }
+}
+__device__ __forceinline__ void tile_store(double *T, const TileRegs &t) {
+#pragma unroll
+    for (int q = 0; q < NB * NB / 2 / 256; ++q) {
+        const int i = threadIdx.x + 256 * q, r = i >> 5, c = (i & 31) * 2;
+        T[r * LDT + c] = t.v[q].x;
+        T[r * LDT + c + 1] = t.v[q].y;
+    }
+}
+
+// 1/x to full double precision for normal positive x: MUFU seed + two Newton steps (no slow-path call)
+__device__ __forceinline__ double fast_rcp(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
 }
 
 // acc += A B^T for 64x64x64 operand tiles in shared memory; warp w owns rows 16*(w>>1).., cols 32*(w&1)..
@@ -90,62 +116,69 @@ __device__ __forceinline__ void mma_64(const double *A, const double *B, double 
     }
 }
 
-// x L^T = a for one row held in registers (right-looking: after x[k] is final, the remaining
-// entries receive its contribution, so the dependent chain is one FMA + one multiply per column).
-// Ls = lower-triangular factor in shared memory (stride LDX), rs[k] = 1 / L[k][k].
-__device__ __forceinline__ void row_trsm(double (&x)[NB], const double *Ls, const double *rs) {
-#pragma unroll
-    for (int k = 0; k < NB; ++k) {
-        x[k] *= rs[k];
-#pragma unroll
-        for (int m = k + 1; m < NB; ++m) x[m] = fma(-x[k], Ls[m * LDX + k], x[m]);
-    }
-}
-
 // In-place Cholesky of the 64x64 block Dg (shared memory, stride LDX, lower triangle valid, identity
-// padded beyond nb) by all 256 threads.  Every thread keeps a 4x4 register tile (rows ty+16a, cols
-// tx+16b); step k publishes column k through a double-buffered shared column, so there is ONE barrier
-// per column; the column scaling by 1/sqrt(pivot) is deferred to the end.  rs[k] = 1/L[k][k] on exit.
-__device__ __forceinline__ void chol_64(double *Dg, double *colbuf, double *pivs, double *rs, int nb, int *flag,
-                                        int gidx0, bool report) {
+// padded beyond nb) by all 256 threads, together with the inverse of its factor: the elimination is
+// run on the augmented block [A | I], which turns I into W = L^-1.  Every thread keeps 4x4 register
+// tiles of A and of the augmented part (rows ty+16a, cols tx+16b); step k publishes column k of A and
+// row k of the augmented part through double-buffered shared vectors, so there is ONE barrier per
+// column; the scalings by 1/sqrt(pivot) are deferred to the end.
+// On exit: Wt[r*LDT + c] = W[r][c] (an MMA operand tile; may alias Dg), the factor L goes to global
+// memory Lg (stride ldl) and W to Wg (64x64, row-major) when `store` is set.
+__device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double *colbuf, double *rowbuf, double *pivs,
+                                            double *rs, int nb, int *flag, int gidx0, bool store, double *Lg, int ldl,
+                                            double *Wg) {
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-    double t[4][4];
+    double t[4][4], e[4][4];
 #pragma unroll
     for (int a = 0; a < 4; ++a)
 #pragma unroll
-        for (int b = 0; b < 4; ++b) t[a][b] = Dg[(ty + 16 * a) * LDX + tx + 16 * b];
+        for (int b = 0; b < 4; ++b) {
+            t[a][b] = Dg[(ty + 16 * a) * LDX + tx + 16 * b];
+            e[a][b] = (a == b && tx == ty) ? 1.0 : 0.0;
+        }
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
         for (int kk = 0; kk < 16; ++kk) {
             const int k = 16 * b + kk;
             if (k >= nb) break;                              // uniform
-            double *cb = colbuf + (k & 1) * NB;
+            double *cb = colbuf + (k & 1) * NB, *rb = rowbuf + (k & 1) * NB;
             if (tx == kk) {
 #pragma unroll
                 for (int a = 0; a < 4; ++a) cb[ty + 16 * a] = t[a][b];
             }
+            if (ty == kk) {
+#pragma unroll
+                for (int bb = 0; bb < 4; ++bb) rb[tx + 16 * bb] = e[b][bb];
+            }
             __syncthreads();
             double piv = cb[k];
             if (!(piv > 0.0)) {
-                if (report && tid == 0) atomicCAS(flag, -1, gidx0 + k);
+                if (store && tid == 0) atomicCAS(flag, -1, gidx0 + k);
                 piv = 1.0;
             }
             if (tid == 0) pivs[k] = piv;
-            const double inv = 1.0 / piv;
+            const double inv = fast_rcp(piv);
             double lr[4];
 #pragma unroll
-            for (int a = 0; a < 4; ++a) lr[a] = cb[ty + 16 * a];
+            for (int a = 0; a < 4; ++a) lr[a] = cb[ty + 16 * a] * inv;
 #pragma unroll
             for (int bb = b; bb < 4; ++bb) {
-                const double lc = cb[tx + 16 * bb] * inv;
+                const double lc = cb[tx + 16 * bb];
                 if (bb > b || tx > kk) {
 #pragma unroll
                     for (int a = 0; a < 4; ++a) t[a][bb] = fma(-lr[a], lc, t[a][bb]);
                 }
             }
+#pragma unroll
+            for (int bb = 0; bb <= b; ++bb) {
+                const double ec = rb[tx + 16 * bb];
+#pragma unroll
+                for (int a = b; a < 4; ++a)
+                    if (a > b || ty > kk) e[a][bb] = fma(-lr[a], ec, e[a][bb]);
+            }
         }
     }
-    __syncthreads();
+    __syncthreads();       // Dg fully consumed (registers), pivs complete
     if (tid < NB) rs[tid] = (tid < nb) ? rsqrt(pivs[tid]) : 1.0;
     __syncthreads();
 #pragma unroll
@@ -153,22 +186,24 @@ __device__ __forceinline__ void chol_64(double *Dg, double *colbuf, double *pivs
 #pragma unroll
         for (int b = 0; b < 4; ++b) {
             const int r = ty + 16 * a, c = tx + 16 * b;
-            double v = 0.0;
-            if (c < r) v = (r < nb) ? t[a][b] * rs[c] : 0.0;
-            else if (c == r) v = (r < nb) ? pivs[c] * rs[c] : 1.0;
-            Dg[r * LDX + c] = v;
+            const double w = e[a][b] * rs[r];
+            Wt[r * LDT + c] = w;
+            if (store) {
+                Wg[r * NB + c] = w;
+                if (r < nb && c <= r) Lg[(size_t)r * ldl + c] = (c < r) ? t[a][b] * rs[c] : pivs[c] * rs[c];
+            }
         }
     __syncthreads();
 }
 
-constexpr size_t kStepSmem = (size_t)(2 * NB * LDT + 2 * NB + NB + NB) * sizeof(double);
+constexpr size_t kStepSmem = (size_t)(2 * NB * LDT + 4 * NB + NB + NB) * sizeof(double);
 
-// One launch per panel k (see the header).  grid.x = nslab P CTAs, then ntiles U CTAs and one I CTA (k >= 1).
+// One launch per panel k (see the header).  grid.x = nslab P CTAs, then ntiles U CTAs (k >= 1).
 __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, double *__restrict__ Winv, int *flag, int n,
                                                    int ldl, int k, int nslab, int ntiles, int nblk) {
     extern __shared__ double sm[];
     double *T0 = sm, *T1 = sm + NB * LDT;                   // MMA operand tiles; later the factor / slab views
-    double *colbuf = sm + 2 * NB * LDT, *pivs = colbuf + 2 * NB, *rs = pivs + NB;
+    double *colbuf = sm + 2 * NB * LDT, *rowbuf = colbuf + 2 * NB, *pivs = rowbuf + 2 * NB, *rs = pivs + NB;
     const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int r8 = lane >> 2, kq = lane & 3, wm = (warp >> 1) * 16, wn = (warp & 1) * 32;
     double *L = Lf + (size_t)b * (n + 1) * ldl;
@@ -179,20 +214,13 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
         // ------------------------------ P: panel k ------------------------------
         const int r0 = j1 + bx * NB, nr = max(0, min(NB, n + 1 - r0));
         double accD[2][4][2], accX[2][4][2];
+        PROBE(k, 0);
 #pragma unroll
         for (int a = 0; a < 2; ++a)
 #pragma unroll
             for (int c = 0; c < 4; ++c) accD[a][c][0] = accD[a][c][1] = accX[a][c][0] = accX[a][c][1] = 0.0;
-        if (k > 0) {
-            load_tile(T0, L, ldl, j0, jp0, nb);      // diagonal-block rows of panel k-1
-            load_tile(T1, L, ldl, r0, jp0, nr);      // slab rows of panel k-1
-            __syncthreads();
-            mma_64(T0, T0, accD);
-            mma_64(T1, T0, accX);
-            __syncthreads();
-        }
-        // strip values minus the look-ahead update -> factor view Dg (T0) and slab view Xs (T1), stride LDX
-        double *Dg = T0, *Xs = T1;
+        // strip values (diagonal block and slab rows of strip k) in MMA fragment layout, fetched up front
+        double dv[2][4][2], xv[2][4][2];
 #pragma unroll
         for (int a = 0; a < 2; ++a)
 #pragma unroll
@@ -200,33 +228,59 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
                     const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq + q;
-                    double d = (r == cc) ? 1.0 : 0.0, x = 0.0;
-                    if (r < nb && cc <= r) d = L[(size_t)(j0 + r) * ldl + j0 + cc] - accD[a][c][q];
-                    if (r < nr && cc < nb) x = L[(size_t)(r0 + r) * ldl + j0 + cc] - accX[a][c][q];
-                    Dg[r * LDX + cc] = d;
-                    Xs[r * LDX + cc] = x;
+                    dv[a][c][q] = (r < nb && cc <= r) ? L[(size_t)(j0 + r) * ldl + j0 + cc] : ((r == cc) ? 1.0 : 0.0);
+                    xv[a][c][q] = (r < nr && cc < nb) ? L[(size_t)(r0 + r) * ldl + j0 + cc] : 0.0;
+                }
+        if (k > 0) {
+            TileRegs td, ts;
+            tile_fetch(td, L, ldl, j0, jp0, nb);     // diagonal-block rows of panel k-1
+            tile_fetch(ts, L, ldl, r0, jp0, nr);     // slab rows of panel k-1
+            tile_store(T0, td);
+            tile_store(T1, ts);
+            __syncthreads();
+            PROBE(k, 5);
+            mma_64(T0, T0, accD);
+            mma_64(T1, T0, accX);
+            __syncthreads();
+        }
+        PROBE(k, 1);
+        // strip values minus the look-ahead update -> factor view Dg (T0, stride LDX) and slab operand tile S (T1)
+        double *Dg = T0, *St = T1;
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq + q;
+                    const bool dl = (r < nb && cc <= r), xl = (r < nr && cc < nb);
+                    Dg[r * LDX + cc] = dl ? dv[a][c][q] - accD[a][c][q] : dv[a][c][q];
+                    St[r * LDT + cc] = xl ? xv[a][c][q] - accX[a][c][q] : 0.0;
                 }
         __syncthreads();
-        chol_64(Dg, colbuf, pivs, rs, nb, &flag[2 * b], j0, bx == 0);
-        if (bx == 0)
-            for (int i = tid; i < NB * NB; i += 256) {
-                const int r = i >> 6, c = i & 63;
-                if (r < nb && c <= r) L[(size_t)(j0 + r) * ldl + j0 + c] = Dg[r * LDX + c];
-            }
+        PROBE(k, 2);
+        // factor the diagonal block and invert its factor; W replaces Dg in T0 as an MMA operand tile
+        chol_inv_64(Dg, T0, colbuf, rowbuf, pivs, rs, nb, &flag[2 * b], j0, bx == 0, L + (size_t)j0 * ldl + j0, ldl,
+                    Winv + ((size_t)b * nblk + k) * NB * NB);
+        PROBE(k, 3);
         if (nr <= 0) return;
-        if (tid < nr) {
-            double x[NB];
+        // slab solve X L11^T = S as the dense contraction X = S W^T
 #pragma unroll
-            for (int c = 0; c < NB; ++c) x[c] = Xs[tid * LDX + c];
-            row_trsm(x, Dg, rs);
+        for (int a = 0; a < 2; ++a)
 #pragma unroll
-            for (int c = 0; c < NB; ++c) Xs[tid * LDX + c] = x[c];
-        }
-        __syncthreads();
-        for (int i = tid; i < NB * NB; i += 256) {
-            const int r = i >> 6, c = i & 63;
-            if (r < nr && c < nb) L[(size_t)(r0 + r) * ldl + j0 + c] = Xs[r * LDX + c];
-        }
+            for (int c = 0; c < 4; ++c) accX[a][c][0] = accX[a][c][1] = 0.0;
+        mma_64(St, T0, accX);
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq;
+                if (r >= nr) continue;
+                double *dst = &L[(size_t)(r0 + r) * ldl + j0 + cc];
+                if (cc + 1 < nb) *reinterpret_cast<double2 *>(dst) = make_double2(accX[a][c][0], accX[a][c][1]);
+                else if (cc < nb) dst[0] = accX[a][c][0];
+            }
+        PROBE(k, 4);
         return;
     }
     bx -= nslab;
@@ -238,8 +292,13 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
         const int tj = bx - ti * (ti + 1) / 2;
         const int i0 = j1 + ti * NB, c0 = j1 + tj * NB;
         const int nri = max(0, min(NB, n + 1 - i0)), nrj = max(0, min(NB, n - c0));
-        load_tile(T0, L, ldl, i0, jp0, nri);
-        if (tj != ti) load_tile(T1, L, ldl, c0, jp0, nrj);
+        {
+            TileRegs ta, tb;
+            tile_fetch(ta, L, ldl, i0, jp0, nri);
+            if (tj != ti) tile_fetch(tb, L, ldl, c0, jp0, nrj);
+            tile_store(T0, ta);
+            if (tj != ti) tile_store(T1, tb);
+        }
         __syncthreads();
         double acc[2][4][2];
 #pragma unroll
@@ -264,74 +323,73 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
             }
         return;
     }
-    // ------------------------------ I: W = inverse of the diagonal block of panel kI ------------------------------
-    {
-        const int kI = (k < nblk) ? k - 1 : nblk - 1;       // the launch after the last panel inverts the last block
-        const int q0 = kI * NB, nq = min(NB, n - q0);
-        double *Dg = T0;
-        for (int i = tid; i < NB * NB; i += 256) {
-            const int r = i >> 6, c = i & 63;
-            Dg[r * LDX + c] = (r < nq && c <= r) ? L[(size_t)(q0 + r) * ldl + q0 + c] : (r == c ? 1.0 : 0.0);
-        }
-        __syncthreads();
-        if (tid < NB) rs[tid] = 1.0 / Dg[tid * LDX + tid];
-        __syncthreads();
-        double *W = Winv + ((size_t)b * nblk + kI) * NB * NB;
-        if (tid < NB) {
-            double x[NB];
-#pragma unroll
-            for (int c = 0; c < NB; ++c) x[c] = (c == tid) ? 1.0 : 0.0;
-            row_trsm(x, Dg, rs);                    // x[c] = W[c][tid]
-#pragma unroll
-            for (int c = 0; c < NB; ++c) W[c * NB + tid] = x[c];
-        }
-    }
 }
 
 // Backward substitution L^T y = z (z = row n of Lf), c = D y.  One cluster of CS CTAs per system; CTA `rank`
-// owns the 64-column blocks with block % CS == rank and keeps their part of z in shared memory.
+// owns the 64-column blocks with block % CS == rank and keeps their part of z in shared memory.  Per diagonal
+// block (from the last): the owner forms y_b = W_b^T z_b, broadcasts it through distributed shared memory, and
+// after one cluster barrier every CTA subtracts L[b-rows][own columns]^T y_b from its part of z.  All global
+// loads of a step are issued as independent batches of 16 per thread (the step is L2-latency bound).
 __global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(256)
 k_chol_backsolve(const double *__restrict__ Lf, const double *__restrict__ Winv, const double *__restrict__ dscale,
-                 double *__restrict__ coef, int n, int ldl, int nblk) {
-    extern __shared__ double zs[];                 // [nblk * 64] (own blocks valid)
+                 double *__restrict__ coef, int n, int ldl, int nblk, int nown_max) {
+    extern __shared__ double zs[];                 // [nblk * 64] (own blocks valid), then part[4][nown_max * 64]
     __shared__ double ybuf[2][NB];
+    __shared__ double red[4][NB];
+    double *part = zs + (size_t)nblk * NB;
     cg::cluster_group cluster = cg::this_cluster();
     const int rank = (int)cluster.block_rank(), b = blockIdx.y, tid = threadIdx.x;
+    const int col = tid & 63, q = tid >> 6;
     const double *L = Lf + (size_t)b * (n + 1) * ldl;
     for (int i = tid; i < nblk * NB; i += 256) zs[i] = (i < n) ? L[(size_t)n * ldl + i] : 0.0;
     cluster.sync();
     for (int blk = nblk - 1; blk >= 0; --blk) {
         const int i0 = blk * NB, nbk = min(NB, n - i0);
-        if (rank == blk % CS && tid < NB) {
-            // y_i = sum_{k >= i} W[k][i] z_k
-            const double *W = Winv + ((size_t)b * nblk + blk) * NB * NB;
-            double y0 = 0.0, y1 = 0.0;
-            for (int k = tid; k < nbk; k += 2) {   // two chains; entries above the diagonal of W are zero
-                y0 = fma(W[k * NB + tid], zs[i0 + k], y0);
-                if (k + 1 < nbk) y1 = fma(W[(k + 1) * NB + tid], zs[i0 + k + 1], y1);
-            }
-            const double y = y0 + y1;
-            if (tid < nbk) coef[(size_t)b * n + i0 + tid] = y * dscale[(size_t)b * n + i0 + tid];
+        if (rank == blk % CS) {
+            // y_i = sum_k W[k][i] z_k  (W lower triangular, stored with its zeros): quarter q of the k range per thread
+            const double *W = Winv + ((size_t)b * nblk + blk) * NB * NB + (size_t)(16 * q) * NB + col;
+            double w[16];
 #pragma unroll
-            for (int c = 0; c < CS; ++c) cluster.map_shared_rank(&ybuf[blk & 1][0], c)[tid] = (tid < nbk) ? y : 0.0;
+            for (int k = 0; k < 16; ++k) w[k] = W[k * NB];
+            double y0 = 0.0, y1 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 16; k += 2) {
+                y0 = fma(w[k], zs[i0 + 16 * q + k], y0);
+                y1 = fma(w[k + 1], zs[i0 + 16 * q + k + 1], y1);
+            }
+            red[q][col] = y0 + y1;
+            __syncthreads();
+            if (tid < NB) {
+                const double y = (red[0][tid] + red[1][tid]) + (red[2][tid] + red[3][tid]);
+                if (tid < nbk) coef[(size_t)b * n + i0 + tid] = y * dscale[(size_t)b * n + i0 + tid];
+#pragma unroll
+                for (int c = 0; c < CS; ++c) cluster.map_shared_rank(&ybuf[blk & 1][0], c)[tid] = (tid < nbk) ? y : 0.0;
+            }
         }
         cluster.sync();
         // z_j -= sum_k L[i0 + k][j] y_k for the columns of the blocks this CTA owns below blk (nearest first)
-        const int col = tid & 63, slot = tid >> 6;
         const double *yb = ybuf[blk & 1];
-        int first = blk - 1 - ((blk - 1 - rank) % CS + CS) % CS;      // largest owned block < blk
-        for (int ob = first - slot * CS; ob >= 0; ob -= 4 * CS) {
-            const double *src = L + (size_t)i0 * ldl + ob * NB + col;
-            double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-            int kk = 0;
-            for (; kk + 4 <= nbk; kk += 4) {
-                s0 = fma(src[(size_t)kk * ldl], yb[kk], s0);
-                s1 = fma(src[(size_t)(kk + 1) * ldl], yb[kk + 1], s1);
-                s2 = fma(src[(size_t)(kk + 2) * ldl], yb[kk + 2], s2);
-                s3 = fma(src[(size_t)(kk + 3) * ldl], yb[kk + 3], s3);
+        const int first = blk - 1 - ((blk - 1 - rank) % CS + CS) % CS;      // largest owned block < blk
+        const int nown = first >= 0 ? first / CS + 1 : 0;
+        for (int o = 0; o < nown; ++o) {
+            const int ob = first - o * CS;
+            const double *src = L + (size_t)(i0 + 16 * q) * ldl + ob * NB + col;
+            double v[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k) v[k] = (16 * q + k < nbk) ? src[(size_t)k * ldl] : 0.0;
+            double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 16; k += 2) {
+                s0 = fma(v[k], yb[16 * q + k], s0);
+                s1 = fma(v[k + 1], yb[16 * q + k + 1], s1);
             }
-            for (; kk < nbk; ++kk) s0 = fma(src[(size_t)kk * ldl], yb[kk], s0);
-            zs[ob * NB + col] -= (s0 + s1) + (s2 + s3);
+            part[((size_t)q * nown_max + o) * NB + col] = s0 + s1;
+        }
+        __syncthreads();
+        for (int o = q; o < nown; o += 4) {
+            const int ob = first - o * CS;
+            const size_t po = (size_t)o * NB + col, ps = (size_t)nown_max * NB;
+            zs[ob * NB + col] -= (part[po] + part[ps + po]) + (part[2 * ps + po] + part[3 * ps + po]);
         }
         __syncthreads();
     }
@@ -348,21 +406,19 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     p->launches += 2;
     cudaError_t e = cudaFuncSetAttribute(k_chol_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStepSmem);
     if (e != cudaSuccess) return e;
-    for (int k = 0; k <= nblk; ++k) {
-        int nslab = 0, ntiles = 0;
-        if (k < nblk) {
-            const int j1 = std::min(n, (k + 1) * NB);
-            nslab = (n + 1 - j1 + NB - 1) / NB;                       // rows j1..n (the rhs row is row n)
-            if (k > 0) { const int nt = nslab; ntiles = nt * (nt + 1) / 2; }
-        }
-        const int grid = nslab + ntiles + (k > 0 ? 1 : 0);
-        k_chol_step<<<dim3(grid, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, nslab, ntiles, nblk);
+    for (int k = 0; k < nblk; ++k) {
+        const int j1 = std::min(n, (k + 1) * NB);
+        const int nslab = (n + 1 - j1 + NB - 1) / NB;                 // rows j1..n (the rhs row is row n)
+        const int ntiles = k > 0 ? nslab * (nslab + 1) / 2 : 0;
+        k_chol_step<<<dim3(nslab + ntiles, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, nslab,
+                                                                               ntiles, nblk);
         p->launches++;
     }
-    const size_t smem = (size_t)nblk * NB * sizeof(double);
+    const int nown_max = (nblk + CS - 1) / CS;
+    const size_t smem = ((size_t)nblk * NB + 4 * (size_t)nown_max * NB) * sizeof(double);
     e = cudaFuncSetAttribute(k_chol_backsolve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_chol_backsolve<<<dim3(CS, nbat), 256, smem, p->stream>>>(p->Lf, p->Winv, p->dscale, d_coef, n, ldl, nblk);
+    k_chol_backsolve<<<dim3(CS, nbat), 256, smem, p->stream>>>(p->Lf, p->Winv, p->dscale, d_coef, n, ldl, nblk, nown_max);
     p->launches++;
     return cudaGetLastError();
 }
