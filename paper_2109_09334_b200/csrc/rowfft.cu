@@ -11,6 +11,7 @@
 // radix-4 passes plus one radix-2 pass when log2 is odd, ping-pong in shared memory)
 // followed by the even/odd split.  HBM-bound: one 16-byte load and one 16-byte store per
 // complex point, both fully coalesced.
+#include "fft_regs.cuh"
 #include "sfft_internal.h"
 
 namespace sfft {
@@ -131,6 +132,64 @@ cudaError_t launch_fwd(sfft_plan *p, const double *dR, const double *dS) {
     return cudaGetLastError();
 }
 
+// Register-tiled variant for NH >= 512 (fft_regs.cuh): three radix-16/16/R3 passes, RPC rows per CTA.
+// grid: x = image slot, y = row group, z = batch entry; block: (NH/16, RPC).
+template <int NH>
+__global__ void __launch_bounds__(FftCfg<NH>::T * (FftCfg<NH>::T >= 128 ? 1 : 128 / FftCfg<NH>::T))
+k_rowfft_forward16(const double *__restrict__ R, const double *__restrict__ S, const double *__restrict__ gK,
+                   const double2 *__restrict__ twW, double2 *__restrict__ rhat, int H, int nKa) {
+    using C = FftCfg<NH>;
+    constexpr int T = C::T, RPC = T >= 128 ? 1 : 128 / T, W = 2 * NH;
+    extern __shared__ double2 sm2[];
+    double2 *tw2 = sm2, *buf = sm2 + C::TW2 + threadIdx.y * C::BUF;
+    const int tid = threadIdx.x, img = blockIdx.x, x = blockIdx.y * RPC + threadIdx.y, bz = blockIdx.z;
+    if (threadIdx.y == 0) fft_load_tw2<NH>(tw2, twW);
+    const double2 *src = reinterpret_cast<const double2 *>((img < nKa ? R : S) + ((size_t)bz * H + x) * W);
+    double2 v[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) v[r] = __ldg(&src[tid + r * T]);          // z[n] = a[2n] + i a[2n+1]
+    if (img < nKa) {
+        const double2 *g = reinterpret_cast<const double2 *>(gK + (size_t)img * W);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const double2 gg = __ldg(&g[tid + r * T]);
+            v[r].x *= gg.x;
+            v[r].y *= gg.y;
+        }
+    }
+    __syncthreads();                                                       // tw2 visible
+    fft_core<NH>(v, buf, tw2, twW);
+    double2 *dst = rhat + (((size_t)bz * (nKa + 1) + img) * H + x) * NH;
+    // even/odd split (see k_rowfft_forward)
+    for (int k = tid; k <= NH / 2; k += T) {
+        if (k == 0) {
+            const double2 z0 = buf[0];
+            dst[0] = make_double2(z0.x + z0.y, z0.x - z0.y);
+        } else {
+            const double2 zk = buf[k], zn = buf[NH - k];
+            const double2 E = make_double2(0.5 * (zk.x + zn.x), 0.5 * (zk.y - zn.y));
+            const double2 O = make_double2(0.5 * (zk.y + zn.y), -0.5 * (zk.x - zn.x));
+            const double2 wO = cmul(__ldg(&twW[k]), O);
+            dst[k] = make_double2(E.x + wO.x, E.y + wO.y);
+            if (k != NH - k) dst[NH - k] = make_double2(E.x - wO.x, -(E.y - wO.y));
+        }
+    }
+}
+
+template <int NH>
+cudaError_t launch_fwd16(sfft_plan *p, const double *dR, const double *dS) {
+    using C = FftCfg<NH>;
+    constexpr int T = C::T, RPC = T >= 128 ? 1 : 128 / T;
+    const size_t smem = (size_t)(C::TW2 + RPC * C::BUF) * sizeof(double2);
+    auto kern = k_rowfft_forward16<NH>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid(p->nimg, p->H / RPC, p->nbatch);
+    kern<<<grid, dim3(T, RPC), smem, p->stream>>>(dR, dS, p->dt.gK, p->dt.twW, p->rhat, p->H, p->nKa);
+    p->launches++;
+    return cudaGetLastError();
+}
+
 }  // namespace
 
 cudaError_t launch_rowfft_forward(sfft_plan *p, const double *dR, const double *dS) {
@@ -139,10 +198,10 @@ cudaError_t launch_rowfft_forward(sfft_plan *p, const double *dR, const double *
         case 64: return launch_fwd<64>(p, dR, dS);
         case 128: return launch_fwd<128>(p, dR, dS);
         case 256: return launch_fwd<256>(p, dR, dS);
-        case 512: return launch_fwd<512>(p, dR, dS);
-        case 1024: return launch_fwd<1024>(p, dR, dS);
-        case 2048: return launch_fwd<2048>(p, dR, dS);
-        case 4096: return launch_fwd<4096>(p, dR, dS);
+        case 512: return launch_fwd16<512>(p, dR, dS);
+        case 1024: return launch_fwd16<1024>(p, dR, dS);
+        case 2048: return launch_fwd16<2048>(p, dR, dS);
+        case 4096: return launch_fwd16<4096>(p, dR, dS);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -66,6 +66,8 @@ CASES = [
     (4, 256, 128, 17, None, None, None),              # L=17 taps
     (2, 64, 64, 1, None, 2, 1),                       # L=1: no kernel lags, only scale + background
     (2, 64, 8192, 3, None, 0, 0),                     # longest row FFT (W=8192), constant kernel
+    (2, 64, 2048, 3, None, 1, 1),                     # W=2048 row FFT (radix 16-16-4)
+    (3, 64, 4096, 5, None, 2, 1),                     # W=4096 row FFT (radix 16-16-8), the headline width
     (2, 128, 128, 9, None, 1, 2),                     # L without an exact subtract instantiation (padded taps)
     (5, 128, 128, 5, "bspline", 1, 0),                # B-spline weights
     (5, 256, 256, 5, "bspline", 4, 4),                # config-5 basis (8x8 functions), n = 1664
