@@ -122,11 +122,12 @@ __device__ __forceinline__ void mma_64(const double *A, const double *B, double 
 // tiles of A and of the augmented part (rows ty+16a, cols tx+16b); step k publishes column k of A and
 // row k of the augmented part through double-buffered shared vectors, so there is ONE barrier per
 // column; the scalings by 1/sqrt(pivot) are deferred to the end.
-// On exit: Wt[r*LDT + c] = W[r][c] (an MMA operand tile; may alias Dg), the factor L goes to global
-// memory Lg (stride ldl) and W to Wg (64x64, row-major) when `store` is set.
+// On exit: Wt[r*LDT + c] = W[r][c] (an MMA operand tile; may alias Dg) and, when `store` is set, W goes
+// to Wg (64x64, row-major).  The factor's diagonal block itself is NOT written back: nothing downstream
+// reads it (the back substitution uses W), and the other P CTAs of this launch - which may be scheduled
+// after this one has finished when the grid exceeds one wave - still read the unfactored block from Lf.
 __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double *colbuf, double *rowbuf, double *pivs,
-                                            double *rs, int nb, int *flag, int gidx0, bool store, double *Lg, int ldl,
-                                            double *Wg) {
+                                            double *rs, int nb, int *flag, int gidx0, bool store, double *Wg) {
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
     double t[4][4], e[4][4];
 #pragma unroll
@@ -188,10 +189,7 @@ __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double
             const int r = ty + 16 * a, c = tx + 16 * b;
             const double w = e[a][b] * rs[r];
             Wt[r * LDT + c] = w;
-            if (store) {
-                Wg[r * NB + c] = w;
-                if (r < nb && c <= r) Lg[(size_t)r * ldl + c] = (c < r) ? t[a][b] * rs[c] : pivs[c] * rs[c];
-            }
+            if (store) Wg[r * NB + c] = w;
         }
     __syncthreads();
 }
@@ -260,7 +258,7 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
         __syncthreads();
         PROBE(k, 2);
         // factor the diagonal block and invert its factor; W replaces Dg in T0 as an MMA operand tile
-        chol_inv_64(Dg, T0, colbuf, rowbuf, pivs, rs, nb, &flag[2 * b], j0, bx == 0, L + (size_t)j0 * ldl + j0, ldl,
+        chol_inv_64(Dg, T0, colbuf, rowbuf, pivs, rs, nb, &flag[2 * b], j0, bx == 0,
                     Winv + ((size_t)b * nblk + k) * NB * NB);
         PROBE(k, 3);
         if (nr <= 0) return;

@@ -132,6 +132,26 @@ def test_batch_matches_single(cuda_device):
         assert np.max(np.abs(D[e] - Do)) <= TOL_D * pb.sigma
 
 
+def test_batch_solve_grid_beyond_one_wave(cuda_device):
+    """nbatch = 5 systems of n = 1664: each factorisation launch holds ~1900 CTAs, several waves, so the
+    panel CTAs of the later batch entries start after those of the first have finished (a write-back of
+    the factored diagonal block would then be read as input by late CTAs).  Last entry against the
+    oracle, every entry against the same pair run alone."""
+    import torch
+    nb, L, DK, DB = 5, 5, 4, 4
+    pb = synth.make_batch(5, nbatch=nb, H=256, W=256)
+    M, rhs, c, D = _gpu_all(torch, pb, L, "bspline", DK, DB)
+    for e in range(nb):
+        M1, r1, c1, D1 = _gpu_all(torch, pb, L, "bspline", DK, DB, R=pb.R[e], S=pb.S[e])
+        assert np.max(np.abs(c[e] - c1[0])) <= TOL_C * np.max(np.abs(c1[0]))
+        assert np.max(np.abs(D[e] - D1)) <= TOL_D * pb.sigma
+    e = nb - 1
+    Mo, ro, co, Do = _oracle_all(pb.R[e], pb.S[e], L, "bspline", DK, DB)
+    _check_system(M[e], rhs[e], Mo, ro, pb.S[e])
+    _check_coef(c[e], co, Mo.shape[0] - 64)
+    assert np.max(np.abs(D[e] - Do)) <= TOL_D * pb.sigma
+
+
 def test_identical_images(cuda_device):
     """S = R  =>  a_{0,centre} = 1, everything else 0, D = 0 (degenerate but full-rank case)."""
     import torch
