@@ -101,7 +101,13 @@ int sfft_solve(sfft_plan *plan, double *d_coef);
 /* Steps a7-a8: D = S - sum_t sum_ab k_{t,ab} R^t((x-a)%H,(y-b)%W) - sum_s b_s T'_s  (Eqs. 1, 12)
  * with k the delta-basis coefficients folded back to pixel kernels (Eqs. 3-4).  (d_R, d_S)
  * may differ from the fitted pair (fit on the masked pair, apply to the
- * original).  d_D [nbatch][H][W] may alias d_S; no other aliasing. */
+ * original).  d_D [nbatch][H][W] may alias d_S; no other aliasing.
+ * Two routes, chosen by the plan from its sizes: the direct tensor-core contraction, or (wide
+ * kernels on rows of >= 1024 pixels) a FIR filter along x on the row spectra followed by one
+ * inverse row transform.  The second route reuses the row spectra of d_R computed by the last
+ * sfft_build_system when d_R is the very pointer passed to it: in that case the contents of
+ * d_R must not have changed since that call (pass another buffer, or call sfft_build_system
+ * again, otherwise).  It overwrites the workspace slot holding the row spectrum of S. */
 int sfft_subtract(sfft_plan *plan, const double *d_coef, const double *d_R, const double *d_S, double *d_D);
 
 /* Synchronise the plan's stream and report numerical status.  On SFFT_ERR_NOT_SPD, *info =

@@ -180,7 +180,7 @@ void free_tables(sfft_plan *p) {
 }
 
 struct WsLayout {
-    size_t rhat, G, lagpart, tab, Q, QS, LamC, M, rhs, Lf, Winv, dscale, kfold, ctab, flag, stR, stS, stD, stC, total;
+    size_t rhat, G, lagpart, tab, Q, QS, LamC, M, rhs, Lf, Winv, dscale, kfold, ctab, khat, flag, stR, stS, stD, stC, total;
 };
 
 WsLayout ws_layout(const sfft_plan *p) {
@@ -201,6 +201,7 @@ WsLayout ws_layout(const sfft_plan *p) {
     l.dscale = take(nb * n * sizeof(double));
     l.kfold = take(nb * (size_t)p->FK * p->L * p->L * sizeof(double));
     l.ctab = take(nb * (size_t)p->H * p->L * p->LT * sizeof(double));
+    l.khat = take(subtract_use_fourier(p) ? nb * (size_t)p->L * p->FK * p->Nh * sizeof(double2) : 0);
     l.flag = take(nb * sizeof(int) * 2);
     l.stR = take(nb * P * sizeof(double));
     l.stS = take(nb * P * sizeof(double));
@@ -332,10 +333,11 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     p->rhat = (double2 *)(b + l.rhat); p->G = (double2 *)(b + l.G); p->lagpart = (double *)(b + l.lagpart); p->tab = (double *)(b + l.tab);
     p->Q = (double *)(b + l.Q); p->QS = (double *)(b + l.QS); p->LamC = (double *)(b + l.LamC);
     p->M = (double *)(b + l.M); p->rhs = (double *)(b + l.rhs); p->Lf = (double *)(b + l.Lf); p->Winv = (double *)(b + l.Winv);
-    p->dscale = (double *)(b + l.dscale); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->flag = (int *)(b + l.flag);
+    p->dscale = (double *)(b + l.dscale); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
     p->stageR = (double *)(b + l.stR); p->stageS = (double *)(b + l.stS); p->stageD = (double *)(b + l.stD);
     p->stageC = (double *)(b + l.stC);
     p->built = p->solved = false;
+    p->rhat_valid = false;
     return SFFT_OK;
 }
 
@@ -347,6 +349,7 @@ int sfft_build_system(sfft_plan *p, const double *d_R, const double *d_S) {
     if (p->prof_steps > 0) p->prof_cur = p->prof_cur + 1;   // a build opens the next profiled step
     prof_mark(p, 0);
     if (e == cudaSuccess) e = launch_rowfft_forward(p, d_R, d_S);
+    p->rhat_src = d_R; p->rhat_valid = (e == cudaSuccess);
     prof_mark(p, 1);
     if (e == cudaSuccess) e = launch_corr(p);
     prof_mark(p, 2);

@@ -126,7 +126,7 @@ cudaError_t launch_fwd(sfft_plan *p, const double *dR, const double *dS) {
     auto kern = k_rowfft_forward<NH, T>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    dim3 grid(p->nimg, p->H, p->nbatch);
+    dim3 grid(dS ? p->nimg : p->nKa, p->H, p->nbatch);     // dS == nullptr: the weighted R rows only
     kern<<<grid, T, smem, p->stream>>>(dR, dS, p->dt.gK, p->dt.twW, p->rhat, p->H, p->nKa);
     p->launches++;
     return cudaGetLastError();
@@ -184,7 +184,7 @@ cudaError_t launch_fwd16(sfft_plan *p, const double *dR, const double *dS) {
     auto kern = k_rowfft_forward16<NH>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    dim3 grid(p->nimg, p->H / RPC, p->nbatch);
+    dim3 grid(dS ? p->nimg : p->nKa, p->H / RPC, p->nbatch);
     kern<<<grid, dim3(T, RPC), smem, p->stream>>>(dR, dS, p->dt.gK, p->dt.twW, p->rhat, p->H, p->nKa);
     p->launches++;
     return cudaGetLastError();

@@ -80,6 +80,9 @@ struct sfft_plan {
     double2 *rhat = nullptr; double2 *G = nullptr; double *lagpart = nullptr; double *tab = nullptr;
     double *Q = nullptr, *QS = nullptr, *LamC = nullptr;
     double *M = nullptr, *rhs = nullptr, *Lf = nullptr, *Winv = nullptr, *dscale = nullptr, *kfold = nullptr, *ctab = nullptr;
+    double2 *khat = nullptr;                    // [b][L*FK][Nh] row spectra of the pixel kernels (Fourier-route subtract)
+    const double *rhat_src = nullptr;           // device buffer whose weighted row spectra rhat[0..nKa) currently holds
+    bool rhat_valid = false;
     double *stageR = nullptr, *stageS = nullptr, *stageD = nullptr, *stageC = nullptr;
     int *flag = nullptr;
     cudaStream_t stream = nullptr;
@@ -92,7 +95,7 @@ struct sfft_plan {
 
 namespace sfft {
 // stage launchers (each returns cudaError_t of the launch); all enqueue on p->stream
-cudaError_t launch_rowfft_forward(sfft_plan *p, const double *dR, const double *dS);
+cudaError_t launch_rowfft_forward(sfft_plan *p, const double *dR, const double *dS);   // dS == nullptr: R rows only
 cudaError_t launch_corr(sfft_plan *p);
 cudaError_t launch_lagsum(sfft_plan *p);
 cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS);
@@ -102,6 +105,9 @@ int solve_num_blocks(int n);     // 64-column panels of the Cholesky factorisati
 int subtract_kpad(int nKa, int L);
 void prof_mark(sfft_plan *p, int mark);
 cudaError_t launch_subtract(sfft_plan *p, const double *d_coef, const double *dR, const double *dS, double *dD);
+cudaError_t launch_fold_coef(sfft_plan *p, const double *d_coef);          // delta-basis coefficients -> pixel kernels
+bool subtract_use_fourier(const sfft_plan *p);                              // route choice of sfft_subtract
+cudaError_t launch_subtract_fourier(sfft_plan *p, const double *d_coef, const double *dR, const double *dS, double *dD);
 
 // C[M x N] (ldc) = alpha * A[M x K] (lda, row-major) * B + beta * C  on the FP64 tensor cores.
 // bT = true : B given as [N x K] row-major (ldb)  ("A B^T");  false : B is [K x N] row-major.

@@ -159,20 +159,27 @@ cudaError_t launch_sub(sfft_plan *p, const double *d_coef, const double *dR, con
 
 }  // namespace
 
+cudaError_t launch_fold_coef(sfft_plan *p, const double *d_coef) {
+    k_fold_coef<<<dim3(p->FK, p->nbatch), 128, 0, p->stream>>>(d_coef, p->kfold, p->n, p->FK, p->L * p->L);
+    p->launches++;
+    return cudaGetLastError();
+}
+
 // K extent of one source row of the subtract contraction: nKa*L padded to whole k4 steps
 int subtract_kpad(int nKa, int L) { return 4 * ((nKa * L + 3) / 4); }
 
 cudaError_t launch_subtract(sfft_plan *p, const double *d_coef, const double *dR, const double *dS, double *dD) {
-    const int LL = p->L * p->L;
+    if (subtract_use_fourier(p)) return launch_subtract_fourier(p, d_coef, dR, dS, dD);
     SubDims d{};
     d.H = p->H; d.W = p->W; d.L = p->L; d.w = p->w; d.nKa = p->nKa; d.FB = p->FB; d.n = p->n;
     d.KP = subtract_kpad(p->nKa, p->L); d.NKS = d.KP / 4;
     d.ASTR = ((d.KP + 15) / 16) * 16 + 4;
     d.NSRC = p->L + 7;
-    k_fold_coef<<<dim3(p->FK, p->nbatch), 128, 0, p->stream>>>(d_coef, p->kfold, p->n, p->FK, LL);
+    cudaError_t e = launch_fold_coef(p, d_coef);
+    if (e != cudaSuccess) return e;
     k_coef_rows<<<dim3(p->H, p->nbatch), 256, 0, p->stream>>>(p->kfold, p->dt.xwt, p->dt.kti, p->dt.ktj, p->ctab, p->H,
                                                              p->nKa, p->FK, p->L, d.KP);
-    p->launches += 2;
+    p->launches++;
     prof_mark(p, 9);
     if (p->W >= 512) return launch_sub<8>(p, d_coef, dR, dS, dD, d);
     if (p->W >= 256) return launch_sub<4>(p, d_coef, dR, dS, dD, d);

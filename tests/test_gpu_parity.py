@@ -69,6 +69,10 @@ CASES = [
     (2, 64, 2048, 3, None, 1, 1),                     # W=2048 row FFT (radix 16-16-4)
     (3, 64, 4096, 5, None, 2, 1),                     # W=4096 row FFT (radix 16-16-8), the headline width
     (2, 128, 128, 9, None, 1, 2),                     # L without an exact subtract instantiation (padded taps)
+    (2, 64, 1024, 9, None, 2, 1),                     # Fourier-route subtract (W >= 1024, L >= 9), 2w % 4 == 0
+    (2, 256, 1024, 11, None, 1, 0),                   # Fourier route, 2w % 4 == 2 (padded lead-in), several x-ranges
+    (3, 128, 2048, 15, None, 2, 2),                   # Fourier route, L = 15
+    (4, 64, 4096, 17, None, 2, 2),                    # Fourier route at the headline width and kernel size
     (5, 128, 128, 5, "bspline", 1, 0),                # B-spline weights
     (5, 256, 256, 5, "bspline", 4, 4),                # config-5 basis (8x8 functions), n = 1664
 ]
@@ -152,6 +156,18 @@ def test_batch_solve_grid_beyond_one_wave(cuda_device):
     assert np.max(np.abs(D[e] - Do)) <= TOL_D * pb.sigma
 
 
+def test_batch_fourier_route(cuda_device):
+    """nbatch = 2 through the Fourier-route subtract (per-entry kernel spectra and spectrum stacks)."""
+    import torch
+    pb = synth.make_batch(5, nbatch=2, H=64, W=1024)
+    L, DK, DB = 9, 1, 1
+    M, rhs, c, D = _gpu_all(torch, pb, L, "poly", DK, DB)
+    for e in range(2):
+        Mo, ro, co, Do = _oracle_all(pb.R[e], pb.S[e], L, "poly", DK, DB)
+        _check_coef(c[e], co, Mo.shape[0] - 3)
+        assert np.max(np.abs(D[e] - Do)) <= TOL_D * pb.sigma
+
+
 def test_identical_images(cuda_device):
     """S = R  =>  a_{0,centre} = 1, everything else 0, D = 0 (degenerate but full-rank case)."""
     import torch
@@ -162,10 +178,14 @@ def test_identical_images(cuda_device):
     assert np.max(np.abs(D)) <= TOL_D * p.sigma
 
 
-def test_fit_on_one_pair_apply_to_another_and_inplace(cuda_device):
-    """solve on the masked pair, apply to the original pair; D may alias S."""
+@pytest.mark.parametrize("H,W,L", [(None, None, None), (64, 1024, 9)])
+def test_fit_on_one_pair_apply_to_another_and_inplace(cuda_device, H, W, L):
+    """solve on the masked pair, apply to the original pair; D may alias S.
+    The second shape takes the Fourier-route subtract, which must transform the new R itself
+    (the row spectra cached by build belong to the masked reference)."""
     import torch
-    p = synth.make_pair(1)
+    p = synth.make_pair(1, H=H, W=W)
+    p.L = p.L if L is None else L
     mask = np.ones_like(p.R); mask[40:60, 30:50] = 0.0
     Rm, Sm = p.R * mask + 100.0 * (1 - mask), p.S * mask + 100.0 * (1 - mask)
     Mo, ro = oracle.normal_from_lags(Rm, Sm, p.L, oracle.POLY, p.DK, p.DB)
