@@ -151,18 +151,42 @@ __global__ void __launch_bounds__(256) k_rowdot(const double *__restrict__ S, co
     }
 }
 
-// Delta_s = sum_x f'_i(x) QS[x][j]   (one warp per s)
-__global__ void k_delta(const double *__restrict__ QS, const double *__restrict__ xwt, const int *__restrict__ bti,
-                        const int *__restrict__ btj, double *__restrict__ tab, int H, int nKa, int nBa, int FB,
-                        size_t off_de, size_t tab_size) {
-    const int s = blockIdx.x, bz = blockIdx.y, lane = threadIdx.x;
+// POLY: Q[x][c] from the row power moments mu[x][a] and the |beta| row pixels whose shifted partner wraps
+// (tables cq, cwr of plan.cu).  One thread per (x, c).
+__global__ void k_q_poly(const double *__restrict__ R, const double *__restrict__ mu, const double *__restrict__ cq,
+                         const double *__restrict__ cwr, double *__restrict__ Q, int H, int W, int NC, int A, int L) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, bz = blockIdx.y;
+    if (i >= H * NC) return;
+    const int x = i / NC, c = i - x * NC, w = (L - 1) / 2, beta = c % L - w;
+    const double *m = mu + ((size_t)bz * H + x) * A, *q = cq + (size_t)c * A;
+    double v = 0.0;
+    for (int a = 0; a < A; ++a) v = fma(__ldg(&q[a]), m[a], v);
+    const double *row = R + ((size_t)bz * H + x) * W + (beta > 0 ? W - beta : 0);
+    const int nb = beta > 0 ? beta : -beta;
+    for (int k = 0; k < nb; ++k) v = fma(__ldg(&cwr[(size_t)c * w + k]), __ldg(&row[k]), v);
+    Q[(size_t)bz * H * NC + i] = v;
+}
+
+// Delta_s = sum_x f'_i(x) QS[x][j]   (one 256-thread CTA per s)
+__global__ void __launch_bounds__(256) k_delta(const double *__restrict__ QS, const double *__restrict__ xwt,
+                                               const int *__restrict__ bti, const int *__restrict__ btj,
+                                               double *__restrict__ tab, int H, int nKa, int nBa, int FB, size_t off_de,
+                                               size_t tab_size) {
+    const int s = blockIdx.x, bz = blockIdx.y, tid = threadIdx.x, lane = tid & 31;
+    __shared__ double red[8];
     const double *f = xwt + (size_t)(nKa + bti[s]) * H;
     const double *q = QS + (size_t)bz * H * nBa + btj[s];
     double v = 0.0;
-    for (int x = lane; x < H; x += 32) v = fma(f[x], q[(size_t)x * nBa], v);
+    for (int x = tid; x < H; x += 256) v = fma(f[x], q[(size_t)x * nBa], v);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    if (lane == 0) tab[(size_t)bz * tab_size + off_de + s] = v;
+    if (lane == 0) red[tid >> 5] = v;
+    __syncthreads();
+    if (tid == 0) {
+        double t = 0.0;
+        for (int k = 0; k < 8; ++k) t += red[k];
+        tab[(size_t)bz * tab_size + off_de + s] = t;
+    }
 }
 
 }  // namespace
@@ -178,21 +202,32 @@ cudaError_t launch_dgemm(sfft_plan *p, const GemmArgs &g) {
 cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS) {
     const int H = p->H, W = p->W, NC = p->NC;
     const long long P = (long long)H * W;
+    auto rowdot = [&](const double *img, const double *tabl, double *out, int nj) {
+        dim3 grid((H + 7) / 8, p->nbatch);
+        if (nj <= 4) k_rowdot<4><<<grid, 256, 0, p->stream>>>(img, tabl, out, H, W, nj);
+        else if (nj <= 8) k_rowdot<8><<<grid, 256, 0, p->stream>>>(img, tabl, out, H, W, nj);
+        else if (nj <= 12) k_rowdot<12><<<grid, 256, 0, p->stream>>>(img, tabl, out, H, W, nj);
+        else k_rowdot<17><<<grid, 256, 0, p->stream>>>(img, tabl, out, H, W, nj);
+        p->launches++;
+    };
+    cudaError_t e = cudaSuccess;
+    if (p->basis == SFFT_BASIS_POLY) {
+        // Q from nMom row power moments (one streaming pass over R) instead of the NC-column contraction
+        rowdot(dR, p->dt.gM, p->mu, p->nMom);
+        k_q_poly<<<dim3((H * NC + 255) / 256, p->nbatch), 256, 0, p->stream>>>(dR, p->mu, p->dt.cq, p->dt.cwr, p->Q, H, W, NC,
+                                                                           p->nMom, p->L);
+        p->launches++;
+    } else {
     // Q = R * cy^T
     GemmArgs g{};
     g.A = dR; g.B = p->dt.cy; g.C = p->Q; g.M = H; g.N = NC; g.K = W; g.lda = W; g.ldb = W; g.ldc = NC;
     g.sA = P; g.sB = 0; g.sC = (long long)p->ksq * H * NC; g.sCk = (long long)H * NC; g.nz = p->nbatch; g.ksplit = p->ksq;
     g.alpha = 1.0; g.beta = 0.0; g.bT = true; g.lower = false; g.kmodA = 0;
-    cudaError_t e = launch_dgemm(p, g);
+    e = launch_dgemm(p, g);
     if (e != cudaSuccess) return e;
-    // QS = S * gB^T
-    {
-        dim3 grid((H + 7) / 8, p->nbatch);
-        if (p->nBa <= 4) k_rowdot<4><<<grid, 256, 0, p->stream>>>(dS, p->dt.gB, p->QS, H, W, p->nBa);
-        else if (p->nBa <= 8) k_rowdot<8><<<grid, 256, 0, p->stream>>>(dS, p->dt.gB, p->QS, H, W, p->nBa);
-        else k_rowdot<12><<<grid, 256, 0, p->stream>>>(dS, p->dt.gB, p->QS, H, W, p->nBa);
-        p->launches++;
     }
+    // QS = S * gB^T
+    rowdot(dS, p->dt.gB, p->QS, p->nBa);
     // C = fx * (sum of the ksq partial Q's): K = ksq stacked copies of the x axis, split in ksq*ksplit parts
     const int parts = p->ksq * p->ksplit;
     GemmArgs h{};
@@ -205,7 +240,7 @@ cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS) {
     k_lambda_pick<<<dim3((tot + 255) / 256, p->nbatch), 256, 0, p->stream>>>(
         p->LamC, p->tab, p->dt.kti, p->dt.ktj, p->dt.bti, p->dt.btj, p->FK, p->FB, p->L, p->nBa, NC, parts, p->off_la,
         p->tab_size);
-    k_delta<<<dim3(p->FB, p->nbatch), 32, 0, p->stream>>>(p->QS, p->dt.xwt, p->dt.bti, p->dt.btj, p->tab, H, p->nKa, p->nBa,
+    k_delta<<<dim3(p->FB, p->nbatch), 256, 0, p->stream>>>(p->QS, p->dt.xwt, p->dt.bti, p->dt.btj, p->tab, H, p->nKa, p->nBa,
                                                          p->FB, p->off_de, p->tab_size);
     p->launches += 2;
     return cudaGetLastError();

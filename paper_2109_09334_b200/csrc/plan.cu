@@ -100,7 +100,7 @@ void choose_split(sfft_plan *p) {
     // y-range splits of the first moment GEMM (moments.cu): enough CTAs to fill the machine
     const long tiles = (long)((p->H + 63) / 64) * ((p->NC + 63) / 64) * p->nbatch;
     p->ksq = 1;
-    while (p->ksq < 8 && tiles * p->ksq < 4 * 148 && p->W / (2 * p->ksq) >= 256) p->ksq *= 2;
+    while (p->basis != SFFT_BASIS_POLY && p->ksq < 8 && tiles * p->ksq < 4 * 148 && p->W / (2 * p->ksq) >= 256) p->ksq *= 2;
 }
 
 void build_jobs(sfft_plan *p) {
@@ -162,7 +162,7 @@ void build_jobs(sfft_plan *p) {
     p->NC = p->nKa * p->nBa * L;
     choose_split(p);
     p->nch = (p->Nh + 1 + kLagChunk - 1) / kLagChunk;
-    p->ksplit = std::max(1, std::min(16, p->H / 128));
+    p->ksplit = std::max(1, std::min(32, p->H / 64));
 }
 
 int fail_cuda(sfft_plan *p, cudaError_t e) {
@@ -172,7 +172,7 @@ int fail_cuda(sfft_plan *p, cudaError_t e) {
 
 void free_tables(sfft_plan *p) {
     DeviceTables &d = p->dt;
-    cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.lagtw); cudaFree(d.cy); cudaFree(d.fx);
+    cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.lagtw); cudaFree(d.cy); cudaFree(d.fx); cudaFree(d.gM); cudaFree(d.cq); cudaFree(d.cwr);
     cudaFree(d.phi0);
     cudaFree(d.seqs); cudaFree(d.jobs); cudaFree(d.units);
     cudaFree(d.kti); cudaFree(d.ktj); cudaFree(d.bti); cudaFree(d.btj);
@@ -180,7 +180,7 @@ void free_tables(sfft_plan *p) {
 }
 
 struct WsLayout {
-    size_t rhat, G, lagpart, tab, Q, QS, LamC, M, rhs, Lf, Winv, dscale, kfold, ctab, khat, flag, stR, stS, stD, stC, total;
+    size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, kfold, ctab, khat, flag, stR, stS, stD, stC, total;
 };
 
 WsLayout ws_layout(const sfft_plan *p) {
@@ -194,6 +194,7 @@ WsLayout ws_layout(const sfft_plan *p) {
     l.Q = take(nb * p->ksq * (size_t)p->H * p->NC * sizeof(double));
     l.QS = take(nb * (size_t)p->H * p->nBa * sizeof(double));
     l.LamC = take(nb * p->ksq * p->ksplit * (size_t)p->NC * p->NC * sizeof(double));
+    l.mu = take(nb * (size_t)p->H * p->nMom * sizeof(double));
     l.M = take(nb * n * n * sizeof(double));
     l.rhs = take(nb * n * sizeof(double));
     l.Lf = take(nb * (n + 1) * (size_t)p->ldl * sizeof(double));
@@ -237,6 +238,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     p->nimg = p->nKa + 1;
     p->ldl = (p->n + 1 + 7) & ~7;
     p->LT = subtract_kpad(p->nKa, L);
+    p->nMom = basis == SFFT_BASIS_POLY ? DK + DB + 1 : 0;
     build_jobs(p);
 
     // ---- constant tables (host, long double where it matters) ----
@@ -276,6 +278,33 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
                 double *row = &fx[((size_t)(ib * p->nBa + i) * L + a) * H];
                 for (int x = 0; x < H; ++x) row[x] = fK[(size_t)ib * H + x] * fB[(size_t)i * H + ((x + a - wl + H) & (H - 1))];
             }
+    // POLY shortcut of the first moment contraction (moments.cu): u(y+beta) = u(y) + beta*delta away from the wrap, so
+    //   Q[x][(jb,j,beta)] = sum_k C(j,k) (beta delta)^(j-k) mu_{jb+k}(x) + sum_{wrapping y} R(x,y) u^jb [u(y')^j - (u + beta delta)^j]
+    std::vector<double> gM, cq, cwr;
+    if (basis == SFFT_BASIS_POLY) {
+        const int A = p->nMom;
+        gM.resize((size_t)A * W); cq.assign((size_t)p->NC * A, 0.0); cwr.assign((size_t)p->NC * std::max(wl, 1), 0.0);
+        auto uy = [&](int y) { return (2.0L * y + 1.0L) / (long double)W - 1.0L; };
+        for (int y = 0; y < W; ++y) {
+            long double pw = 1.0L;
+            for (int a = 0; a < A; ++a) { gM[(size_t)a * W + y] = (double)pw; pw *= uy(y); }
+        }
+        const long double delta = 2.0L / (long double)W;
+        for (int jb = 0; jb < p->nKa; ++jb)
+            for (int j = 0; j < p->nBa; ++j)
+                for (int b = 0; b < L; ++b) {
+                    const int c = (jb * p->nBa + j) * L + b, beta = b - wl;
+                    long double binom = 1.0L;                       // C(j,k)
+                    for (int k = 0; k <= j; ++k) {
+                        cq[(size_t)c * A + jb + k] = (double)(binom * powl(beta * delta, j - k));
+                        binom = binom * (j - k) / (k + 1);
+                    }
+                    for (int q = 0; q < std::abs(beta); ++q) {
+                        const int y = beta > 0 ? W - beta + q : q, yw = beta > 0 ? y + beta - W : y + beta + W;
+                        cwr[(size_t)c * wl + q] = (double)(powl(uy(y), jb) * (powl(uy(yw), j) - powl(uy(y) + beta * delta, j)));
+                    }
+                }
+    }
     // M_bb = sum_x f_ib f_i * sum_y g_jb g_j  (Eq. 22 / B11 at lag 0; separable, plan constant)
     std::vector<double> phi0((size_t)p->FB * p->FB);
     {
@@ -296,7 +325,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     cudaError_t e = cudaSuccess;
     DeviceTables &d = p->dt;
 #define UP(dst, vec) if (e == cudaSuccess) e = upload(&d.dst, vec.data(), vec.size())
-    UP(xwt, xwt); UP(gK, gK); UP(gB, gB); UP(twW, twW); UP(lagtw, lagtw); UP(cy, cy); UP(fx, fx); UP(phi0, phi0);
+    UP(xwt, xwt); UP(gK, gK); UP(gB, gB); UP(twW, twW); UP(lagtw, lagtw); UP(cy, cy); UP(fx, fx); UP(gM, gM); UP(cq, cq); UP(cwr, cwr); UP(phi0, phi0);
     UP(seqs, p->seqs); UP(jobs, p->jobs); UP(units, p->units);
     UP(kti, p->kti); UP(ktj, p->ktj); UP(bti, p->bti); UP(btj, p->btj);
 #undef UP
@@ -331,7 +360,7 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     char *b = (char *)d_ws;
     p->ws = d_ws; p->ws_bytes = bytes;
     p->rhat = (double2 *)(b + l.rhat); p->G = (double2 *)(b + l.G); p->lagpart = (double *)(b + l.lagpart); p->tab = (double *)(b + l.tab);
-    p->Q = (double *)(b + l.Q); p->QS = (double *)(b + l.QS); p->LamC = (double *)(b + l.LamC);
+    p->Q = (double *)(b + l.Q); p->QS = (double *)(b + l.QS); p->LamC = (double *)(b + l.LamC); p->mu = (double *)(b + l.mu);
     p->M = (double *)(b + l.M); p->rhs = (double *)(b + l.rhs); p->Lf = (double *)(b + l.Lf); p->Winv = (double *)(b + l.Winv);
     p->dscale = (double *)(b + l.dscale); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
     p->stageR = (double *)(b + l.stR); p->stageS = (double *)(b + l.stS); p->stageD = (double *)(b + l.stD);

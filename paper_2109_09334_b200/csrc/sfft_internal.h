@@ -42,6 +42,9 @@ struct DeviceTables {
     double *gB = nullptr;       // [nBa][W]         background y-axis basis
     double2 *twW = nullptr;     // [W]              exp(-2 pi i k / W)
     double2 *lagtw = nullptr;   // [Nh+1][L]        (w_m cos, w_m sin)(2 pi m k / W) / W
+    double *gM = nullptr;       // [nMom][W]        POLY: u_y^a, a < nMom = DK + DB + 1 (row power moments, moments.cu)
+    double *cq = nullptr;       // [NC][nMom]       POLY: Q_c = sum_a cq[c][a] mu_a + border terms (binomial shift of g'_j by beta)
+    double *cwr = nullptr;      // [NC][w]          POLY: coefficients of the |beta| row pixels whose shifted partner wraps
     double *cy = nullptr;       // [NC][W]          g_jb(y) g'_j((y+beta) mod W),  c = (jb*nBa + j)*L + beta+w
     double *fx = nullptr;       // [NC][H]          f_ib(x) f'_i((x+alpha) mod H), c = (ib*nBa + i)*L + alpha+w
     double *phi0 = nullptr;     // [FB][FB]         M_bb (plan constant)
@@ -64,6 +67,7 @@ struct sfft_plan {
     int nch = 0;         // column chunks of the lagsum partials
     int NC = 0;          // nKa*nBa*L columns of the moment GEMMs
     int ksplit = 1;      // K (x-range) splits of the second moment GEMM
+    int nMom = 0;        // POLY: row power moments mu_a(x) = sum_y R(x,y) u_y^a kept per row
     int ksq = 1;         // K (y-range) splits of the first moment GEMM; its partial Q's are summed by the second
     int npairs = 0;      // FK(FK+1)/2
     int ldl = 0;         // leading dimension of the Cholesky factor buffer (>= n+1)
@@ -78,7 +82,7 @@ struct sfft_plan {
     // workspace partition (device pointers into the caller's buffer)
     void *ws = nullptr; size_t ws_bytes = 0;
     double2 *rhat = nullptr; double2 *G = nullptr; double *lagpart = nullptr; double *tab = nullptr;
-    double *Q = nullptr, *QS = nullptr, *LamC = nullptr;
+    double *Q = nullptr, *QS = nullptr, *LamC = nullptr, *mu = nullptr;
     double *M = nullptr, *rhs = nullptr, *Lf = nullptr, *Winv = nullptr, *dscale = nullptr, *kfold = nullptr, *ctab = nullptr;
     double2 *khat = nullptr;                    // [b][L*FK][Nh] row spectra of the pixel kernels (Fourier-route subtract)
     const double *rhat_src = nullptr;           // device buffer whose weighted row spectra rhat[0..nKa) currently holds
