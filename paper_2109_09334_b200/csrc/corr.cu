@@ -18,11 +18,14 @@
 // i.e. two mma.sync.m8n8k4.f64 (DMMA) per 4 x-values give 4 x 8 complex lag sums with no wasted
 // multiply:  Re G = Cr[p] + Ci[p+4],  Im G = Ci[p] - Cr[p+4]   (Cr = A Br, Ci = A Bi).
 // The Hankel operand needs no data movement: lane (k, n) of the B fragment reads z_q(x0 + k + n + rho0)
-// straight from the x-contiguous shared-memory plane.  Lag 0 uses one extra block whose columns are the
-// eight N-side sequences at rho = 0.  The packed DC/Nyquist slot (column 0 holds (X[0], X[W/2]), both
+// straight from the x-contiguous shared-memory plane.  When L-1 is a multiple of 8 lag 0 uses one extra
+// block whose columns are eight N-side sequences at rho = 0 (blocks then start at lag 1); otherwise the
+// blocks start at lag 0.  Each job carries its own block list (only the lags the normal system reads:
+// L-1 between kernel terms, w against S, none for S with S) and its own x-ranges (compactly supported
+// B-spline x-factors: outside the overlap of the two supports every product vanishes identically).  The packed DC/Nyquist slot (column 0 holds (X[0], X[W/2]), both
 // real) falls out of the same arithmetic: Cr[p] is the DC sum and Ci[p+4] the Nyquist sum.
 //
-// CTA = 8 warps = 2 columns x 2 row blocks x 2 halves of the N side; two CTAs per SM overlap one
+// CTA = 8 warps = 2 columns x 2 row blocks x 2 halves of the block list; two CTAs per SM overlap one
 // CTA's staging with the other's MMAs.  FP64-MMA bound.
 #include "sfft_internal.h"
 
@@ -35,14 +38,32 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
         : "d"(a), "d"(b));
 }
 
+__device__ __forceinline__ double lds_f64(unsigned addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+
+// MMAs of one staged tile for a warp with exactly NB blocks (compile-time trip counts, no predication:
+// mma.sync under a predicate costs a warp re-convergence per instruction).
+template <int NB, int XS>
+__device__ __forceinline__ void corr_tile_mma(double (&acc)[kCorrBlk][2][2], unsigned aA, const unsigned (&aB)[kCorrBlk],
+                                              int kmax) {
+#pragma unroll 2
+    for (int kk = 0; kk < kmax; kk += 4) {
+        const double a = lds_f64(aA + kk * 8);
+#pragma unroll
+        for (int i = 0; i < NB; ++i)
+#pragma unroll
+            for (int pt = 0; pt < 2; ++pt) dmma884(acc[i][pt], a, lds_f64(aB[i] + (pt * 2 * XS + kk) * 8));
+    }
+}
+
 template <int XT, int NLB>
 struct CorrCfg {
-    static constexpr int NTH = NLB <= 2 ? 4 : 2;           // N-side sequences per warp half
-    static constexpr int KNT = 2 * NTH - 1;                // N-side sequences per job
-    static constexpr int ROWS = XT + 8 * NLB;              // staged x-rows per tile
+    static constexpr int ROWS = XT + 8 * NLB;              // staged x-rows per tile (largest lag offset + fragment extent)
     static constexpr int XS = ((ROWS + 7) / 16) * 16 + 8;  // plane stride, = 8 mod 16 (conflict-free staging stores)
     static constexpr int SS = 4 * XS + 4;                  // slot stride [part 2][col 2][XS] + 4 (conflict-free A loads)
-    static constexpr int LBA = NLB > 0 ? NLB : 1;
     static constexpr size_t SMEM = (size_t)kCorrSlots * SS * sizeof(double);
 };
 
@@ -53,7 +74,7 @@ k_corr_mma(const double2 *__restrict__ rhat, const double *__restrict__ xwt, con
            const CorrJob *__restrict__ jobs, double2 *__restrict__ G, int H, int Nh, int nimg, int nseq, int L, int E,
            int Sx) {
     using C = CorrCfg<XT, NLB>;
-    constexpr int NTH = C::NTH, KNT = C::KNT, ROWS = C::ROWS, XS = C::XS, SS = C::SS, LBA = C::LBA;
+    constexpr int ROWS = C::ROWS, XS = C::XS, SS = C::SS;
     extern __shared__ double sm[];
     __shared__ CorrJob job;
     __shared__ Seq sseq[kCorrSlots];
@@ -69,50 +90,56 @@ k_corr_mma(const double2 *__restrict__ rhat, const double *__restrict__ xwt, con
 
     const double2 *rhat_b = rhat + (size_t)bz * nimg * H * Nh;
     const int row = lane >> 2, kq = lane & 3;
-    // per-lane fragment bases (doubles)
-    const double *sA = sm + job.mslot[mb][row & 3] * SS + ((row >> 2) * 2 + col) * XS + kq;
-    const double *sB = sm + (nh * NTH) * SS + col * XS + 1 + kq + row;
-    const double *s0 = sm + (row < KNT ? row : kCorrNSeq) * SS + col * XS + kq;
+    // per-lane fragment bases (doubles): A = rows (Re, Im) of four M-side sequences; B = per block, a Hankel read
+    // of one plane at its first lag, or (lag-0 block) one plane per column
+    const unsigned sm0 = (unsigned)__cvta_generic_to_shared(sm);
+    const unsigned aA = sm0 + 8u * (job.mslot[mb][row & 3] * SS + ((row >> 2) * 2 + col) * XS + kq);
+    const int nb = job.nblk[nh];
+    unsigned aB[kCorrBlk];
+#pragma unroll
+    for (int i = 0; i < kCorrBlk; ++i) {
+        const int sl = job.blk_slot[nh][i];
+        aB[i] = sm0 + 8u * ((sl >= 0 ? sl * SS + job.blk_lag[nh][i] + row : job.zslot[row] * SS) + col * XS + kq);
+    }
 
-    double acc[NTH][LBA][2][2];
+    double acc[kCorrBlk][2][2];
 #pragma unroll
-    for (int q = 0; q < NTH; ++q)
+    for (int i = 0; i < kCorrBlk; ++i)
 #pragma unroll
-        for (int lb = 0; lb < LBA; ++lb)
-#pragma unroll
-            for (int pt = 0; pt < 2; ++pt) acc[q][lb][pt][0] = acc[q][lb][pt][1] = 0.0;
+        for (int pt = 0; pt < 2; ++pt) acc[i][pt][0] = acc[i][pt][1] = 0.0;
 
-    const int xlen = H / Sx, xbeg = xs * xlen;
     const int nitems = job.nstage * ROWS * kCorrCols;
-    for (int x0 = xbeg; x0 < xbeg + xlen; x0 += XT) {
-        __syncthreads();
-        // ---- stage the tile: weighted sequences, split into Re / Im planes, x-contiguous ----
-        for (int i = tid; i < nitems; i += 256) {
-            const int c = i & 1, r = (i >> 1) % ROWS, si = (i >> 1) / ROWS;
-            const int x = (x0 + r) & (H - 1);
-            const Seq sq = sseq[si];
-            double2 v = __ldg(&rhat_b[((size_t)sq.img * H + x) * Nh + m0 + c]);
-            if (sq.xw >= 0) { const double wgt = __ldg(&xwt[(size_t)sq.xw * H + x]); v.x *= wgt; v.y *= wgt; }
-            double *pl = sm + job.stage_slot[si] * SS + c * XS + r;
-            pl[0] = v.x;
-            pl[2 * XS] = v.y;
-        }
-        __syncthreads();
-        // ---- MMAs ----
-#pragma unroll 2
-        for (int kk = 0; kk < XT; kk += 4) {
-            const double a = sA[kk];
-#pragma unroll
-            for (int q = 0; q < NTH; ++q) {
-                if (q == NTH - 1 && nh == 1) {      // warp-uniform: the lag-0 block takes this slot
-#pragma unroll
-                    for (int pt = 0; pt < 2; ++pt) dmma884(acc[q][0][pt], a, s0[pt * 2 * XS + kk]);
-                } else {
-#pragma unroll
-                    for (int lb = 0; lb < NLB; ++lb)
-#pragma unroll
-                        for (int pt = 0; pt < 2; ++pt) dmma884(acc[q][lb][pt], a, sB[q * SS + pt * 2 * XS + lb * 8 + kk]);
-                }
+    for (int rg = 0; rg < job.nrange; ++rg) {
+        // this CTA's part of the range: Sx parts of whole 4-row steps
+        const int rb = job.xbeg[rg], re = job.xend[rg];
+        const int plen = (((re - rb) / 4 + Sx - 1) / Sx) * 4;
+        const int xbeg = rb + xs * plen, xend = min(re, xbeg + plen);
+        for (int x0 = xbeg; x0 < xend; x0 += XT) {
+            __syncthreads();
+            // ---- stage the tile: weighted sequences, split into Re / Im planes, x-contiguous ----
+            for (int i = tid; i < nitems; i += 256) {
+                const int c = i & 1, r = (i >> 1) % ROWS, si = (i >> 1) / ROWS;
+                const int x = (x0 + r) & (H - 1);
+                const Seq sq = sseq[si];
+                double2 v = __ldg(&rhat_b[((size_t)sq.img * H + x) * Nh + m0 + c]);
+                if (sq.xw >= 0) { const double wgt = __ldg(&xwt[(size_t)sq.xw * H + x]); v.x *= wgt; v.y *= wgt; }
+                double *pl = sm + job.stage_slot[si] * SS + c * XS + r;
+                pl[0] = v.x;
+                pl[2 * XS] = v.y;
+            }
+            __syncthreads();
+            // ---- MMAs ----
+            const int kmax = min(XT, xend - x0);
+            switch (nb) {               // warp-uniform
+                case 1: corr_tile_mma<1, XS>(acc, aA, aB, kmax); break;
+                case 2: corr_tile_mma<2, XS>(acc, aA, aB, kmax); break;
+                case 3: corr_tile_mma<3, XS>(acc, aA, aB, kmax); break;
+                case 4: corr_tile_mma<4, XS>(acc, aA, aB, kmax); break;
+                case 5: corr_tile_mma<5, XS>(acc, aA, aB, kmax); break;
+                case 6: corr_tile_mma<6, XS>(acc, aA, aB, kmax); break;
+                case 7: corr_tile_mma<7, XS>(acc, aA, aB, kmax); break;
+                case 8: corr_tile_mma<8, XS>(acc, aA, aB, kmax); break;
+                default: break;
             }
         }
     }
@@ -123,30 +150,28 @@ k_corr_mma(const double2 *__restrict__ rhat, const double *__restrict__ xwt, con
     double2 *Gn = G + (((size_t)bz * Sx + xs) * (Nh + 1) + Nh) * E;     // Nyquist row (used by column 0 only)
     const int p = job.mseq[mb][row & 3];
 #pragma unroll
-    for (int q = 0; q < NTH; ++q)
+    for (int i = 0; i < kCorrBlk; ++i) {
+        if (i >= nb) continue;
+        const int sl = job.blk_slot[nh][i];
 #pragma unroll
-        for (int lb = 0; lb < LBA; ++lb) {
-            const bool zero_blk = (q == NTH - 1 && nh == 1);
-            if (zero_blk ? (lb > 0) : (lb >= NLB)) continue;
-#pragma unroll
-            for (int i = 0; i < 2; ++i) {
-                const double cr = acc[q][lb][0][i], ci = acc[q][lb][1][i];
-                const double ocr = __shfl_xor_sync(0xffffffffu, cr, 16), oci = __shfl_xor_sync(0xffffffffu, ci, 16);
-                if (row >= 4) continue;
-                const int nn = 2 * kq + i;
-                int rho, qs;
-                if (zero_blk) { rho = 0; qs = nn < KNT ? job.nseq[nn] : -1; }
-                else { rho = 1 + 8 * lb + nn; qs = job.nseq[nh * NTH + q]; }
-                if (p < 0 || qs < 0 || rho >= L) continue;
-                const int e = (p * nseq + qs) * L + rho;
-                if (mcol == 0) {
-                    Gm[e] = make_double2(cr, 0.0);
-                    Gn[e] = make_double2(oci, 0.0);
-                } else {
-                    Gm[e] = make_double2(cr + oci, ci - ocr);
-                }
+        for (int q = 0; q < 2; ++q) {
+            const double cr = acc[i][0][q], ci = acc[i][1][q];
+            const double ocr = __shfl_xor_sync(0xffffffffu, cr, 16), oci = __shfl_xor_sync(0xffffffffu, ci, 16);
+            if (row >= 4) continue;
+            const int nn = 2 * kq + q;
+            int rho, qs;
+            if (sl < 0) { rho = 0; qs = job.zseq[nn]; }
+            else { rho = job.blk_lag[nh][i] + nn; qs = nn < job.blk_nlag[nh][i] ? job.blk_seq[nh][i] : -1; }
+            if (p < 0 || qs < 0 || rho >= L) continue;
+            const int e = (p * nseq + qs) * L + rho;
+            if (mcol == 0) {
+                Gm[e] = make_double2(cr, 0.0);
+                Gn[e] = make_double2(oci, 0.0);
+            } else {
+                Gm[e] = make_double2(cr + oci, ci - ocr);
             }
         }
+    }
 }
 
 template <int XT, int NLB>

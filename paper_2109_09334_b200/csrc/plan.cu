@@ -103,8 +103,15 @@ void choose_split(sfft_plan *p) {
     while (p->basis != SFFT_BASIS_POLY && p->ksq < 8 && tiles * p->ksq < 4 * 148 && p->W / (2 * p->ksq) >= 256) p->ksq *= 2;
 }
 
-void build_jobs(sfft_plan *p) {
-    const int FK = p->FK, FB = p->FB, L = p->L, w = p->w, nO = 2 * L - 1;
+// Lags of G_{p,q} the normal system reads: L-1 between kernel terms (Omega, B5/B6), w against S (Theta, B13/B14),
+// none for S with S.
+int need_lag(const sfft_plan *p, int sp, int sq) {
+    const bool ps = sp == p->FK, qs = sq == p->FK;
+    return (ps && qs) ? -1 : ((ps || qs) ? p->w : p->L - 1);
+}
+
+void build_jobs(sfft_plan *p, const std::vector<double> &fK) {
+    const int FK = p->FK, FB = p->FB, L = p->L, w = p->w, nO = 2 * L - 1, H = p->H;
     p->seqs.clear(); p->jobs.clear(); p->units.clear();
     // column sequences: kernel terms z_t = f_i(x) r_j(x,m), then S
     for (int t = 0; t < FK; ++t) p->seqs.push_back({p->ktj[t], p->kti[t]});
@@ -112,34 +119,79 @@ void build_jobs(sfft_plan *p) {
     p->seqs.push_back({p->nKa, -1});
     p->nseq = FK + 1;
     p->E = p->nseq * p->nseq * L;
-    p->nlb = (L - 1 + 7) / 8;
+    // lag blocks: a shared lag-0 block plus blocks from lag 1 when L-1 is a multiple of 8, else blocks from lag 0
+    const bool lag0blk = ((L - 1) % 8 == 0);
+    p->nlb = lag0blk ? (L - 1) / 8 : (L + 7) / 8;
     p->npairs = FK * (FK + 1) / 2;
     p->off_om = 0;
     p->off_th = p->off_om + (size_t)p->npairs * nO * nO;
     p->off_la = p->off_th + (size_t)FK * L * L;
     p->off_de = p->off_la + (size_t)FK * FB * L * L;
     p->tab_size = p->off_de + FB;
-    // correlation jobs: (group of 8 M-side sequences) x (tile of knt N-side sequences)
-    const int knt = p->nlb <= 2 ? 7 : 3;
+    // x-support [lo, hi) of every sequence (B-spline x-factors are compactly supported; everything else is dense)
+    std::vector<int> slo(p->nseq, 0), shi(p->nseq, H);
+    if (p->basis == SFFT_BASIS_BSPLINE)
+        for (int t = 0; t < FK; ++t) {
+            const double *f = &fK[(size_t)p->kti[t] * H];
+            int lo = 0, hi = H;
+            while (lo < H && f[lo] == 0.0) ++lo;
+            while (hi > lo && f[hi - 1] == 0.0) --hi;
+            slo[t] = lo; shi[t] = hi;
+        }
+    // correlation jobs: (group of 8 M-side sequences) x (tile of knt N-side sequences, at most 16 blocks)
+    const int knt = p->nlb == 0 ? 8 : std::min(8, (2 * kCorrBlk - (lag0blk ? 1 : 0)) / p->nlb);
     for (int m0 = 0; m0 < p->nseq; m0 += 8)
         for (int n0 = 0; n0 < p->nseq; n0 += knt) {
             CorrJob j{};
-            j.nstage = 0;
-            for (int q = 0; q < 8; ++q) {
-                j.nseq[q] = (q < knt && n0 + q < p->nseq) ? n0 + q : -1;
-                if (j.nseq[q] >= 0) { j.stage_slot[j.nstage] = q; j.stage_seq[j.nstage] = j.nseq[q]; ++j.nstage; }
+            const int mcnt = std::min(8, p->nseq - m0), ncnt = std::min(knt, p->nseq - n0);
+            for (int q = 0; q < 8; ++q) { j.zslot[q] = kCorrZero; j.zseq[q] = -1; }
+            // N side: planes 0..ncnt-1, blocks dealt to the two warp halves in turn
+            struct Blk { int slot, seq, lag, nlag; };
+            std::vector<Blk> blks;
+            bool any0 = false;
+            int Alo = H, Ahi = 0, Nlo = H, Nhi = 0, maxlag = 0;
+            for (int q = 0; q < ncnt; ++q) {
+                const int sq = n0 + q;
+                int ml = -1;
+                for (int r = 0; r < mcnt; ++r) ml = std::max(ml, need_lag(p, m0 + r, sq));
+                if (ml < 0) continue;
+                j.stage_slot[j.nstage] = q; j.stage_seq[j.nstage] = sq; ++j.nstage;
+                Nlo = std::min(Nlo, slo[sq]); Nhi = std::max(Nhi, shi[sq]); maxlag = std::max(maxlag, ml);
+                if (lag0blk) { j.zslot[q] = q; j.zseq[q] = sq; any0 = true; }
+                for (int l0 = lag0blk ? 1 : 0; l0 <= ml; l0 += 8) blks.push_back({q, sq, l0, std::min(8, ml - l0 + 1)});
             }
-            int extra = kCorrNSeq + 1;
+            if (any0) blks.push_back({-1, -1, 0, 8});
+            if (blks.empty()) continue;
+            for (size_t i = 0; i < blks.size(); ++i) {
+                const int h = (int)(i & 1), k = j.nblk[h]++;
+                j.blk_slot[h][k] = blks[i].slot; j.blk_seq[h][k] = blks[i].seq;
+                j.blk_lag[h][k] = blks[i].lag; j.blk_nlag[h][k] = blks[i].nlag;
+            }
+            for (int h = 0; h < 2; ++h)
+                for (int k = j.nblk[h]; k < kCorrBlk; ++k) { j.blk_slot[h][k] = kCorrZero; j.blk_seq[h][k] = -1; j.blk_lag[h][k] = 0; j.blk_nlag[h][k] = 0; }
+            // M side: share the plane of an N-side sequence, else an extra plane
+            int extra = kCorrZero + 1;
             for (int h = 0; h < 2; ++h)
                 for (int r = 0; r < 4; ++r) {
-                    int sq = m0 + 4 * h + r;
-                    if (sq >= p->nseq) { j.mseq[h][r] = -1; j.mslot[h][r] = kCorrNSeq; continue; }
+                    const int sq = m0 + 4 * h + r;
+                    if (sq >= p->nseq) { j.mseq[h][r] = -1; j.mslot[h][r] = kCorrZero; continue; }
                     j.mseq[h][r] = sq;
+                    Alo = std::min(Alo, slo[sq]); Ahi = std::max(Ahi, shi[sq]);
                     int slot = -1;
-                    for (int q = 0; q < 8; ++q) if (j.nseq[q] == sq) slot = q;
+                    for (int k = 0; k < j.nstage; ++k) if (j.stage_seq[k] == sq) slot = j.stage_slot[k];
                     if (slot < 0) { slot = extra++; j.stage_slot[j.nstage] = slot; j.stage_seq[j.nstage] = sq; ++j.nstage; }
                     j.mslot[h][r] = slot;
                 }
+            // x-ranges where z_p(x) z_q(x + rho) can be non-zero: x in A with x + rho in N, directly or wrapped
+            auto round4 = [&](int &lo, int &hi) { lo = std::max(0, lo & ~3); hi = std::min(H, (hi + 3) & ~3); };
+            int lo1 = std::max(Alo, Nlo - maxlag), hi1 = std::min(Ahi, Nhi);
+            int lo2 = std::max(Alo, H + Nlo - maxlag), hi2 = std::min(Ahi, H);      // x + rho - H in [Nlo, Nhi)
+            round4(lo1, hi1); round4(lo2, hi2);
+            const bool e1 = hi1 <= lo1, e2 = hi2 <= lo2;
+            if (e1 && e2) { j.nrange = 1; j.xbeg[0] = 0; j.xend[0] = 4; }              // nothing overlaps: one all-zero step
+            else if (e2 || (!e1 && lo2 <= hi1)) { j.nrange = 1; j.xbeg[0] = lo1; j.xend[0] = e2 ? hi1 : std::max(hi1, hi2); }
+            else if (e1) { j.nrange = 1; j.xbeg[0] = lo2; j.xend[0] = hi2; }
+            else { j.nrange = 2; j.xbeg[0] = lo1; j.xend[0] = hi1; j.xbeg[1] = lo2; j.xend[1] = hi2; }
             p->jobs.push_back(j);
         }
     // lag-table rows.  Negative x-lags use G_{p,q}(-rho) = conj G_{q,p}(rho): entry (q,p,|rho|) with eps negated.
@@ -239,11 +291,11 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     p->ldl = (p->n + 1 + 7) & ~7;
     p->LT = subtract_kpad(p->nKa, L);
     p->nMom = basis == SFFT_BASIS_POLY ? DK + DB + 1 : 0;
-    build_jobs(p);
 
     // ---- constant tables (host, long double where it matters) ----
     std::vector<double> fK = axis_table(basis, H, DK), gK = axis_table(basis, W, DK);
     std::vector<double> fB = axis_table(basis, H, DB), gB = axis_table(basis, W, DB);
+    build_jobs(p, fK);
     std::vector<double> xwt((size_t)(p->nKa + p->nBa) * H);
     std::copy(fK.begin(), fK.end(), xwt.begin());
     std::copy(fB.begin(), fB.end(), xwt.begin() + (size_t)p->nKa * H);

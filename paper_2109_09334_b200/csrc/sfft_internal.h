@@ -12,8 +12,10 @@ namespace sfft {
 
 constexpr int kProfMarks = 11;     // event marks per profiled step (see sfft_plan_profile_read)
 constexpr int kCorrCols = 2;       // spectrum columns (m) per CTA of the correlation kernel
-constexpr int kCorrNSeq = 7;       // N-side (shifted) sequences per correlation job (max)
-constexpr int kCorrSlots = 16;     // shared-memory sequence planes per CTA: 0..6 N side, 7 zero, 8..15 extra M side
+constexpr int kCorrNSlots = 8;     // N-side (shifted) sequence planes per correlation job: slots 0..7
+constexpr int kCorrZero = 8;       // slot of the all-zero plane (absent M-side rows, absent lag-0 columns)
+constexpr int kCorrSlots = 17;     // shared-memory sequence planes per CTA: 0..7 N side, 8 zero, 9..16 extra M side
+constexpr int kCorrBlk = 8;        // N-side 8-lag blocks per warp half (16 per job)
 constexpr int kLagChunk = 32;      // spectrum columns per partial sum of the y-direction inverse DFT
 
 // One column-sequence of the x-direction correlation:  z_s(x, m) = xw[x] * rhat[img][x][m]
@@ -21,15 +23,23 @@ constexpr int kLagChunk = 32;      // spectrum columns per partial sum of the y-
 //   xw  : row of the x-weight table (kernel x-basis function f_i), < 0 = no weight
 struct Seq { int img; int xw; };
 
-// One job of k_corr_mma: all ordered pairs (p in mseq) x (q in nseq) at lags 0..L-1,
-//   G_{p,q}(rho; m) = sum_x conj(z_p(x,m)) z_q((x+rho) mod H, m).
+// One job of k_corr_mma: ordered pairs (p in mseq) x (q on the N side) at the lags its blocks list,
+//   G_{p,q}(rho; m) = sum_x conj(z_p(x,m)) z_q((x+rho) mod H, m),   x over the job's x-ranges.
+// An N-side block is either eight consecutive lags of ONE sequence (Hankel operand read in place) or the
+// lag-0 block, whose eight columns are eight different sequences at rho = 0.
 struct CorrJob {
-    int nseq[8];        // N-side sequence ids (slot q = nseq[q]); -1 = none (zero plane)
-    int mseq[2][4];     // M-side sequence ids of the two 4-row blocks; -1 = none
-    int mslot[2][4];    // shared-memory slot of each M-side sequence (kCorrNSeq = the zero plane)
-    int nstage;         // number of staged slots
-    int stage_slot[kCorrSlots];   // slot index of each staged sequence
-    int stage_seq[kCorrSlots];    // its sequence id
+    int mseq[2][4];         // M-side sequence ids of the two 4-row blocks; -1 = none
+    int mslot[2][4];        // their plane slots (kCorrZero if none)
+    int nstage;             // number of staged planes
+    int stage_slot[kCorrSlots], stage_seq[kCorrSlots];
+    int nblk[2];            // blocks of each warp half
+    int blk_slot[2][kCorrBlk];   // plane slot of the block's sequence; -1 = the lag-0 block
+    int blk_seq[2][kCorrBlk];    // its sequence id
+    int blk_lag[2][kCorrBlk];    // first lag of the block
+    int blk_nlag[2][kCorrBlk];   // valid lags (1..8)
+    int zslot[8], zseq[8];  // lag-0 block: plane slot (kCorrZero if none) and sequence id (-1) of each column
+    int nrange;             // x-ranges (1 or 2; bounds are multiples of 4); outside them every product vanishes
+    int xbeg[2], xend[2];
 };
 
 // One row of a lag table produced by the y-direction pruned inverse DFT:
