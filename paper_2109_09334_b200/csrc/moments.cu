@@ -10,6 +10,8 @@
 // Phi(0,0) = M_bb does not depend on the images and is a plan constant (plan.cu).
 //
 // k_dgemm : generic C = alpha A B(^T) + beta C, 64x64 CTA tile, mma.sync.m8n8k4.f64; also used by solve.cu.
+#include <algorithm>
+
 #include "sfft_internal.h"
 
 namespace sfft {
@@ -151,6 +153,45 @@ __global__ void __launch_bounds__(256) k_rowdot(const double *__restrict__ S, co
     }
 }
 
+// POLY: row power moments  out[x][a] = sum_y img(x,y) u_y^a,  u_y = (2y+1)/W - 1  (exact in double), a < na.
+// One warp per image row, four independent 16-byte loads in flight per lane; grid.y selects the image
+// (0: R -> mu with naR moments, 1: S -> QS with naS, since g'_j = u^j for the polynomial background).
+template <int NA>
+__global__ void __launch_bounds__(256) k_rowmom(const double *__restrict__ R, const double *__restrict__ S,
+                                                double *__restrict__ mu, double *__restrict__ QS, int H, int W, int naR,
+                                                int naS) {
+    const int lane = threadIdx.x & 31, x = blockIdx.x * 8 + (threadIdx.x >> 5), bz = blockIdx.z;
+    if (x >= H) return;
+    const bool isS = blockIdx.y == 1;
+    const int na = isS ? naS : naR;
+    const double2 *src = reinterpret_cast<const double2 *>((isS ? S : R) + ((size_t)bz * H + x) * W);
+    const double invW = 1.0 / W;
+    double acc[NA];
+#pragma unroll
+    for (int a = 0; a < NA; ++a) acc[a] = 0.0;
+    for (int y2 = lane; y2 < W / 2; y2 += 128) {
+        double2 v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) v[q] = (y2 + 32 * q < W / 2) ? __ldg(&src[y2 + 32 * q]) : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const double u0 = (double)(4 * (y2 + 32 * q) + 1) * invW - 1.0, u1 = u0 + 2.0 * invW;
+            double p0 = v[q].x, p1 = v[q].y;
+#pragma unroll
+            for (int a = 0; a < NA; ++a)
+                if (a < na) { acc[a] += p0 + p1; p0 *= u0; p1 *= u1; }
+        }
+    }
+    double *dst = isS ? QS + ((size_t)bz * H + x) * naS : mu + ((size_t)bz * H + x) * naR;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        double t = acc[a];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (lane == 0 && a < na) dst[a] = t;
+    }
+}
+
 // POLY: Q[x][c] from the row power moments mu[x][a] and the |beta| row pixels whose shifted partner wraps
 // (tables cq, cwr of plan.cu).  One thread per (x, c).
 __global__ void k_q_poly(const double *__restrict__ R, const double *__restrict__ mu, const double *__restrict__ cq,
@@ -213,7 +254,13 @@ cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS) {
     cudaError_t e = cudaSuccess;
     if (p->basis == SFFT_BASIS_POLY) {
         // Q from nMom row power moments (one streaming pass over R) instead of the NC-column contraction
-        rowdot(dR, p->dt.gM, p->mu, p->nMom);
+        const int na = std::max(p->nMom, p->nBa);
+        dim3 grid((H + 7) / 8, 2, p->nbatch);
+        if (na <= 3) k_rowmom<3><<<grid, 256, 0, p->stream>>>(dR, dS, p->mu, p->QS, H, W, p->nMom, p->nBa);
+        else if (na <= 5) k_rowmom<5><<<grid, 256, 0, p->stream>>>(dR, dS, p->mu, p->QS, H, W, p->nMom, p->nBa);
+        else if (na <= 9) k_rowmom<9><<<grid, 256, 0, p->stream>>>(dR, dS, p->mu, p->QS, H, W, p->nMom, p->nBa);
+        else k_rowmom<17><<<grid, 256, 0, p->stream>>>(dR, dS, p->mu, p->QS, H, W, p->nMom, p->nBa);
+        p->launches++;
         k_q_poly<<<dim3((H * NC + 255) / 256, p->nbatch), 256, 0, p->stream>>>(dR, p->mu, p->dt.cq, p->dt.cwr, p->Q, H, W, NC,
                                                                            p->nMom, p->L);
         p->launches++;
@@ -226,8 +273,8 @@ cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS) {
     e = launch_dgemm(p, g);
     if (e != cudaSuccess) return e;
     }
-    // QS = S * gB^T
-    rowdot(dS, p->dt.gB, p->QS, p->nBa);
+    // QS = S * gB^T  (POLY: done by k_rowmom above)
+    if (p->basis != SFFT_BASIS_POLY) rowdot(dS, p->dt.gB, p->QS, p->nBa);
     // C = fx * (sum of the ksq partial Q's): K = ksq stacked copies of the x axis, split in ksq*ksplit parts
     const int parts = p->ksq * p->ksplit;
     GemmArgs h{};

@@ -224,7 +224,7 @@ int fail_cuda(sfft_plan *p, cudaError_t e) {
 
 void free_tables(sfft_plan *p) {
     DeviceTables &d = p->dt;
-    cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.lagtw); cudaFree(d.cy); cudaFree(d.fx); cudaFree(d.gM); cudaFree(d.cq); cudaFree(d.cwr);
+    cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.lagtw); cudaFree(d.cy); cudaFree(d.fx); cudaFree(d.cq); cudaFree(d.cwr);
     cudaFree(d.phi0);
     cudaFree(d.seqs); cudaFree(d.jobs); cudaFree(d.units);
     cudaFree(d.kti); cudaFree(d.ktj); cudaFree(d.bti); cudaFree(d.btj);
@@ -332,15 +332,11 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
             }
     // POLY shortcut of the first moment contraction (moments.cu): u(y+beta) = u(y) + beta*delta away from the wrap, so
     //   Q[x][(jb,j,beta)] = sum_k C(j,k) (beta delta)^(j-k) mu_{jb+k}(x) + sum_{wrapping y} R(x,y) u^jb [u(y')^j - (u + beta delta)^j]
-    std::vector<double> gM, cq, cwr;
+    std::vector<double> cq, cwr;
     if (basis == SFFT_BASIS_POLY) {
         const int A = p->nMom;
-        gM.resize((size_t)A * W); cq.assign((size_t)p->NC * A, 0.0); cwr.assign((size_t)p->NC * std::max(wl, 1), 0.0);
+        cq.assign((size_t)p->NC * A, 0.0); cwr.assign((size_t)p->NC * std::max(wl, 1), 0.0);
         auto uy = [&](int y) { return (2.0L * y + 1.0L) / (long double)W - 1.0L; };
-        for (int y = 0; y < W; ++y) {
-            long double pw = 1.0L;
-            for (int a = 0; a < A; ++a) { gM[(size_t)a * W + y] = (double)pw; pw *= uy(y); }
-        }
         const long double delta = 2.0L / (long double)W;
         for (int jb = 0; jb < p->nKa; ++jb)
             for (int j = 0; j < p->nBa; ++j)
@@ -377,7 +373,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     cudaError_t e = cudaSuccess;
     DeviceTables &d = p->dt;
 #define UP(dst, vec) if (e == cudaSuccess) e = upload(&d.dst, vec.data(), vec.size())
-    UP(xwt, xwt); UP(gK, gK); UP(gB, gB); UP(twW, twW); UP(lagtw, lagtw); UP(cy, cy); UP(fx, fx); UP(gM, gM); UP(cq, cq); UP(cwr, cwr); UP(phi0, phi0);
+    UP(xwt, xwt); UP(gK, gK); UP(gB, gB); UP(twW, twW); UP(lagtw, lagtw); UP(cy, cy); UP(fx, fx); UP(cq, cq); UP(cwr, cwr); UP(phi0, phi0);
     UP(seqs, p->seqs); UP(jobs, p->jobs); UP(units, p->units);
     UP(kti, p->kti); UP(ktj, p->ktj); UP(bti, p->bti); UP(btj, p->btj);
 #undef UP

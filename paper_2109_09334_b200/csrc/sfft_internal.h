@@ -52,7 +52,6 @@ struct DeviceTables {
     double *gB = nullptr;       // [nBa][W]         background y-axis basis
     double2 *twW = nullptr;     // [W]              exp(-2 pi i k / W)
     double2 *lagtw = nullptr;   // [Nh+1][L]        (w_m cos, w_m sin)(2 pi m k / W) / W
-    double *gM = nullptr;       // [nMom][W]        POLY: u_y^a, a < nMom = DK + DB + 1 (row power moments, moments.cu)
     double *cq = nullptr;       // [NC][nMom]       POLY: Q_c = sum_a cq[c][a] mu_a + border terms (binomial shift of g'_j by beta)
     double *cwr = nullptr;      // [NC][w]          POLY: coefficients of the |beta| row pixels whose shifted partner wraps
     double *cy = nullptr;       // [NC][W]          g_jb(y) g'_j((y+beta) mod W),  c = (jb*nBa + j)*L + beta+w

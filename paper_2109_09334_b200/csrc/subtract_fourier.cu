@@ -13,8 +13,8 @@
 //
 //   k_kernel_spectrum : khat[b][(a,t)][m] from the folded pixel kernels (17-term DFTs)
 //   k_fir_x           : the FIR filter; one thread per column m walks down x with the L+3 partial
-//                       outputs of a 4-row step in registers (FP64 FMA pipe bound)
-//   k_fir_col0        : the packed DC/Nyquist column (two real filters)
+//                       outputs of a 4-row step in registers (FP64 FMA pipe bound); the packed
+//                       DC/Nyquist column runs the same code as two real filters
 //   k_rowfft_inverse_sub : complex-to-real inverse row FFT (conjugate trick on the forward
 //                       radix-16 passes of fft_regs.cuh) fused with the difference (HBM bound)
 #include "fft_regs.cuh"
@@ -61,11 +61,13 @@ __global__ void k_kernel_spectrum(const double *__restrict__ kfold, const double
     khat[((size_t)b * L * FK + blockIdx.y) * Nh + m] = make_double2(re, im);
 }
 
-__device__ __forceinline__ void cmac(double2 &acc, const double2 k, const double2 z) {
-    acc.x = fma(k.x, z.x, acc.x);
-    acc.y = fma(k.x, z.y, acc.y);
-    acc.x = fma(-k.y, z.y, acc.x);
-    acc.y = fma(k.y, z.x, acc.y);
+// acc += k z for a complex column; for the packed column 0 (two real filters: DC in .x, Nyquist in .y)
+// the caller passes (kb, kc, kd) = (0, k.y, 0) instead of (-k.y, k.x, k.y), giving acc += (k.x z.x, k.y z.y).
+__device__ __forceinline__ void cmac(double2 &acc, double ka, double kb, double kc, double kd, const double2 z) {
+    acc.x = fma(ka, z.x, acc.x);
+    acc.y = fma(kc, z.y, acc.y);
+    acc.x = fma(kb, z.y, acc.x);
+    acc.y = fma(kd, z.x, acc.y);
 }
 
 struct FirDims { int H, Nh, nimg, nKa, FK, NO, pad; };
@@ -85,6 +87,7 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
     __shared__ Seq sseq[kFirMaxFK];
     const int tid = threadIdx.x, col = tid & 31, wq = tid >> 5, bz = blockIdx.z;
     const int m = blockIdx.x * kFirCols + col;
+    const bool packed = (m == 0);          // column 0 holds (X[0], X[W/2]), both real
     const int H = d.H, Nh = d.Nh, FK = d.FK, nKa = d.nKa;
     for (int i = tid; i < L * FK * kFirCols; i += kFirCols * kFirWarps)
         kh[i] = __ldg(&khat[((size_t)bz * L * FK + (i >> 5)) * Nh + blockIdx.x * kFirCols + (i & 31)]);
@@ -131,8 +134,9 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
 #pragma unroll
             for (int ai = 0; ai < L; ++ai) {
                 const double2 k = kp[(size_t)ai * FK * kFirCols];
+                const double kb = packed ? 0.0 : -k.y, kc = packed ? k.y : k.x, kd = packed ? 0.0 : k.y;
 #pragma unroll
-                for (int q = 0; q < 4; ++q) cmac(acc[ai + q], k, z[q]);
+                for (int q = 0; q < 4; ++q) cmac(acc[ai + q], k.x, kb, kc, kd, z[q]);
             }
         }
         if (g >= lead) {
@@ -145,29 +149,6 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
 #pragma unroll
         for (int i = NA - 4; i < NA; ++i) acc[i] = make_double2(0.0, 0.0);
     }
-}
-
-// Column 0 holds (X[0], X[W/2]), both real: two real FIR filters, component by component.
-// grid: x = row block, y = batch.  Runs after k_fir_x and overwrites its column-0 output.
-__global__ void k_fir_col0(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const Seq *__restrict__ seqs,
-                           const double2 *__restrict__ khat, double2 *mhat, FirDims d, int L) {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x, bz = blockIdx.y;
-    if (x >= d.H) return;
-    const int w = (L - 1) / 2, H = d.H, Nh = d.Nh;
-    const double2 *rb = rhat + (size_t)bz * d.nimg * H * Nh;
-    double2 acc = make_double2(0.0, 0.0);
-    for (int ai = 0; ai < L; ++ai) {
-        const int xs = (x - (ai - w)) & (H - 1);
-        for (int t = 0; t < d.FK; ++t) {
-            const Seq sq = seqs[t];
-            const double f = __ldg(&xwt[(size_t)sq.xw * H + xs]);
-            const double2 rv = __ldg(&rb[((size_t)sq.img * H + xs) * Nh]);
-            const double2 k = __ldg(&khat[((size_t)bz * L * d.FK + ai * d.FK + t) * Nh]);
-            acc.x = fma(k.x, f * rv.x, acc.x);
-            acc.y = fma(k.y, f * rv.y, acc.y);
-        }
-    }
-    mhat[((size_t)bz * d.nimg * H + x) * Nh] = acc;
 }
 
 // D(x, .) = S(x, .) - irfft(mdl(x, .)) - sum_s b_s f'_i(x) g'_j(.)   for one row per thread row.
@@ -310,9 +291,6 @@ cudaError_t launch_subtract_fourier(sfft_plan *p, const double *d_coef, const do
         default: return cudaErrorInvalidValue;
     }
     if (e != cudaSuccess) return e;
-    k_fir_col0<<<dim3((p->H + 127) / 128, p->nbatch), 128, 0, p->stream>>>(p->rhat, p->dt.xwt, p->dt.seqs, p->khat,
-                                                                          p->rhat + (size_t)p->nKa * p->H * p->Nh, d, p->L);
-    p->launches++;
     switch (p->Nh) {
         case 512: return launch_inv<512>(p, d_coef, dS, dD);
         case 1024: return launch_inv<1024>(p, d_coef, dS, dD);
