@@ -29,6 +29,9 @@ from paper_2109_09334_b200 import synth  # noqa: E402
 
 METRIC = "difference-image pairs/s at 4096^2 FP64 (build+solve+subtract, L=17, DK=DB=2)"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/clk x 2 flop x 1.965 GHz
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's dominant kernel at config 4, from the
+# `ncu --set full` capture summarised in profiles/r01_c_launches_and_ncu_full.md (bytes)
+NCU_TRAFFIC_CFG4 = {"corr": 542.0e6 + 46.8e6, "rowfft": 268.6e6 + 478.7e6, "subtract": 467.8e6 + 113.1e6}
 
 
 def shard_units(nunits, rank, world):
@@ -271,15 +274,29 @@ def main():
             # lag correlation: SURVEY 8(d) pruned-FFT figure ~ (FK(FK+1)/2 + FK) maps x columns x 5 N log2 N x 0.6
             "corr": ("alu", (FK * (FK + 1) // 2 + FK) * (c["W"] // 2 + 1) * 5.0 * c["H"] * np.log2(c["H"]) * 0.6 * nb / 1e12,
                      FP64_PEAK_TFLOPS, "TFLOP/s"),
-            "subtract": ("alu", 2.0 * P * L * L * nKa * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
+            # subtract: SURVEY 8(d) Fourier-route figure, L*FK complex MACs per spectrum point (8 flop each)
+            "subtract": ("alu", 8.0 * L * FK * c["H"] * (c["W"] // 2) * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
             "solve": ("alu", (plan.n ** 3 / 3.0) * 2 * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
         }
         tname = names[top]
         bound, work, peak, unit = alg.get(tname, ("hbm", 0.0, hbm_peak, "GB/s"))
         achieved = work / (stage_ms[top] * 1e-3)
         roofline = {"kernel": tname, "bound": bound, "achieved": achieved, "peak": peak, "unit": unit,
-                    "frac": achieved / peak, "traffic": None, "ms": float(stage_ms[top]),
+                    "frac": achieved / peak, "traffic": NCU_TRAFFIC_CFG4.get(tname) if cfg == 4 else None,
+                    "ms": float(stage_ms[top]),
                     "peak_source": peak_src if bound == "hbm" else "derived: 148 SM x 64 FP64 FMA/clk x 1.965 GHz"}
+        if tname == "corr":
+            # the x-direction is executed as direct lag sums on the FP64 tensor cores: DMMA flops actually issued
+            ex = plan.corr_executed_flops() * nb
+            st_dm, dmma = B.sfft_measure_fp64_peak(1)
+            roofline["executed_tflops"] = ex / 1e12 / (stage_ms[top] * 1e-3)
+            roofline["dmma_peak_measured_tflops"] = dmma if st_dm == B.SFFT_OK else None
+        rf_all = {}
+        for nm, (bd, wk, pk, un) in alg.items():
+            t_ms = stage_ms[names.index(nm)]
+            if t_ms > 0:
+                rf_all[nm] = {"bound": bd, "achieved": round(wk / (t_ms * 1e-3), 3), "peak": round(pk, 1), "unit": un,
+                              "frac": round(wk / (t_ms * 1e-3) / pk, 4)}
         line = {
             "metric": METRIC, "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
@@ -291,6 +308,7 @@ def main():
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": roofline,
+            "stage_roofline": rf_all,
             "stage_ms": stages,
         }
         if not args.no_cpu_baseline and world == 1:

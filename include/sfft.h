@@ -68,6 +68,9 @@ int sfft_plan_set_stream(sfft_plan *plan, void *cuda_stream);
 /* n = F_K*L*L + F_B (Eq. 18's dimension), or -1 for a null plan. */
 int sfft_plan_num_unknowns(const sfft_plan *plan);
 int sfft_plan_num_kernel_terms(const sfft_plan *plan);     /* F_K */
+/* Measurement support: FP64 tensor-core flops (mma.sync.m8n8k4.f64, 512 each) one sfft_build_system issues
+ * per batch entry in the x-direction lag correlation (steps a3+a4), counted from the plan's job list. */
+double sfft_plan_corr_executed_flops(const sfft_plan *plan);
 int sfft_plan_num_background_terms(const sfft_plan *plan); /* F_B */
 
 /* Bytes of device workspace the plan needs for its current batch size. */

@@ -18,7 +18,7 @@ SFFT_OK, SFFT_ERR_INVALID_ARG, SFFT_ERR_STATE, SFFT_ERR_WORKSPACE, SFFT_ERR_CUDA
 # every symbol include/sfft.h declares (checked against the built library by tests/test_abi.py)
 EXPORTS = [
     "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_num_unknowns",
-    "sfft_plan_num_kernel_terms", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
+    "sfft_plan_num_kernel_terms", "sfft_plan_corr_executed_flops", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
     "sfft_subtract", "sfft_plan_status", "sfft_run_host", "sfft_plan_launch_count", "sfft_plan_destroy",
     "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
@@ -59,6 +59,7 @@ def load_library(build_if_missing=True):
         "sfft_plan_set_stream": (ci, [vp, vp]),
         "sfft_plan_num_unknowns": (ci, [vp]),
         "sfft_plan_num_kernel_terms": (ci, [vp]),
+        "sfft_plan_corr_executed_flops": (ctypes.c_double, [vp]),
         "sfft_plan_num_background_terms": (ci, [vp]),
         "sfft_plan_workspace_bytes": (cs, [vp]),
         "sfft_plan_set_workspace": (ci, [vp, vp, cs]),
@@ -284,6 +285,9 @@ class Plan:
         st, ms = sfft_plan_profile_read(self.h, nsteps)
         self._check(st, "sfft_plan_profile_read")
         return ms
+
+    def corr_executed_flops(self):
+        return load_library().sfft_plan_corr_executed_flops(self.h)
 
     def launch_count(self):
         return sfft_plan_launch_count(self.h)

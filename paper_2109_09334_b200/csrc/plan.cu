@@ -397,6 +397,16 @@ int sfft_plan_set_stream(sfft_plan *p, void *stream) {
 
 int sfft_plan_num_unknowns(const sfft_plan *p) { return p ? p->n : -1; }
 int sfft_plan_num_kernel_terms(const sfft_plan *p) { return p ? p->FK : -1; }
+double sfft_plan_corr_executed_flops(const sfft_plan *p) {
+    if (!p) return -1.0;
+    double f = 0.0;
+    for (const CorrJob &j : p->jobs) {
+        int rows = 0;
+        for (int r = 0; r < j.nrange; ++r) rows += j.xend[r] - j.xbeg[r];
+        f += 2.0 * (j.nblk[0] + j.nblk[1]) * 2.0 * 512.0 * (rows / 4) * p->Nh;    // 2 row blocks x blocks x (Re, Im) per 4 rows per column
+    }
+    return f;
+}
 int sfft_plan_num_background_terms(const sfft_plan *p) { return p ? p->FB : -1; }
 
 size_t sfft_plan_workspace_bytes(const sfft_plan *p) { return p ? ws_layout(p).total : 0; }
