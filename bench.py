@@ -276,7 +276,7 @@ def main():
                      FP64_PEAK_TFLOPS, "TFLOP/s"),
             # subtract: SURVEY 8(d) Fourier-route figure, L*FK complex MACs per spectrum point (8 flop each)
             "subtract": ("alu", 8.0 * L * FK * c["H"] * (c["W"] // 2) * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
-            "solve": ("alu", (plan.n ** 3 / 3.0) * 2 * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
+            "solve": ("alu", (plan.n ** 3 / 3.0) * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
         }
         tname = names[top]
         bound, work, peak, unit = alg.get(tname, ("hbm", 0.0, hbm_peak, "GB/s"))

@@ -123,6 +123,75 @@ def test_parity_full_size(cuda_device, cfg):
     assert np.max(np.abs(D[px, py] - Dref)) <= TOL_D * p.sigma
 
 
+def _oracle_column(R, L, bid, DK, DB, k, wcache):
+    """Column k of the design matrix Phi (Eqs. 3-4, 11-12) from the oracle's weighted images / axis tables."""
+    H, W = R.shape
+    LL, w = L * L, (L - 1) // 2
+    FK = oracle.num_terms(bid, DK)
+    if k < FK * LL:
+        t, a = divmod(k, LL)
+        al, be = a // L - w, a % L - w
+        if t not in wcache:
+            wcache[t] = oracle.weighted_ref(R, bid, DK, t)
+        Rt = wcache[t]
+        return Rt if (al == 0 and be == 0) else np.roll(Rt, (al, be), axis=(0, 1)) - Rt
+    i, j = oracle.terms(bid, DB)[k - FK * LL]
+    return np.outer(oracle.axis_table(bid, H, DB)[i], oracle.axis_table(bid, W, DB)[j])
+
+
+@pytest.mark.slow
+def test_parity_config5_full_size(cuda_device):
+    """Config 5 at BASELINE.json's sub-field size and basis (1024x1024, L=11, cubic B-splines with 4 interior
+    knots per axis, n = 7808), two sub-fields in one batched call.  The oracle's full system for this case is
+    ~1e12 pixel sums plus an unblocked n=7808 factorisation per sub-field, so it is checked on sampled outputs
+    the oracle computes one by one: 150 entries of M and 40 of rhs from the definition (oracle-weighted images,
+    np.roll), D on 2000 pixels through oracle.difference_at, and the coefficients against LAPACK + long-double
+    iterative refinement applied to the (sample-checked) GPU matrix."""
+    import torch
+    nb = 2
+    c5 = synth.CONFIGS[5]
+    pb = synth.make_batch(5, nbatch=nb)
+    L, DK, DB, bid = c5["L"], c5["DK"], c5["DB"], oracle.BSPLINE
+    M, rhs, c, D = _gpu_all(torch, pb, L, "bspline", DK, DB)
+    n = M.shape[1]
+    na = n - oracle.num_terms(bid, DB)
+    assert n == 7808
+    rng = np.random.default_rng(55)
+    for e in range(nb):
+        R, S = pb.R[e], pb.S[e]
+        assert np.array_equal(M[e], M[e].T)
+        d = np.sqrt(np.diag(M[e]))
+        # sampled entries: neighbouring spatial terms and lags (large), far-apart terms (zero overlap), background
+        ks = np.r_[rng.integers(0, na, 24), rng.integers(na, n, 6), [0, 60, na - 1, n - 1]]
+        cols, wc = {}, {}
+        for k in ks:
+            cols[int(k)] = _oracle_column(R, L, bid, DK, DB, int(k), wc)
+        kk = list(cols)
+        worst = 0.0
+        for a in range(len(kk)):
+            for b in range(a, len(kk), 3):
+                ref = float(np.sum(cols[kk[a]].astype(np.longdouble) * cols[kk[b]]))
+                worst = max(worst, abs(M[e][kk[a], kk[b]] - ref) / (d[kk[a]] * d[kk[b]]))
+        assert worst <= TOL_M, worst
+        sn = np.sqrt(np.sum(S * S))
+        for k in kk:
+            ref = float(np.sum(cols[k].astype(np.longdouble) * S))
+            assert abs(rhs[e][k] - ref) <= TOL_M * d[k] * sn
+        # solution of the GPU's own system by LAPACK + extended-precision refinement
+        ds = 1.0 / d
+        Ms, rs = M[e] * ds[:, None] * ds[None, :], rhs[e] * ds
+        x = np.linalg.solve(Ms, rs)
+        for _ in range(3):
+            r = rs.astype(np.longdouble) - Ms.astype(np.longdouble) @ x.astype(np.longdouble)
+            x = x + np.linalg.solve(Ms, r.astype(np.float64))
+        co = x * ds
+        _check_coef(c[e], co, na)
+        px, py = rng.integers(0, 1024, 2000), rng.integers(0, 1024, 2000)
+        px[:4], py[:4] = [0, 0, 1023, 1023], [0, 1023, 0, 1023]
+        Dref = oracle.difference_at(R, S, co, L, bid, DK, DB, px, py)
+        assert np.max(np.abs(D[e][px, py] - Dref)) <= TOL_D * pb.sigma
+
+
 def test_batch_matches_single(cuda_device):
     """nbatch = 3 independent pairs in one call: each entry equals the oracle on that pair."""
     import torch
