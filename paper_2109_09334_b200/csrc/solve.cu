@@ -194,7 +194,53 @@ __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double
     __syncthreads();
 }
 
+// U: rank-64 update of trailing tile `bx` = (ti, tj), tj <= ti, of the lower triangle right of strip k with
+// panel k-1 (columns jp0..jp0+63); j1 = first row/column after strip k.  T0, T1: MMA operand tiles.
+__device__ __forceinline__ void chol_update_tile(double *__restrict__ L, int ldl, int n, int j1, int jp0, int bx,
+                                                 double *T0, double *T1) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int r8 = lane >> 2, kq = lane & 3, wm = (warp >> 1) * 16, wn = (warp & 1) * 32;
+    int ti = (int)((sqrt(8.0 * (double)bx + 1.0) - 1.0) * 0.5);
+    while ((ti + 1) * (ti + 2) / 2 <= bx) ++ti;
+    while (ti * (ti + 1) / 2 > bx) --ti;
+    const int tj = bx - ti * (ti + 1) / 2;
+    const int i0 = j1 + ti * NB, c0 = j1 + tj * NB;
+    const int nri = max(0, min(NB, n + 1 - i0)), nrj = max(0, min(NB, n - c0));
+    {
+        TileRegs ta;
+        tile_fetch(ta, L, ldl, i0, jp0, nri);
+        tile_store(T0, ta);
+        if (tj != ti) {
+            tile_fetch(ta, L, ldl, c0, jp0, nrj);
+            tile_store(T1, ta);
+        }
+    }
+    __syncthreads();
+    double acc[2][4][2];
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc[a][c][0] = acc[a][c][1] = 0.0;
+    mma_64(T0, tj != ti ? T1 : T0, acc);
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int i = i0 + wm + 8 * a + r8, j = c0 + wn + 8 * c + 2 * kq;
+            if (i > n) continue;
+            double *dst = &L[(size_t)i * ldl + j];
+            if (j + 1 < n && j + 1 <= i) {
+                double2 v = *reinterpret_cast<double2 *>(dst);
+                v.x -= acc[a][c][0]; v.y -= acc[a][c][1];
+                *reinterpret_cast<double2 *>(dst) = v;
+            } else if (j < n && j <= i) {
+                dst[0] -= acc[a][c][0];
+            }
+        }
+}
+
 constexpr size_t kStepSmem = (size_t)(2 * NB * LDT + 4 * NB + NB + NB) * sizeof(double);
+constexpr size_t kUpdSmem = (size_t)(2 * NB * LDT) * sizeof(double);
 
 // One launch per panel k (see the header).  grid.x = nslab P CTAs, then ntiles U CTAs (k >= 1).
 __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, double *__restrict__ Winv, int *flag, int n,
@@ -282,45 +328,17 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
         return;
     }
     bx -= nslab;
-    if (bx < ntiles) {
-        // ------------------------------ U: trailing tile (ti, tj), tj <= ti, with panel k-1 ------------------------------
-        int ti = (int)((sqrt(8.0 * (double)bx + 1.0) - 1.0) * 0.5);
-        while ((ti + 1) * (ti + 2) / 2 <= bx) ++ti;
-        while (ti * (ti + 1) / 2 > bx) --ti;
-        const int tj = bx - ti * (ti + 1) / 2;
-        const int i0 = j1 + ti * NB, c0 = j1 + tj * NB;
-        const int nri = max(0, min(NB, n + 1 - i0)), nrj = max(0, min(NB, n - c0));
-        {
-            TileRegs ta, tb;
-            tile_fetch(ta, L, ldl, i0, jp0, nri);
-            if (tj != ti) tile_fetch(tb, L, ldl, c0, jp0, nrj);
-            tile_store(T0, ta);
-            if (tj != ti) tile_store(T1, tb);
-        }
-        __syncthreads();
-        double acc[2][4][2];
-#pragma unroll
-        for (int a = 0; a < 2; ++a)
-#pragma unroll
-            for (int c = 0; c < 4; ++c) acc[a][c][0] = acc[a][c][1] = 0.0;
-        mma_64(T0, tj != ti ? T1 : T0, acc);
-#pragma unroll
-        for (int a = 0; a < 2; ++a)
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int i = i0 + wm + 8 * a + r8, j = c0 + wn + 8 * c + 2 * kq;
-                if (i > n) continue;
-                double *dst = &L[(size_t)i * ldl + j];
-                if (j + 1 < n && j + 1 <= i) {
-                    double2 v = *reinterpret_cast<double2 *>(dst);
-                    v.x -= acc[a][c][0]; v.y -= acc[a][c][1];
-                    *reinterpret_cast<double2 *>(dst) = v;
-                } else if (j < n && j <= i) {
-                    dst[0] -= acc[a][c][0];
-                }
-            }
-        return;
-    }
+    if (bx < ntiles) chol_update_tile(L, ldl, n, j1, jp0, bx, T0, T1);
+}
+
+// The trailing update alone (U CTAs of launch k), for batched / large systems where it is throughput bound:
+// without the panel code this kernel needs half the registers, so three CTAs share an SM and one CTA's tile
+// loads overlap another's MMAs.  grid.x = ntiles, grid.y = batch.
+__global__ void __launch_bounds__(256, 3) k_chol_update(double *__restrict__ Lf, int n, int ldl, int k) {
+    extern __shared__ double sm[];
+    double *L = Lf + (size_t)blockIdx.y * (n + 1) * ldl;
+    const int j0 = k * NB, nb = min(NB, n - j0);
+    chol_update_tile(L, ldl, n, j0 + nb, j0 - NB, blockIdx.x, sm, sm + NB * LDT);
 }
 
 // Backward substitution L^T y = z (z = row n of Lf), c = D y.  One cluster of CS CTAs per system; CTA `rank`
@@ -403,14 +421,22 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     k_scale_copy<<<dim3((n + 127) / 128, n + 1, nbat), 128, 0, p->stream>>>(p->M, p->rhs, p->dscale, p->Lf, n, ldl);
     p->launches += 2;
     cudaError_t e = cudaFuncSetAttribute(k_chol_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStepSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUpdSmem);
     if (e != cudaSuccess) return e;
     for (int k = 0; k < nblk; ++k) {
         const int j1 = std::min(n, (k + 1) * NB);
         const int nslab = (n + 1 - j1 + NB - 1) / NB;                 // rows j1..n (the rhs row is row n)
         const int ntiles = k > 0 ? nslab * (nslab + 1) / 2 : 0;
-        k_chol_step<<<dim3(nslab + ntiles, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, nslab,
-                                                                               ntiles, nblk);
-        p->launches++;
+        if ((long)ntiles * nbat >= 16 * 148) {
+            // throughput regime: panel CTAs and the (register-lean) trailing update as two launches
+            k_chol_step<<<dim3(nslab, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, nslab, 0, nblk);
+            k_chol_update<<<dim3(ntiles, nbat), 256, kUpdSmem, p->stream>>>(p->Lf, n, ldl, k);
+            p->launches += 2;
+        } else {
+            k_chol_step<<<dim3(nslab + ntiles, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, nslab,
+                                                                                   ntiles, nblk);
+            p->launches++;
+        }
     }
     const int nown_max = (nblk + CS - 1) / CS;
     const size_t smem = ((size_t)nblk * NB + 4 * (size_t)nown_max * NB) * sizeof(double);
