@@ -52,6 +52,9 @@ def _load():
     L.orc_corr_diff_one.restype = ctypes.c_double
     L.orc_weighted_ref.argtypes = [_ci] * 5 + [_D, _D]
     L.orc_num_threads.restype = _ci
+    L.orc_cpr_num_unknowns.argtypes = [_ci] * 4
+    L.orc_cpr_constrain.argtypes = [_ci] * 4 + [_D] * 4
+    L.orc_cpr_expand.argtypes = [_ci] * 4 + [_D] * 2
     _lib = L
     return L
 
@@ -185,3 +188,25 @@ def weighted_ref(R, basis, DK, t):
     out = np.zeros((H, W))
     _load().orc_weighted_ref(H, W, basis, DK, t, R, out)
     return out
+
+
+def cpr_num_unknowns(L, basis, DK, DB):
+    """NEXT-1 (constant photometric ratio): number of unknowns n' = n - (F_K - 1)."""
+    return _load().orc_cpr_num_unknowns(L, basis, DK, DB)
+
+
+def cpr_constrain(M, rhs, L, basis, DK, DB):
+    """M' = C^T M C, rhs' = C^T rhs of the constant-kernel-integral model."""
+    M, rhs = _c(M), _c(rhs)
+    nr = cpr_num_unknowns(L, basis, DK, DB)
+    Mc, rc = np.zeros((nr, nr)), np.zeros(nr)
+    _load().orc_cpr_constrain(L, basis, DK, DB, M, rhs, Mc, rc)
+    return Mc, rc
+
+
+def cpr_expand(cr, L, basis, DK, DB):
+    """c = C c' (full coefficient layout, constrained entries filled in)."""
+    cr = _c(cr)
+    c = np.zeros(num_unknowns(L, basis, DK, DB))
+    _load().orc_cpr_expand(L, basis, DK, DB, cr, c)
+    return c

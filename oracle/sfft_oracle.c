@@ -456,6 +456,58 @@ void orc_difference_at(int H, int W, int L, int basis, int DK, int DB, const dou
     basis_free(&b);
 }
 
+/* ---------------------------------------------------------------------------------------------
+ * NEXT-1: constant photometric ratio.  "The constant flux scaling between
+ * images requires a constant kernel integral, that is, A_xy00 = a_0000": the kernel-sum field
+ * sum_t a_{t,00} T_t(x,y) must not depend on position.
+ *   POLY    : T_0 = 1 and the other monomials vary  =>  a_{t,00} = 0 for t >= 1.
+ *   BSPLINE : the T_t form a partition of unity      =>  all a_{t,00} equal.
+ * Either way c = C c' with one shared unknown s in place of the F_K centre coefficients:
+ *   c_k = c'_{r(k)} for a non-centre k;  c_{t*LL+a0} = omega_t * c'_s,  omega = e_0 (POLY) or 1 (BSPLINE),
+ * and the basis image of s is sum_t omega_t R^t = R.  The reduced unknowns keep the original order with
+ * the centre entries of t >= 1 removed (s sits where a_{0,00} was), n' = n - (F_K - 1).
+ * Least squares over c' has the normal system  M' = C^T M C,  rhs' = C^T rhs  (plain definition).
+ * ------------------------------------------------------------------------------------------- */
+int orc_cpr_num_unknowns(int L, int basis, int DK, int DB) {
+    return orc_num_unknowns(L, basis, DK, DB) - (orc_num_terms(basis, DK) - 1);
+}
+
+/* map[k] = reduced index of full unknown k; wgt[k] = its weight omega (1 for non-centre entries) */
+static void cpr_map(int L, int basis, int DK, int DB, int *map, double *wgt) {
+    int FK = orc_num_terms(basis, DK), LL = L * L, a0 = (L / 2) * L + L / 2, n = orc_num_unknowns(L, basis, DK, DB);
+    int next = 0;
+    for (int k = 0; k < n; ++k) {
+        int centre = (k < FK * LL) && (k % LL == a0), t = k / LL;
+        if (centre && t >= 1) { map[k] = a0; wgt[k] = (basis == ORC_POLY) ? 0.0 : 1.0; }
+        else { map[k] = next++; wgt[k] = 1.0; }
+    }
+}
+
+void orc_cpr_constrain(int L, int basis, int DK, int DB, const double *M, const double *rhs, double *Mc, double *rc) {
+    int n = orc_num_unknowns(L, basis, DK, DB), nr = orc_cpr_num_unknowns(L, basis, DK, DB);
+    int *map = (int *)malloc(sizeof(int) * n);
+    double *wgt = (double *)malloc(sizeof(double) * n);
+    long double *acc = (long double *)calloc((size_t)nr * nr, sizeof(long double));
+    long double *ar = (long double *)calloc((size_t)nr, sizeof(long double));
+    cpr_map(L, basis, DK, DB, map, wgt);
+    for (int k = 0; k < n; ++k) {
+        ar[map[k]] += (long double)wgt[k] * rhs[k];
+        for (int l = 0; l < n; ++l) acc[(size_t)map[k] * nr + map[l]] += (long double)wgt[k] * wgt[l] * M[(size_t)k * n + l];
+    }
+    for (size_t i = 0; i < (size_t)nr * nr; ++i) Mc[i] = (double)acc[i];
+    for (int i = 0; i < nr; ++i) rc[i] = (double)ar[i];
+    free(map); free(wgt); free(acc); free(ar);
+}
+
+void orc_cpr_expand(int L, int basis, int DK, int DB, const double *cr, double *c) {
+    int n = orc_num_unknowns(L, basis, DK, DB);
+    int *map = (int *)malloc(sizeof(int) * n);
+    double *wgt = (double *)malloc(sizeof(double) * n);
+    cpr_map(L, basis, DK, DB, map, wgt);
+    for (int k = 0; k < n; ++k) c[k] = wgt[k] * cr[map[k]];
+    free(map); free(wgt);
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -333,3 +333,70 @@ def test_affine_coordinate_invariance_of_difference():
     Phi = np.array(cols).T
     c_raw = np.linalg.lstsq(Phi, S.ravel(), rcond=None)[0]
     np.testing.assert_allclose(D.ravel(), S.ravel() - Phi @ c_raw, rtol=0, atol=1e-8)
+
+
+# --------------------------------------------------------------------------- NEXT-1: constant photometric ratio
+
+def _cpr_design(R, L, basis, DK, DB):
+    """Design matrix of the constant-kernel-integral model written from PAPER.md:121 directly: the F_K centre
+    columns R^t are replaced by ONE column, the unweighted reference R (the kernel integral multiplies R itself)."""
+    Phi = oracle.design_matrix(R, L, basis, DK, DB)
+    FK, LL, a0 = oracle.num_terms(basis, DK), L * L, (L // 2) * L + L // 2
+    keep = [k for k in range(Phi.shape[0]) if not (k < FK * LL and k % LL == a0 and k >= LL)]
+    Phir = Phi[keep].copy()
+    Phir[a0] = R.ravel()
+    return Phir
+
+
+@pytest.mark.parametrize("basis,DK,DB", [(POLY, 1, 1), (POLY, 2, 0), (BSPL, 1, 0)])
+def test_cpr_system_and_solution_vs_bruteforce_lstsq(basis, DK, DB):
+    """Catches a wrong index map (which centre entries merge), a wrong weight (zero vs one) and a transposed C."""
+    H, W, L = 14, 18, 3
+    R, S = _rand_pair(H, W, 21)
+    M, rhs = oracle.normal_from_lags(R, S, L, basis, DK, DB)
+    Mc, rc = oracle.cpr_constrain(M, rhs, L, basis, DK, DB)
+    Phir = _cpr_design(R, L, basis, DK, DB)
+    assert Mc.shape[0] == Phir.shape[0] == oracle.cpr_num_unknowns(L, basis, DK, DB)
+    assert np.allclose(Mc, Phir @ Phir.T, rtol=1e-11, atol=1e-8 * np.abs(Mc).max() * 1e-3)
+    assert np.allclose(rc, Phir @ S.ravel(), rtol=1e-11)
+    cr = oracle.solve(Mc, rc)
+    ref = np.linalg.lstsq(Phir.T, S.ravel(), rcond=None)[0]
+    assert np.max(np.abs(cr - ref)) <= 1e-8 * np.max(np.abs(ref))
+    # expansion reproduces the same model image
+    c = oracle.cpr_expand(cr, L, basis, DK, DB)
+    Phi = oracle.design_matrix(R, L, basis, DK, DB)
+    assert np.allclose(Phi.T @ c, Phir.T @ cr, rtol=1e-12, atol=1e-9)
+
+
+@pytest.mark.parametrize("basis,DK", [(POLY, 2), (BSPL, 1)])
+def test_cpr_kernel_integral_is_constant_over_the_field(basis, DK):
+    """A_xy00 = a_0000.  The kernel-sum field sum_t a_{t,00} T_t(x,y) of the expanded solution must
+    not depend on (x, y) and must equal the shared unknown."""
+    H, W, L, DB = 16, 16, 3, 1
+    R, S = _rand_pair(H, W, 22)
+    M, rhs = oracle.normal_from_lags(R, S, L, basis, DK, DB)
+    cr = oracle.solve(*oracle.cpr_constrain(M, rhs, L, basis, DK, DB))
+    c = oracle.cpr_expand(cr, L, basis, DK, DB)
+    fx, gy = oracle.axis_table(basis, H, DK), oracle.axis_table(basis, W, DK)
+    a0, LL = (L // 2) * L + L // 2, L * L
+    field = sum(c[t * LL + a0] * np.outer(fx[i], gy[j]) for t, (i, j) in enumerate(oracle.terms(basis, DK)))
+    assert np.allclose(field, cr[a0], rtol=1e-12, atol=1e-12)
+
+
+def test_cpr_recovers_constant_scale_with_varying_kernel():
+    """Noiseless S = 1.25 * (R convolved with a kernel whose SHAPE varies linearly in x but whose sum is 1) + 7:
+    the constrained fit recovers the scale 1.25 as the shared unknown and leaves a zero difference."""
+    H, W, L, DK, DB = 24, 24, 3, 1, 0
+    rng = np.random.default_rng(5)
+    R = 100.0 + 50.0 * rng.random((H, W))
+    ux = _u(H)[:, None] * np.ones((1, W))
+    # model image built from the definition: scale * [R + g(x) * (shifted copies - R)], g = 0.2 + 0.1 u_x at the source pixel
+    g = 0.2 + 0.1 * ux
+    Rg = R * g
+    S = 1.25 * (R + (np.roll(Rg, (1, 0), (0, 1)) - Rg) + (np.roll(Rg, (0, -1), (0, 1)) - Rg)) + 7.0
+    M, rhs = oracle.normal_from_lags(R, S, L, POLY, DK, DB)
+    cr = oracle.solve(*oracle.cpr_constrain(M, rhs, L, POLY, DK, DB))
+    a0 = (L // 2) * L + L // 2
+    assert abs(cr[a0] - 1.25) <= 1e-9
+    c = oracle.cpr_expand(cr, L, POLY, DK, DB)
+    assert np.max(np.abs(oracle.difference(R, S, c, L, POLY, DK, DB))) <= 1e-8
