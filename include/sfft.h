@@ -65,6 +65,14 @@ int sfft_plan_set_batch(sfft_plan *plan, int nbatch);
 /* CUDA stream (cudaStream_t cast to void*; NULL = legacy default stream). */
 int sfft_plan_set_stream(sfft_plan *plan, void *cuda_stream);
 
+/* NEXT-1, constant photometric ratio (PAPER.md:121, 264 -ConstPhotRatio): on = 1 constrains the kernel integral
+ * sum_t a_{t,00} T_t(x,y) to a constant (POLY: a_{t,00} = 0 for t >= 1; BSPLINE: all a_{t,00} equal), leaving
+ * sfft_plan_num_solved() = n - (F_K - 1) unknowns in the system returned by sfft_get_system (order of the full
+ * layout with the centre entries of t >= 1 removed).  Coefficient vectors keep the full layout of n entries,
+ * the constrained ones filled in.  Default 0 (BASELINE.json's unknown counts).  Call before sfft_build_system. */
+int sfft_plan_set_const_phot_ratio(sfft_plan *plan, int on);
+int sfft_plan_num_solved(const sfft_plan *plan);
+
 /* n = F_K*L*L + F_B (Eq. 18's dimension), or -1 for a null plan. */
 int sfft_plan_num_unknowns(const sfft_plan *plan);
 int sfft_plan_num_kernel_terms(const sfft_plan *plan);     /* F_K */

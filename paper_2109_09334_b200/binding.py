@@ -17,7 +17,7 @@ SFFT_OK, SFFT_ERR_INVALID_ARG, SFFT_ERR_STATE, SFFT_ERR_WORKSPACE, SFFT_ERR_CUDA
 
 # every symbol include/sfft.h declares (checked against the built library by tests/test_abi.py)
 EXPORTS = [
-    "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_num_unknowns",
+    "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
     "sfft_plan_num_kernel_terms", "sfft_plan_corr_executed_flops", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
     "sfft_subtract", "sfft_plan_status", "sfft_run_host", "sfft_plan_launch_count", "sfft_plan_destroy",
@@ -57,6 +57,8 @@ def load_library(build_if_missing=True):
         "sfft_plan_create": (ci, [pvp, ci, ci, ci, ci, ci, ci]),
         "sfft_plan_set_batch": (ci, [vp, ci]),
         "sfft_plan_set_stream": (ci, [vp, vp]),
+        "sfft_plan_set_const_phot_ratio": (ci, [vp, ci]),
+        "sfft_plan_num_solved": (ci, [vp]),
         "sfft_plan_num_unknowns": (ci, [vp]),
         "sfft_plan_num_kernel_terms": (ci, [vp]),
         "sfft_plan_corr_executed_flops": (ctypes.c_double, [vp]),
@@ -114,6 +116,14 @@ def sfft_plan_set_batch(plan, nbatch):
 
 def sfft_plan_set_stream(plan, stream_ptr):
     return load_library().sfft_plan_set_stream(plan, ctypes.c_void_p(stream_ptr))
+
+
+def sfft_plan_set_const_phot_ratio(plan, on):
+    return load_library().sfft_plan_set_const_phot_ratio(plan, int(on))
+
+
+def sfft_plan_num_solved(plan):
+    return load_library().sfft_plan_num_solved(plan)
 
 
 def sfft_plan_num_unknowns(plan):
@@ -198,7 +208,7 @@ def _basis_id(basis):
 class Plan:
     """sfft_plan handle + workspace tensor on the current CUDA device and stream."""
 
-    def __init__(self, H, W, L, DK, DB, basis="poly", nbatch=1, device="cuda:0"):
+    def __init__(self, H, W, L, DK, DB, basis="poly", nbatch=1, device="cuda:0", const_phot_ratio=False):
         import torch
         if not torch.cuda.is_available():
             raise SfftError(SFFT_ERR_CUDA, "Plan", "no CUDA device: libsfft_b200 has no CPU fallback")
@@ -210,7 +220,9 @@ class Plan:
             raise SfftError(st, "sfft_plan_create")
         self.H, self.W, self.L, self.nbatch = H, W, L, nbatch
         self._check(sfft_plan_set_batch(self.h, nbatch), "sfft_plan_set_batch")
+        self._check(sfft_plan_set_const_phot_ratio(self.h, const_phot_ratio), "sfft_plan_set_const_phot_ratio")
         self.n = sfft_plan_num_unknowns(self.h)
+        self.ns = sfft_plan_num_solved(self.h)
         self.ws_bytes = sfft_plan_workspace_bytes(self.h)
         self.ws = torch.empty(self.ws_bytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (self.ws.data_ptr() + 255) & ~255
@@ -262,7 +274,7 @@ class Plan:
         st, pM, pr, ld = sfft_get_system(self.h)
         self._check(st, "sfft_get_system")
         self.status()
-        return self._ws_view(pM, (self.nbatch, self.n, ld)), self._ws_view(pr, (self.nbatch, self.n))
+        return self._ws_view(pM, (self.nbatch, self.ns, ld)), self._ws_view(pr, (self.nbatch, self.ns))
 
     def lag_table(self, which):
         st, pt, cnt = sfft_get_lag_table(self.h, which)

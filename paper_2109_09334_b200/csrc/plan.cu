@@ -232,7 +232,7 @@ void free_tables(sfft_plan *p) {
 }
 
 struct WsLayout {
-    size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, kfold, ctab, khat, flag, stR, stS, stD, stC, total;
+    size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, coefr, kfold, ctab, khat, flag, stR, stS, stD, stC, total;
 };
 
 WsLayout ws_layout(const sfft_plan *p) {
@@ -252,6 +252,7 @@ WsLayout ws_layout(const sfft_plan *p) {
     l.Lf = take(nb * (n + 1) * (size_t)p->ldl * sizeof(double));
     l.Winv = take(nb * (size_t)solve_num_blocks(p->n) * 64 * 64 * sizeof(double));
     l.dscale = take(nb * n * sizeof(double));
+    l.coefr = take(nb * n * sizeof(double));
     l.kfold = take(nb * (size_t)p->FK * p->L * p->L * sizeof(double));
     l.ctab = take(nb * (size_t)p->H * p->L * p->LT * sizeof(double));
     l.khat = take(subtract_use_fourier(p) ? nb * (size_t)p->L * p->FK * p->Nh * sizeof(double2) : 0);
@@ -287,6 +288,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     term_list(basis, DB, p->bti, p->btj);
     p->FK = (int)p->kti.size(); p->FB = (int)p->bti.size();
     p->n = p->FK * L * L + p->FB;
+    p->ns = p->n;
     p->nimg = p->nKa + 1;
     p->ldl = (p->n + 1 + 7) & ~7;
     p->LT = subtract_kpad(p->nKa, L);
@@ -389,6 +391,16 @@ int sfft_plan_set_batch(sfft_plan *p, int nbatch) {
     return SFFT_OK;
 }
 
+int sfft_plan_set_const_phot_ratio(sfft_plan *p, int on) {
+    if (!p || (on != 0 && on != 1)) return SFFT_ERR_INVALID_ARG;
+    p->cpr = on;
+    p->ns = on ? p->n - (p->FK - 1) : p->n;
+    p->built = p->solved = false;
+    return SFFT_OK;
+}
+
+int sfft_plan_num_solved(const sfft_plan *p) { return p ? p->ns : -1; }
+
 int sfft_plan_set_stream(sfft_plan *p, void *stream) {
     if (!p) return SFFT_ERR_INVALID_ARG;
     p->stream = (cudaStream_t)stream;
@@ -420,7 +432,7 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     p->rhat = (double2 *)(b + l.rhat); p->G = (double2 *)(b + l.G); p->lagpart = (double *)(b + l.lagpart); p->tab = (double *)(b + l.tab);
     p->Q = (double *)(b + l.Q); p->QS = (double *)(b + l.QS); p->LamC = (double *)(b + l.LamC); p->mu = (double *)(b + l.mu);
     p->M = (double *)(b + l.M); p->rhs = (double *)(b + l.rhs); p->Lf = (double *)(b + l.Lf); p->Winv = (double *)(b + l.Winv);
-    p->dscale = (double *)(b + l.dscale); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
+    p->dscale = (double *)(b + l.dscale); p->coefr = (double *)(b + l.coefr); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
     p->stageR = (double *)(b + l.stR); p->stageS = (double *)(b + l.stS); p->stageD = (double *)(b + l.stD);
     p->stageC = (double *)(b + l.stC);
     p->built = p->solved = false;
@@ -488,7 +500,7 @@ int sfft_get_system(const sfft_plan *p, const double **d_M, const double **d_rhs
     if (!p->built) return SFFT_ERR_STATE;
     if (d_M) *d_M = p->M;
     if (d_rhs) *d_rhs = p->rhs;
-    if (ld) *ld = p->n;
+    if (ld) *ld = p->ns;
     return SFFT_OK;
 }
 

@@ -68,6 +68,8 @@ struct DeviceTables {
 struct sfft_plan {
     int H = 0, W = 0, L = 0, w = 0, DK = 0, DB = 0, basis = 0, nbatch = 1;
     int FK = 0, FB = 0, nKa = 0, nBa = 0, n = 0, Nh = 0;
+    int cpr = 0;         // constant photometric ratio: centre coefficients of the terms t >= 1 not free
+    int ns = 0;          // solved unknowns: n, or n - (FK - 1) under cpr
     int nimg = 0;        // spectrum stack depth per batch entry: nKa weighted-y images + S
     int nseq = 0;        // FK + 1 column sequences (kernel terms, then S)
     int E = 0;           // G entries per spectrum column: nseq*nseq*L
@@ -96,6 +98,7 @@ struct sfft_plan {
     double2 *khat = nullptr;                    // [b][L*FK][Nh] row spectra of the pixel kernels (Fourier-route subtract)
     const double *rhat_src = nullptr;           // device buffer whose weighted row spectra rhat[0..nKa) currently holds
     bool rhat_valid = false;
+    double *coefr = nullptr;                    // [b][ns] reduced solution (cpr) before expansion to the full layout
     double *stageR = nullptr, *stageS = nullptr, *stageD = nullptr, *stageC = nullptr;
     int *flag = nullptr;
     cudaStream_t stream = nullptr;
@@ -113,6 +116,7 @@ cudaError_t launch_corr(sfft_plan *p);
 cudaError_t launch_lagsum(sfft_plan *p);
 cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS);
 cudaError_t launch_gather(sfft_plan *p);
+cudaError_t launch_expand_coef(sfft_plan *p, const double *d_cr, double *d_coef);   // c = C c' (cpr)
 cudaError_t launch_solve(sfft_plan *p, double *d_coef);
 int solve_num_blocks(int n);     // 64-column panels of the Cholesky factorisation
 int subtract_kpad(int nKa, int L);

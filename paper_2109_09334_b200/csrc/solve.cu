@@ -416,7 +416,8 @@ k_chol_backsolve(const double *__restrict__ Lf, const double *__restrict__ Winv,
 int solve_num_blocks(int n) { return (n + NB - 1) / NB; }
 
 cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
-    const int n = p->n, ldl = p->ldl, nbat = p->nbatch, nblk = solve_num_blocks(n);
+    const int n = p->ns, ldl = p->ldl, nbat = p->nbatch, nblk = solve_num_blocks(n);
+    double *d_out = p->cpr ? p->coefr : d_coef;      // reduced solution first when the photometric ratio is constrained
     k_scale_diag<<<dim3((n + 255) / 256, nbat), 256, 0, p->stream>>>(p->M, p->dscale, p->flag, n);
     k_scale_copy<<<dim3((n + 127) / 128, n + 1, nbat), 128, 0, p->stream>>>(p->M, p->rhs, p->dscale, p->Lf, n, ldl);
     p->launches += 2;
@@ -442,9 +443,11 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     const size_t smem = ((size_t)nblk * NB + 4 * (size_t)nown_max * NB) * sizeof(double);
     e = cudaFuncSetAttribute(k_chol_backsolve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_chol_backsolve<<<dim3(CS, nbat), 256, smem, p->stream>>>(p->Lf, p->Winv, p->dscale, d_coef, n, ldl, nblk, nown_max);
+    k_chol_backsolve<<<dim3(CS, nbat), 256, smem, p->stream>>>(p->Lf, p->Winv, p->dscale, d_out, n, ldl, nblk, nown_max);
     p->launches++;
-    return cudaGetLastError();
+    e = cudaGetLastError();
+    if (e == cudaSuccess && p->cpr) e = launch_expand_coef(p, p->coefr, d_coef);
+    return e;
 }
 
 }  // namespace sfft

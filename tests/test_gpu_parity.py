@@ -237,6 +237,36 @@ def test_batch_fourier_route(cuda_device):
         assert np.max(np.abs(D[e] - Do)) <= TOL_D * pb.sigma
 
 
+@pytest.mark.parametrize("cfg,H,W,L,basis,DK,DB", [
+    (1, None, None, None, "poly", 1, 1),          # config 1 with the paper's default -ConstPhotRatio True: 148 unknowns
+    (2, 64, 1024, 9, "poly", 2, 1),               # Fourier-route subtract
+    (5, 128, 128, 5, "bspline", 1, 0),            # B-splines: all centre coefficients equal (shared unknown sums 25 terms)
+    (2, 64, 64, 1, "poly", 2, 1),                 # L = 1: only the scale and the background remain
+])
+def test_parity_constant_photometric_ratio(cuda_device, cfg, H, W, L, basis, DK, DB):
+    """NEXT-1: constrained normal system, solution (full layout) and difference."""
+    import torch
+    p = synth.make_pair(cfg, H=H, W=W)
+    L = p.L if L is None else L
+    bid = _bid(basis)
+    Mf, rf = oracle.normal_from_lags(p.R, p.S, L, bid, DK, DB)
+    Mo, ro = oracle.cpr_constrain(Mf, rf, L, bid, DK, DB)
+    co = oracle.cpr_expand(oracle.solve(Mo, ro), L, bid, DK, DB)
+    Do = oracle.difference(p.R, p.S, co, L, bid, DK, DB)
+    plan = B.Plan(p.H, p.W, L, DK, DB, basis, const_phot_ratio=True)
+    assert plan.ns == oracle.cpr_num_unknowns(L, bid, DK, DB) and plan.n == Mf.shape[0]
+    dR, dS = torch.from_numpy(p.R).cuda(), torch.from_numpy(p.S).cuda()
+    plan.build_system(dR, dS)
+    coef = plan.solve()
+    D = plan.subtract(coef, dR, dS)
+    plan.status()
+    M, rhs = plan.system()
+    _check_system(M[0].cpu().numpy(), rhs[0].cpu().numpy(), Mo, ro, p.S)
+    _check_coef(coef[0].cpu().numpy(), co, Mf.shape[0] - oracle.num_terms(bid, DB))
+    assert np.max(np.abs(D.cpu().numpy() - Do)) <= TOL_D * p.sigma
+    plan.close()
+
+
 def test_identical_images(cuda_device):
     """S = R  =>  a_{0,centre} = 1, everything else 0, D = 0 (degenerate but full-rank case)."""
     import torch
