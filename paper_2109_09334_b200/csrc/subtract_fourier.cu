@@ -26,6 +26,7 @@ namespace {
 constexpr int kFirCols = 32;     // spectrum columns per CTA of k_fir_x (one warp = one x-range of 32 columns)
 constexpr int kFirWarps = 4;     // x-ranges per CTA
 constexpr int kFirMaxFK = 48;
+constexpr int kFirMaxNKa = 8;    // x-basis functions of the FIR route (their 4-row weight tiles live in shared memory)
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -102,6 +103,13 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
     double2 *rtw = rt + (size_t)wq * nKa * 4 * kFirCols + col;
     const size_t bufstride = (size_t)kFirWarps * nKa * 4 * kFirCols;
 
+    // x-weights f_i(x) of the 4 rows of a group, per warp: lane (i*4+q) fetches one value a group ahead
+    // (register), stores it at the top of the next group; __syncwarp orders the store before the reads.
+    double *fws = reinterpret_cast<double *>(smf + (size_t)L * FK * kFirCols + 2 * bufstride) + wq * 2 * 4 * kFirMaxNKa;
+    const int lane = col;
+    auto fetch_w = [&](int g) -> double {
+        return lane < nKa * 4 ? __ldg(&xwt[(size_t)(lane >> 2) * H + ((xs0 + 4 * g + (lane & 3)) & (H - 1))]) : 0.0;
+    };
     auto issue = [&](int g) {
         double2 *dst = rtw + (size_t)(g & 1) * bufstride;
         for (int j = 0; j < nKa; ++j)
@@ -117,8 +125,12 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
 #pragma unroll
     for (int i = 0; i < NA; ++i) acc[i] = make_double2(0.0, 0.0);
     issue(0);
+    double wnext = fetch_w(0);
     for (int g = 0; g < ngroups; ++g) {
-        if (g + 1 < ngroups) { issue(g + 1); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+        double *fw = fws + (g & 1) * 4 * kFirMaxNKa;
+        if (lane < nKa * 4) fw[lane] = wnext;
+        if (g + 1 < ngroups) { issue(g + 1); wnext = fetch_w(g + 1); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+        __syncwarp();
         const double2 *r = rtw + (size_t)(g & 1) * bufstride;
         const int xg = xs0 + 4 * g;
         for (int t = 0; t < FK; ++t) {
@@ -126,7 +138,7 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
             double2 z[4];
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const double f = __ldg(&xwt[(size_t)sq.xw * H + ((xg + q) & (H - 1))]);
+                const double f = fw[sq.xw * 4 + q];
                 const double2 rv = r[(sq.img * 4 + q) * kFirCols];
                 z[q] = make_double2(f * rv.x, f * rv.y);
             }
@@ -229,7 +241,8 @@ cudaError_t launch_inv(sfft_plan *p, const double *d_coef, const double *dS, dou
 }
 
 size_t fir_smem(const sfft_plan *p) {
-    return ((size_t)p->L * p->FK * kFirCols + 2 * (size_t)kFirWarps * p->nKa * 4 * kFirCols) * sizeof(double2);
+    return ((size_t)p->L * p->FK * kFirCols + 2 * (size_t)kFirWarps * p->nKa * 4 * kFirCols) * sizeof(double2) +
+           (size_t)kFirWarps * 2 * 4 * kFirMaxNKa * sizeof(double);
 }
 
 template <int L>
@@ -251,7 +264,7 @@ cudaError_t launch_fir(sfft_plan *p, const FirDims &d, int ny) {
 // pixel, plus the transforms, on the plain FMA pipe at ~half the efficiency of the tensor-core contraction)
 // is below the direct form's (L+7) * KP tensor-core MACs per pixel.
 bool subtract_use_fourier(const sfft_plan *p) {
-    if (p->Nh < 512 || p->L < 9 || p->L > 25 || p->FK > kFirMaxFK || p->nBa > 16) return false;
+    if (p->Nh < 512 || p->L < 9 || p->L > 25 || p->FK > kFirMaxFK || p->nKa > kFirMaxNKa || p->nBa > 16) return false;
     if (fir_smem(p) > 200 * 1024) return false;
     const double direct = (double)(p->L + 7) * subtract_kpad(p->nKa, p->L);
     const double fourier = 2.5 * (2.0 * p->L * p->FK) + 40.0 * (p->nKa + 1);
