@@ -32,13 +32,19 @@ __global__ void __launch_bounds__(128) k_lagsum_partial(const double2 *__restric
     for (int k = 0; k < LP; ++k) P[k] = Q[k] = 0.0;
     for (int xs = 0; xs < Sx; ++xs) {
         const double2 *g = G + (((size_t)bz * Sx + xs) * (Nh + 1) + mbeg) * E + e;
-        for (int mm = 0; mm < mcnt; ++mm) {
-            const double2 v = g[(size_t)mm * E];
+        // eight column loads in flight per thread (the loop is otherwise one L2 round trip per column)
+        for (int m8 = 0; m8 < mcnt; m8 += 8) {
+            double2 v[8];
 #pragma unroll
-            for (int k = 0; k < LP; ++k) {
-                const double2 t = tw[mm][k];
-                P[k] = fma(v.x, t.x, P[k]);
-                Q[k] = fma(v.y, t.y, Q[k]);
+            for (int q = 0; q < 8; ++q) v[q] = (m8 + q < mcnt) ? g[(size_t)(m8 + q) * E] : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+#pragma unroll
+                for (int k = 0; k < LP; ++k) {
+                    const double2 t = tw[m8 + q][k];
+                    P[k] = fma(v[q].x, t.x, P[k]);
+                    Q[k] = fma(v[q].y, t.y, Q[k]);
+                }
             }
         }
     }
@@ -58,9 +64,16 @@ __global__ void k_lagsum_final(const double *__restrict__ part, const LagUnit *_
     const int eps = j - u.hw, k = eps < 0 ? -eps : eps;
     const double *src = part + ((size_t)bz * nch * L + k) * 2 * E + u.e;
     double P = 0.0, Q = 0.0;
-    for (int ch = 0; ch < nch; ++ch) {
-        P += src[(size_t)ch * L * 2 * E];
-        Q += src[(size_t)ch * L * 2 * E + E];
+    for (int c8 = 0; c8 < nch; c8 += 8) {
+        double p8[8], q8[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const bool ok = c8 + q < nch;
+            p8[q] = ok ? src[(size_t)(c8 + q) * L * 2 * E] : 0.0;
+            q8[q] = ok ? src[(size_t)(c8 + q) * L * 2 * E + E] : 0.0;
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { P += p8[q]; Q += q8[q]; }      // fixed order: deterministic
     }
     const int s = (eps == 0) ? 0 : ((eps > 0) == (u.sgn > 0) ? 1 : -1);
     tab[(size_t)bz * tab_size + u.dst_off + j] = P - s * Q;
