@@ -341,6 +341,75 @@ __global__ void __launch_bounds__(256, 3) k_chol_update(double *__restrict__ Lf,
     chol_update_tile(L, ldl, n, j0 + nb, j0 - NB, blockIdx.x, sm, sm + NB * LDT);
 }
 
+// Slab CTAs of launch k without the diagonal-block factorisation (throughput regime): slab `1 + blockIdx.x`
+// applies panel k-1 to its 64 rows of strip k and multiplies by W^T, with W = L_kk^-1 read from Winv (written
+// by the one k_chol_step CTA per system launched just before).  grid.x = nslab - 1, grid.y = batch.
+__global__ void __launch_bounds__(256, 2) k_chol_slab(double *__restrict__ Lf, const double *__restrict__ Winv, int n,
+                                                      int ldl, int k, int nblk) {
+    extern __shared__ double sm[];
+    double *T0 = sm, *T1 = sm + NB * LDT;
+    const int b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int r8 = lane >> 2, kq = lane & 3, wm = (warp >> 1) * 16, wn = (warp & 1) * 32;
+    double *L = Lf + (size_t)b * (n + 1) * ldl;
+    const int j0 = k * NB, nb = min(NB, n - j0), j1 = j0 + nb, jp0 = j0 - NB;
+    const int r0 = j1 + (blockIdx.x + 1) * NB, nr = max(0, min(NB, n + 1 - r0));
+    if (nr <= 0) return;
+    double acc[2][4][2], xv[2][4][2];
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq + q;
+                acc[a][c][q] = 0.0;
+                xv[a][c][q] = (r < nr && cc < nb) ? L[(size_t)(r0 + r) * ldl + j0 + cc] : 0.0;
+            }
+    if (k > 0) {
+        TileRegs t;
+        tile_fetch(t, L, ldl, j0, jp0, nb);      // diagonal-block rows of panel k-1
+        tile_store(T0, t);
+        tile_fetch(t, L, ldl, r0, jp0, nr);      // slab rows of panel k-1
+        tile_store(T1, t);
+        __syncthreads();
+        mma_64(T1, T0, acc);
+        __syncthreads();
+    }
+    // S = strip values minus the look-ahead update (operand tile T1); W (operand tile T0)
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq + q;
+                T1[r * LDT + cc] = (r < nr && cc < nb) ? xv[a][c][q] - acc[a][c][q] : 0.0;
+                acc[a][c][q] = 0.0;
+            }
+    {
+        const double *W = Winv + ((size_t)b * nblk + k) * NB * NB;
+#pragma unroll
+        for (int q = 0; q < NB * NB / 2 / 256; ++q) {
+            const int i = tid + 256 * q, r = i >> 5, c = (i & 31) * 2;
+            const double2 v = *reinterpret_cast<const double2 *>(&W[r * NB + c]);
+            T0[r * LDT + c] = v.x;
+            T0[r * LDT + c + 1] = v.y;
+        }
+    }
+    __syncthreads();
+    mma_64(T1, T0, acc);
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq;
+            if (r >= nr) continue;
+            double *dst = &L[(size_t)(r0 + r) * ldl + j0 + cc];
+            if (cc + 1 < nb) *reinterpret_cast<double2 *>(dst) = make_double2(acc[a][c][0], acc[a][c][1]);
+            else if (cc < nb) dst[0] = acc[a][c][0];
+        }
+}
+
 // Backward substitution L^T y = z (z = row n of Lf), c = D y.  One cluster of CS CTAs per system; CTA `rank`
 // owns the 64-column blocks with block % CS == rank and keeps their part of z in shared memory.  Per diagonal
 // block (from the last): the owner forms y_b = W_b^T z_b, broadcasts it through distributed shared memory, and
@@ -423,6 +492,7 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     p->launches += 2;
     cudaError_t e = cudaFuncSetAttribute(k_chol_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStepSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUpdSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_slab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUpdSmem);
     if (e != cudaSuccess) return e;
     for (int k = 0; k < nblk; ++k) {
         const int j1 = std::min(n, (k + 1) * NB);
@@ -430,7 +500,12 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
         const int ntiles = k > 0 ? nslab * (nslab + 1) / 2 : 0;
         if ((long)ntiles * nbat >= 16 * 148) {
             // throughput regime: panel CTAs and the (register-lean) trailing update as two launches
-            k_chol_step<<<dim3(nslab, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, nslab, 0, nblk);
+            // one factoring CTA per system (it also solves slab 0), lean CTAs for the other slabs, then the update
+            k_chol_step<<<dim3(1, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, 1, 0, nblk);
+            if (nslab > 1) {
+                k_chol_slab<<<dim3(nslab - 1, nbat), 256, kUpdSmem, p->stream>>>(p->Lf, p->Winv, n, ldl, k, nblk);
+                p->launches++;
+            }
             k_chol_update<<<dim3(ntiles, nbat), 256, kUpdSmem, p->stream>>>(p->Lf, n, ldl, k);
             p->launches += 2;
         } else {
