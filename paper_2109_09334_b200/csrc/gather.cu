@@ -23,12 +23,14 @@ __device__ __forceinline__ double omega(const double *om, const GatherDims &d, i
 }
 
 // entry (kb <= k) of the full normal matrix, from the lag tables
-__device__ __forceinline__ double m_entry(const double *om, const double *la, const double *phi0, const GatherDims &d,
-                                          int kb, int k) {
+// kdec[k] = t << 16 | (alpha + w) << 8 | (beta + w) for a kernel unknown k (plan table: no integer divisions here)
+__device__ __forceinline__ double m_entry(const double *om, const double *la, const double *phi0, const int *kdec,
+                                          const GatherDims &d, int kb, int k) {
     const int na = d.FK * d.LL;
     if (k < na) {
-        int tbar = kb / d.LL, ab = kb % d.LL, t = k / d.LL, a = k % d.LL;
-        int alb = ab / d.L - d.w, beb = ab % d.L - d.w, al = a / d.L - d.w, be = a % d.L - d.w;
+        const int db = __ldg(&kdec[kb]), dk = __ldg(&kdec[k]);
+        const int tbar = db >> 16, t = dk >> 16;
+        const int alb = ((db >> 8) & 255) - d.w, beb = (db & 255) - d.w, al = ((dk >> 8) & 255) - d.w, be = (dk & 255) - d.w;
         bool cb = (alb == 0 && beb == 0), c = (al == 0 && be == 0);
         double o0 = omega(om, d, tbar, t, 0, 0);
         if (cb && c) return o0;
@@ -38,7 +40,8 @@ __device__ __forceinline__ double m_entry(const double *om, const double *la, co
                (omega(om, d, tbar, t, -al, -be) - o0);
     }
     if (kb < na) {
-        int tbar = kb / d.LL, ab = kb % d.LL, s = k - na;
+        const int db = __ldg(&kdec[kb]);
+        const int tbar = db >> 16, ab = ((db >> 8) & 255) * d.L + (db & 255), s = k - na;
         const double *l = la + ((size_t)tbar * d.FB + s) * d.LL;
         double l0 = l[d.w * d.L + d.w];
         return (ab == d.w * d.L + d.w) ? l0 : l[ab] - l0;
@@ -67,8 +70,8 @@ __device__ __forceinline__ int full_index(const GatherDims &d, int r) {
     return t * d.LL + (a < a0 ? a : a + 1);
 }
 
-__global__ void k_gather(const double *__restrict__ tab, const double *__restrict__ phi0, double *__restrict__ M,
-                         double *__restrict__ rhs, GatherDims d) {
+__global__ void k_gather(const double *__restrict__ tab, const double *__restrict__ phi0, const int *__restrict__ kdec,
+                         double *__restrict__ M, double *__restrict__ rhs, GatherDims d) {
     const int col = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y, b = blockIdx.z;
     if (col >= d.ns) return;
     const double *tb_ = tab + (size_t)b * d.tab_size;
@@ -82,7 +85,7 @@ __global__ void k_gather(const double *__restrict__ tab, const double *__restric
     for (int p = 0; p < nlo; ++p)
         for (int q = 0; q < nhi; ++q) {
             const int k1 = klo + p * d.LL, k2 = khi + q * d.LL;
-            v += m_entry(om, la, phi0, d, min(k1, k2), max(k1, k2));
+            v += m_entry(om, la, phi0, kdec, d, min(k1, k2), max(k1, k2));
         }
     M[((size_t)b * d.ns + row) * d.ns + col] = v;
     if (row == 0) {   // the first row of CTAs also fills the right-hand side
@@ -121,7 +124,7 @@ static GatherDims gather_dims(const sfft_plan *p) {
 cudaError_t launch_gather(sfft_plan *p) {
     GatherDims d = gather_dims(p);
     dim3 grid((p->ns + 127) / 128, p->ns, p->nbatch);
-    k_gather<<<grid, 128, 0, p->stream>>>(p->tab, p->dt.phi0, p->M, p->rhs, d);
+    k_gather<<<grid, 128, 0, p->stream>>>(p->tab, p->dt.phi0, p->dt.kdec, p->M, p->rhs, d);
     p->launches++;
     return cudaGetLastError();
 }

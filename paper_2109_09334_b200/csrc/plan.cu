@@ -227,7 +227,7 @@ void free_tables(sfft_plan *p) {
     cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.lagtw); cudaFree(d.cy); cudaFree(d.fx); cudaFree(d.cq); cudaFree(d.cwr);
     cudaFree(d.phi0);
     cudaFree(d.seqs); cudaFree(d.jobs); cudaFree(d.units);
-    cudaFree(d.kti); cudaFree(d.ktj); cudaFree(d.bti); cudaFree(d.btj);
+    cudaFree(d.kdec); cudaFree(d.kti); cudaFree(d.ktj); cudaFree(d.bti); cudaFree(d.btj);
     d = DeviceTables();
 }
 
@@ -376,6 +376,10 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     DeviceTables &d = p->dt;
 #define UP(dst, vec) if (e == cudaSuccess) e = upload(&d.dst, vec.data(), vec.size())
     UP(xwt, xwt); UP(gK, gK); UP(gB, gB); UP(twW, twW); UP(lagtw, lagtw); UP(cy, cy); UP(fx, fx); UP(cq, cq); UP(cwr, cwr); UP(phi0, phi0);
+    std::vector<int> kdec((size_t)p->FK * L * L);
+    for (int t = 0; t < p->FK; ++t)
+        for (int a = 0; a < L * L; ++a) kdec[(size_t)t * L * L + a] = (t << 16) | ((a / L) << 8) | (a % L);
+    UP(kdec, kdec);
     UP(seqs, p->seqs); UP(jobs, p->jobs); UP(units, p->units);
     UP(kti, p->kti); UP(ktj, p->ktj); UP(bti, p->bti); UP(btj, p->btj);
 #undef UP

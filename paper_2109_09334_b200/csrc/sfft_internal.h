@@ -61,6 +61,7 @@ struct DeviceTables {
     CorrJob *jobs = nullptr;
     LagUnit *units = nullptr;
     int *kti = nullptr, *ktj = nullptr, *bti = nullptr, *btj = nullptr;
+    int *kdec = nullptr;        // [FK*L*L]         t << 16 | (alpha+w) << 8 | (beta+w) of every kernel unknown (gather.cu)
 };
 
 }  // namespace sfft
