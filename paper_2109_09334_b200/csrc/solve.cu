@@ -241,6 +241,7 @@ __device__ __forceinline__ void chol_update_tile(double *__restrict__ L, int ldl
 
 constexpr size_t kStepSmem = (size_t)(2 * NB * LDT + 4 * NB + NB + NB) * sizeof(double);
 constexpr size_t kUpdSmem = (size_t)(2 * NB * LDT) * sizeof(double);
+constexpr size_t kRowSmem = (size_t)(3 * NB * LDT) * sizeof(double);
 
 // One launch per panel k (see the header).  grid.x = nslab P CTAs, then ntiles U CTAs (k >= 1).
 __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, double *__restrict__ Winv, int *flag, int n,
@@ -339,6 +340,73 @@ __global__ void __launch_bounds__(256, 3) k_chol_update(double *__restrict__ Lf,
     double *L = Lf + (size_t)blockIdx.y * (n + 1) * ldl;
     const int j0 = k * NB, nb = min(NB, n - j0);
     chol_update_tile(L, ldl, n, j0 + nb, j0 - NB, blockIdx.x, sm, sm + NB * LDT);
+}
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(a), "l"(gmem));
+}
+
+// T[r][0..63] = L[row0 + r][col0 ..] for r < nr (else 0) by asynchronous 16-byte copies (stride LDT)
+__device__ __forceinline__ void tile_fetch_async(double *T, const double *L, int ldl, int row0, int col0, int nr) {
+#pragma unroll
+    for (int q = 0; q < NB * NB / 2 / 256; ++q) {
+        const int i = threadIdx.x + 256 * q, r = i >> 5, c = (i & 31) * 2;
+        if (r < nr) cp_async16(&T[r * LDT + c], &L[(size_t)(row0 + r) * ldl + col0 + c]);
+        else { T[r * LDT + c] = 0.0; T[r * LDT + c + 1] = 0.0; }
+    }
+    asm volatile("cp.async.commit_group;");
+}
+
+// Trailing update, throughput regime: one CTA per tile ROW ti of the lower triangle right of strip k.  The row's
+// own panel rows stay in shared memory; the column operands A_tj stream through a double buffer (cp.async) and
+// the C tile is fetched into registers before the MMAs, so loads of tile tj+1 overlap the MMAs of tile tj.
+// grid.x = nslab (row nslab-1-blockIdx.x: long rows first), grid.y = batch.
+__global__ void __launch_bounds__(256, 2) k_chol_update_row(double *__restrict__ Lf, int n, int ldl, int k, int nslab) {
+    extern __shared__ double sm[];
+    double *Ti = sm, *Tj0 = sm + NB * LDT, *Tj1 = sm + 2 * NB * LDT;
+    double *L = Lf + (size_t)blockIdx.y * (n + 1) * ldl;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int r8 = lane >> 2, kq = lane & 3, wm = (warp >> 1) * 16, wn = (warp & 1) * 32;
+    const int j0 = k * NB, nb = min(NB, n - j0), j1 = j0 + nb, jp0 = j0 - NB;
+    const int ti = nslab - 1 - blockIdx.x, i0 = j1 + ti * NB;
+    const int nri = max(0, min(NB, n + 1 - i0));
+    if (nri <= 0) return;
+    tile_fetch_async(Ti, L, ldl, i0, jp0, nri);
+    if (ti > 0) tile_fetch_async(Tj0, L, ldl, j1, jp0, min(NB, n - j1));
+    for (int tj = 0; tj <= ti; ++tj) {
+        const int c0 = j1 + tj * NB;
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                 // tile tj (and Ti) visible; MMAs of tile tj-1 done by every warp
+        if (tj + 1 < ti) tile_fetch_async((tj & 1) ? Tj0 : Tj1, L, ldl, c0 + NB, jp0, max(0, min(NB, n - (c0 + NB))));
+        // C tile into registers ahead of the MMAs
+        double2 cv[2][4];
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int i = i0 + wm + 8 * a + r8, j = c0 + wn + 8 * c + 2 * kq;
+                cv[a][c] = make_double2(0.0, 0.0);
+                if (i <= n && j + 1 < n && j + 1 <= i) cv[a][c] = *reinterpret_cast<const double2 *>(&L[(size_t)i * ldl + j]);
+                else if (i <= n && j < n && j <= i) cv[a][c].x = L[(size_t)i * ldl + j];
+            }
+        double acc[2][4][2];
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) acc[a][c][0] = acc[a][c][1] = 0.0;
+        mma_64(Ti, tj == ti ? Ti : ((tj & 1) ? Tj1 : Tj0), acc);
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int i = i0 + wm + 8 * a + r8, j = c0 + wn + 8 * c + 2 * kq;
+                if (i > n) continue;
+                double *dst = &L[(size_t)i * ldl + j];
+                if (j + 1 < n && j + 1 <= i) *reinterpret_cast<double2 *>(dst) = make_double2(cv[a][c].x - acc[a][c][0], cv[a][c].y - acc[a][c][1]);
+                else if (j < n && j <= i) dst[0] = cv[a][c].x - acc[a][c][0];
+            }
+    }
 }
 
 // Slab CTAs of launch k without the diagonal-block factorisation (throughput regime): slab `1 + blockIdx.x`
@@ -492,6 +560,7 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     p->launches += 2;
     cudaError_t e = cudaFuncSetAttribute(k_chol_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStepSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUpdSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_update_row, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_slab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUpdSmem);
     if (e != cudaSuccess) return e;
     for (int k = 0; k < nblk; ++k) {
@@ -506,7 +575,9 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
                 k_chol_slab<<<dim3(nslab - 1, nbat), 256, kUpdSmem, p->stream>>>(p->Lf, p->Winv, n, ldl, k, nblk);
                 p->launches++;
             }
-            k_chol_update<<<dim3(ntiles, nbat), 256, kUpdSmem, p->stream>>>(p->Lf, n, ldl, k);
+            // many systems: one CTA per tile row (operand reuse + software pipelining); few: one CTA per tile
+            if ((long)nslab * nbat >= 2048) k_chol_update_row<<<dim3(nslab, nbat), 256, kRowSmem, p->stream>>>(p->Lf, n, ldl, k, nslab);
+            else k_chol_update<<<dim3(ntiles, nbat), 256, kUpdSmem, p->stream>>>(p->Lf, n, ldl, k);
             p->launches += 2;
         } else {
             k_chol_step<<<dim3(nslab + ntiles, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, nslab,
