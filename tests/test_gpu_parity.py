@@ -225,6 +225,24 @@ def test_batch_solve_grid_beyond_one_wave(cuda_device):
     assert np.max(np.abs(D[e] - Do)) <= TOL_D * pb.sigma
 
 
+def test_batch_solve_large_batch_regime(cuda_device):
+    """nbatch = 80 systems of n = 1664 (26 slabs): the solve takes its throughput path (one factoring CTA per
+    system, lean slab CTAs, trailing update by tile rows with the cp.async double buffer).  Entries 0, 41, 79
+    against the same pair run alone (latency path), entry 79 against the oracle."""
+    import torch
+    nb, L, DK, DB = 80, 5, 4, 4
+    pb = synth.make_batch(5, nbatch=nb, H=128, W=128)
+    M, rhs, c, D = _gpu_all(torch, pb, L, "bspline", DK, DB)
+    for e in (0, 41, 79):
+        M1, r1, c1, D1 = _gpu_all(torch, pb, L, "bspline", DK, DB, R=pb.R[e], S=pb.S[e])
+        assert np.max(np.abs(c[e] - c1[0])) <= TOL_C * np.max(np.abs(c1[0]))
+        assert np.max(np.abs(D[e] - D1)) <= TOL_D * pb.sigma
+    e = nb - 1
+    Mo, ro, co, Do = _oracle_all(pb.R[e], pb.S[e], L, "bspline", DK, DB)
+    _check_coef(c[e], co, Mo.shape[0] - 64)
+    assert np.max(np.abs(D[e] - Do)) <= TOL_D * pb.sigma
+
+
 def test_batch_fourier_route(cuda_device):
     """nbatch = 2 through the Fourier-route subtract (per-entry kernel spectra and spectrum stacks)."""
     import torch
