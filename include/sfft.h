@@ -91,7 +91,9 @@ int sfft_plan_set_workspace(sfft_plan *plan, void *d_ws, size_t bytes);
 /* Steps a1-a5: assemble the normal system of Eq. 18 in real-space scaling,
  * M = Phi^T Phi, rhs = Phi^T S, from the pair (d_R, d_S), each [nbatch][H][W] double.
  * Every block is a cross-correlation of weighted images evaluated by FFT and read at the
- * kernel-lag offsets only (App. B).  Inputs are not modified. */
+ * kernel-lag offsets only (App. B).  Inputs are not modified.
+ * Part of the work (the image-by-basis-function moments) is enqueued on a stream the plan owns, forked from
+ * and joined back into the plan's stream with events: ordering on the plan's stream is all a caller sees. */
 int sfft_build_system(sfft_plan *plan, const double *d_R, const double *d_S);
 
 /* Device pointers to the assembled system (valid until the next build): M is [nbatch][n][ld]

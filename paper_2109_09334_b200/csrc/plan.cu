@@ -383,7 +383,10 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     UP(seqs, p->seqs); UP(jobs, p->jobs); UP(units, p->units);
     UP(kti, p->kti); UP(ktj, p->ktj); UP(bti, p->bti); UP(btj, p->btj);
 #undef UP
-    if (e != cudaSuccess) { free_tables(p); delete p; cudaGetLastError(); return SFFT_ERR_CUDA; }
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
+    if (e != cudaSuccess) { sfft_plan_destroy(p); cudaGetLastError(); return SFFT_ERR_CUDA; }
     *out = p;
     return SFFT_OK;
 }
@@ -451,6 +454,21 @@ int sfft_build_system(sfft_plan *p, const double *d_R, const double *d_S) {
     cudaError_t e = cudaMemsetAsync(p->flag, 0xff, sizeof(int) * 2 * p->nbatch, p->stream);  // -1 = no failure
     if (p->prof_steps > 0) p->prof_cur = p->prof_cur + 1;   // a build opens the next profiled step
     prof_mark(p, 0);
+    // The moment stage depends only on (R, S): unless stages are being timed it is forked onto the plan's
+    // side stream, where its streaming passes run beside the tensor-bound lag correlation, and joined
+    // before the gather.
+    const bool fork = p->side && p->prof_steps <= 0;
+    if (fork && e == cudaSuccess) {
+        e = cudaEventRecord(p->ev_fork, p->stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->side, p->ev_fork, 0);
+        if (e == cudaSuccess) {
+            cudaStream_t main = p->stream;
+            p->stream = p->side;
+            e = launch_moments(p, d_R, d_S);
+            p->stream = main;
+        }
+        if (e == cudaSuccess) e = cudaEventRecord(p->ev_join, p->side);
+    }
     if (e == cudaSuccess) e = launch_rowfft_forward(p, d_R, d_S);
     p->rhat_src = d_R; p->rhat_valid = (e == cudaSuccess);
     prof_mark(p, 1);
@@ -458,7 +476,8 @@ int sfft_build_system(sfft_plan *p, const double *d_R, const double *d_S) {
     prof_mark(p, 2);
     if (e == cudaSuccess) e = launch_lagsum(p);
     prof_mark(p, 3);
-    if (e == cudaSuccess) e = launch_moments(p, d_R, d_S);
+    if (!fork && e == cudaSuccess) e = launch_moments(p, d_R, d_S);
+    if (fork && e == cudaSuccess) e = cudaStreamWaitEvent(p->stream, p->ev_join, 0);
     prof_mark(p, 4);
     if (e == cudaSuccess) e = launch_gather(p);
     prof_mark(p, 5);
@@ -579,6 +598,9 @@ long sfft_plan_launch_count(const sfft_plan *p) { return p ? p->launches : -1; }
 void sfft_plan_destroy(sfft_plan *p) {
     if (!p) return;
     for (cudaEvent_t ev : p->prof_events) cudaEventDestroy(ev);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
+    if (p->side) cudaStreamDestroy(p->side);
     free_tables(p);
     delete p;
 }

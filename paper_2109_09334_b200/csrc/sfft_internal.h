@@ -103,6 +103,8 @@ struct sfft_plan {
     double *stageR = nullptr, *stageS = nullptr, *stageD = nullptr, *stageC = nullptr;
     int *flag = nullptr;
     cudaStream_t stream = nullptr;
+    cudaStream_t side = nullptr;                // plan-owned stream: the moment stage (HBM bound) runs beside the
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;   // tensor-bound lag correlation (fork/join on `stream`)
     bool built = false, solved = false;
     long launches = 0;
     int prof_steps = 0, prof_cur = -1;          // stage profiling (sfft_plan_profile)
