@@ -159,15 +159,17 @@ __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double
             }
             if (tid == 0) pivs[k] = piv;
             const double inv = fast_rcp(piv);
+            // only the lower sub-blocks (a >= bb >= b) are ever read: the step is bound by FP64 issue
+            // (two warps per scheduler, two cycles per FP64 warp instruction), so the dead upper ones are skipped
             double lr[4];
 #pragma unroll
-            for (int a = 0; a < 4; ++a) lr[a] = cb[ty + 16 * a] * inv;
+            for (int a = b; a < 4; ++a) lr[a] = cb[ty + 16 * a] * inv;
 #pragma unroll
             for (int bb = b; bb < 4; ++bb) {
                 const double lc = cb[tx + 16 * bb];
                 if (bb > b || tx > kk) {
 #pragma unroll
-                    for (int a = 0; a < 4; ++a) t[a][bb] = fma(-lr[a], lc, t[a][bb]);
+                    for (int a = bb; a < 4; ++a) t[a][bb] = fma(-lr[a], lc, t[a][bb]);
                 }
             }
 #pragma unroll
