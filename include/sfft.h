@@ -133,6 +133,14 @@ int sfft_plan_status(sfft_plan *plan, int *info);
  * h_D [nbatch][H][W], h_coef [nbatch][n] (either may be NULL to skip that copy). */
 int sfft_run_host(sfft_plan *plan, const double *h_R, const double *h_S, double *h_D, double *h_coef);
 
+/* The same, without the final synchronisation: the host-to-device copies, the compute and the device-to-host
+ * copies are enqueued on three streams (two of them owned by the plan) over two staging slots, so that the
+ * copies of one pair overlap the compute of the previous one when calls are issued back to back.  Host buffers
+ * must be page-locked for the copies to be asynchronous and must stay valid (h_D, h_coef: unread) until
+ * sfft_run_host_wait returns.  sfft_run_host_wait drains everything submitted and reports like sfft_plan_status. */
+int sfft_run_host_async(sfft_plan *plan, const double *h_R, const double *h_S, double *h_D, double *h_coef);
+int sfft_run_host_wait(sfft_plan *plan);
+
 /* Per-stage device timing.  sfft_plan_profile(plan, nsteps) with nsteps > 0 makes the next nsteps
  * build/solve/subtract rounds record CUDA events on the plan's stream around each stage (no host
  * synchronisation; 0 disables).  sfft_plan_profile_read synchronises the stream and writes

@@ -20,7 +20,7 @@ EXPORTS = [
     "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
     "sfft_plan_num_kernel_terms", "sfft_plan_corr_executed_flops", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
-    "sfft_subtract", "sfft_plan_status", "sfft_run_host", "sfft_plan_launch_count", "sfft_plan_destroy",
+    "sfft_subtract", "sfft_plan_status", "sfft_run_host", "sfft_run_host_async", "sfft_run_host_wait", "sfft_plan_launch_count", "sfft_plan_destroy",
     "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
     "sfft_measure_fp64_peak",
 ]
@@ -72,6 +72,8 @@ def load_library(build_if_missing=True):
         "sfft_subtract": (ci, [vp, vp, vp, vp, vp]),
         "sfft_plan_status": (ci, [vp, pci]),
         "sfft_run_host": (ci, [vp, vp, vp, vp, vp]),
+        "sfft_run_host_async": (ci, [vp, vp, vp, vp, vp]),
+        "sfft_run_host_wait": (ci, [vp]),
         "sfft_plan_launch_count": (ctypes.c_long, [vp]),
         "sfft_plan_destroy": (None, [vp]),
         "sfft_strerror": (ctypes.c_char_p, [ci]),
@@ -172,6 +174,15 @@ def sfft_plan_status(plan):
 def sfft_run_host(plan, h_R, h_S, h_D, h_coef):
     return load_library().sfft_run_host(plan, ctypes.c_void_p(h_R), ctypes.c_void_p(h_S), ctypes.c_void_p(h_D),
                                         ctypes.c_void_p(h_coef))
+
+
+def sfft_run_host_async(plan, h_R, h_S, h_D, h_coef):
+    return load_library().sfft_run_host_async(plan, ctypes.c_void_p(h_R), ctypes.c_void_p(h_S), ctypes.c_void_p(h_D),
+                                              ctypes.c_void_p(h_coef))
+
+
+def sfft_run_host_wait(plan):
+    return load_library().sfft_run_host_wait(plan)
 
 
 def sfft_plan_launch_count(plan):

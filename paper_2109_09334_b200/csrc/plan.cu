@@ -232,7 +232,7 @@ void free_tables(sfft_plan *p) {
 }
 
 struct WsLayout {
-    size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, coefr, kfold, ctab, khat, flag, stR, stS, stD, stC, total;
+    size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, coefr, kfold, ctab, khat, flag, stR[2], stS[2], stD[2], stC[2], total;
 };
 
 WsLayout ws_layout(const sfft_plan *p) {
@@ -257,10 +257,12 @@ WsLayout ws_layout(const sfft_plan *p) {
     l.ctab = take(nb * (size_t)p->H * p->L * p->LT * sizeof(double));
     l.khat = take(subtract_use_fourier(p) ? nb * (size_t)p->L * p->FK * p->Nh * sizeof(double2) : 0);
     l.flag = take(nb * sizeof(int) * 2);
-    l.stR = take(nb * P * sizeof(double));
-    l.stS = take(nb * P * sizeof(double));
-    l.stD = take(nb * P * sizeof(double));
-    l.stC = take(nb * n * sizeof(double));
+    for (int q = 0; q < 2; ++q) {
+        l.stR[q] = take(nb * P * sizeof(double));
+        l.stS[q] = take(nb * P * sizeof(double));
+        l.stD[q] = take(nb * P * sizeof(double));
+        l.stC[q] = take(nb * n * sizeof(double));
+    }
     l.total = off;
     return l;
 }
@@ -386,6 +388,13 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking);
+    for (int q = 0; q < 2 && e == cudaSuccess; ++q) {
+        e = cudaEventCreateWithFlags(&p->ev_in[q], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_done[q], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_out[q], cudaEventDisableTiming);
+    }
     if (e != cudaSuccess) { sfft_plan_destroy(p); cudaGetLastError(); return SFFT_ERR_CUDA; }
     *out = p;
     return SFFT_OK;
@@ -440,8 +449,11 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     p->Q = (double *)(b + l.Q); p->QS = (double *)(b + l.QS); p->LamC = (double *)(b + l.LamC); p->mu = (double *)(b + l.mu);
     p->M = (double *)(b + l.M); p->rhs = (double *)(b + l.rhs); p->Lf = (double *)(b + l.Lf); p->Winv = (double *)(b + l.Winv);
     p->dscale = (double *)(b + l.dscale); p->coefr = (double *)(b + l.coefr); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
-    p->stageR = (double *)(b + l.stR); p->stageS = (double *)(b + l.stS); p->stageD = (double *)(b + l.stD);
-    p->stageC = (double *)(b + l.stC);
+    for (int q = 0; q < 2; ++q) {
+        p->stageR[q] = (double *)(b + l.stR[q]); p->stageS[q] = (double *)(b + l.stS[q]);
+        p->stageD[q] = (double *)(b + l.stD[q]); p->stageC[q] = (double *)(b + l.stC[q]);
+    }
+    p->host_slot = 0;
     p->built = p->solved = false;
     p->rhat_valid = false;
     return SFFT_OK;
@@ -575,22 +587,47 @@ int sfft_plan_status(sfft_plan *p, int *info) {
     return SFFT_OK;
 }
 
-int sfft_run_host(sfft_plan *p, const double *h_R, const double *h_S, double *h_D, double *h_coef) {
+int sfft_run_host_async(sfft_plan *p, const double *h_R, const double *h_S, double *h_D, double *h_coef) {
     if (!p || !h_R || !h_S) return SFFT_ERR_INVALID_ARG;
     if (!p->ws) return SFFT_ERR_WORKSPACE;
-    size_t img = (size_t)p->nbatch * p->H * p->W * sizeof(double);
-    cudaError_t e = cudaMemcpyAsync(p->stageR, h_R, img, cudaMemcpyHostToDevice, p->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(p->stageS, h_S, img, cudaMemcpyHostToDevice, p->stream);
+    const int q = p->host_slot;
+    p->host_slot ^= 1;
+    const size_t img = (size_t)p->nbatch * p->H * p->W * sizeof(double);
+    // H2D on the copy stream, after the previous user of this slot (two calls ago) has finished computing
+    cudaError_t e = cudaStreamWaitEvent(p->s_h2d, p->ev_done[q], 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(p->stageR[q], h_R, img, cudaMemcpyHostToDevice, p->s_h2d);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(p->stageS[q], h_S, img, cudaMemcpyHostToDevice, p->s_h2d);
+    if (e == cudaSuccess) e = cudaEventRecord(p->ev_in[q], p->s_h2d);
+    // compute on the plan's stream once the inputs are in and the slot's previous result has left
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->stream, p->ev_in[q], 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->stream, p->ev_out[q], 0);
     if (e != cudaSuccess) return fail_cuda(p, e);
-    int st = sfft_build_system(p, p->stageR, p->stageS);
-    if (st == SFFT_OK) st = sfft_solve(p, p->stageC);
-    if (st == SFFT_OK) st = sfft_subtract(p, p->stageC, p->stageR, p->stageS, p->stageD);
+    int st = sfft_build_system(p, p->stageR[q], p->stageS[q]);
+    if (st == SFFT_OK) st = sfft_solve(p, p->stageC[q]);
+    if (st == SFFT_OK) st = sfft_subtract(p, p->stageC[q], p->stageR[q], p->stageS[q], p->stageD[q]);
     if (st != SFFT_OK) return st;
-    if (h_D) e = cudaMemcpyAsync(h_D, p->stageD, img, cudaMemcpyDeviceToHost, p->stream);
+    e = cudaEventRecord(p->ev_done[q], p->stream);
+    // D2H on the other copy stream
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_d2h, p->ev_done[q], 0);
+    if (e == cudaSuccess && h_D) e = cudaMemcpyAsync(h_D, p->stageD[q], img, cudaMemcpyDeviceToHost, p->s_d2h);
     if (e == cudaSuccess && h_coef)
-        e = cudaMemcpyAsync(h_coef, p->stageC, (size_t)p->nbatch * p->n * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
+        e = cudaMemcpyAsync(h_coef, p->stageC[q], (size_t)p->nbatch * p->n * sizeof(double), cudaMemcpyDeviceToHost, p->s_d2h);
+    if (e == cudaSuccess) e = cudaEventRecord(p->ev_out[q], p->s_d2h);
+    if (e != cudaSuccess) return fail_cuda(p, e);
+    return SFFT_OK;
+}
+
+int sfft_run_host_wait(sfft_plan *p) {
+    if (!p) return SFFT_ERR_INVALID_ARG;
+    cudaError_t e = cudaStreamSynchronize(p->s_h2d);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->s_d2h);
     if (e != cudaSuccess) return fail_cuda(p, e);
     return sfft_plan_status(p, nullptr);
+}
+
+int sfft_run_host(sfft_plan *p, const double *h_R, const double *h_S, double *h_D, double *h_coef) {
+    int st = sfft_run_host_async(p, h_R, h_S, h_D, h_coef);
+    return st == SFFT_OK ? sfft_run_host_wait(p) : st;
 }
 
 long sfft_plan_launch_count(const sfft_plan *p) { return p ? p->launches : -1; }
@@ -601,6 +638,13 @@ void sfft_plan_destroy(sfft_plan *p) {
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);
     if (p->side) cudaStreamDestroy(p->side);
+    for (int q = 0; q < 2; ++q) {
+        if (p->ev_in[q]) cudaEventDestroy(p->ev_in[q]);
+        if (p->ev_done[q]) cudaEventDestroy(p->ev_done[q]);
+        if (p->ev_out[q]) cudaEventDestroy(p->ev_out[q]);
+    }
+    if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
+    if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
     free_tables(p);
     delete p;
 }

@@ -100,7 +100,12 @@ struct sfft_plan {
     const double *rhat_src = nullptr;           // device buffer whose weighted row spectra rhat[0..nKa) currently holds
     bool rhat_valid = false;
     double *coefr = nullptr;                    // [b][ns] reduced solution (cpr) before expansion to the full layout
-    double *stageR = nullptr, *stageS = nullptr, *stageD = nullptr, *stageC = nullptr;
+    // host-call staging: two slots so that the copies of one pair overlap the compute of another (sfft_run_host_async)
+    double *stageR[2] = {nullptr, nullptr}, *stageS[2] = {nullptr, nullptr}, *stageD[2] = {nullptr, nullptr},
+           *stageC[2] = {nullptr, nullptr};
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;           // plan-owned copy streams
+    cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+    int host_slot = 0;                                       // next staging slot (round robin)
     int *flag = nullptr;
     cudaStream_t stream = nullptr;
     cudaStream_t side = nullptr;                // plan-owned stream: the moment stage (HBM bound) runs beside the

@@ -330,6 +330,28 @@ def test_run_host_end_to_end(cuda_device):
     plan.close()
 
 
+def test_run_host_async_pipeline(cuda_device):
+    """Three different pairs submitted back to back through sfft_run_host_async (two staging slots, copy streams):
+    every result equals the one-call-at-a-time result of that pair."""
+    import torch
+    ps = [synth.make_pair(1, seed=900 + i) for i in range(3)]
+    plan = B.Plan(ps[0].H, ps[0].W, ps[0].L, ps[0].DK, ps[0].DB, ps[0].basis)
+    ref = [plan.run_host(p.R, p.S) for p in ps]
+    hR = [torch.from_numpy(p.R).pin_memory() for p in ps]
+    hS = [torch.from_numpy(p.S).pin_memory() for p in ps]
+    hD = [torch.empty_like(x).pin_memory() for x in hR]
+    hC = [torch.empty((1, plan.n), dtype=torch.float64).pin_memory() for _ in ps]
+    for i in range(3):
+        assert B.sfft_run_host_async(plan.h, hR[i].data_ptr(), hS[i].data_ptr(), hD[i].data_ptr(), hC[i].data_ptr()) == B.SFFT_OK
+    assert B.sfft_run_host_wait(plan.h) == B.SFFT_OK
+    for i in range(3):
+        assert np.array_equal(hD[i].numpy(), ref[i][0])
+        assert np.array_equal(hC[i].numpy(), ref[i][1])
+    _, _, co, Do = _oracle_all(ps[2].R, ps[2].S, ps[2].L, ps[2].basis, ps[2].DK, ps[2].DB)
+    assert np.max(np.abs(hD[2].numpy() - Do)) <= TOL_D * ps[2].sigma
+    plan.close()
+
+
 def test_rank_deficient_input_reports_not_spd(cuda_device):
     """DESIGN g11: a constant reference makes the shifted-difference columns vanish -> M singular."""
     import torch
