@@ -137,7 +137,7 @@ cudaError_t launch_fwd(sfft_plan *p, const double *dR, const double *dS) {
 template <int NH>
 __global__ void __launch_bounds__(FftCfg<NH>::T * (FftCfg<NH>::T >= 128 ? 1 : 128 / FftCfg<NH>::T))
 k_rowfft_forward16(const double *__restrict__ R, const double *__restrict__ S, const double *__restrict__ gK,
-                   const double2 *__restrict__ twW, double2 *__restrict__ rhat, int H, int nKa) {
+                   const double2 *__restrict__ twW, double2 *__restrict__ rhat, int H, int nKa, int poly) {
     using C = FftCfg<NH>;
     constexpr int T = C::T, RPC = T >= 128 ? 1 : 128 / T, W = 2 * NH;
     extern __shared__ double2 sm2[];
@@ -148,7 +148,22 @@ k_rowfft_forward16(const double *__restrict__ R, const double *__restrict__ S, c
     double2 v[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) v[r] = __ldg(&src[tid + r * T]);          // z[n] = a[2n] + i a[2n+1]
-    if (img < nKa) {
+    if (img < nKa && poly) {
+        // g_j(y) = u_y^j with u_y = (2y+1)/W - 1 exact in double: no table traffic (the kernel is bound by the
+        // L1/shared data pipe); j = 0 needs no multiplication at all
+        if (img > 0) {
+            constexpr double invW = 1.0 / W;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const int nn = tid + r * T;
+                const double u0 = (double)(4 * nn + 1) * invW - 1.0, u1 = (double)(4 * nn + 3) * invW - 1.0;
+                double w0 = u0, w1 = u1;
+                for (int j = 1; j < img; ++j) { w0 *= u0; w1 *= u1; }
+                v[r].x *= w0;
+                v[r].y *= w1;
+            }
+        }
+    } else if (img < nKa) {
         const double2 *g = reinterpret_cast<const double2 *>(gK + (size_t)img * W);
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
@@ -185,7 +200,8 @@ cudaError_t launch_fwd16(sfft_plan *p, const double *dR, const double *dS) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid(dS ? p->nimg : p->nKa, p->H / RPC, p->nbatch);
-    kern<<<grid, dim3(T, RPC), smem, p->stream>>>(dR, dS, p->dt.gK, p->dt.twW, p->rhat, p->H, p->nKa);
+    kern<<<grid, dim3(T, RPC), smem, p->stream>>>(dR, dS, p->dt.gK, p->dt.twW, p->rhat, p->H, p->nKa,
+                                                  p->basis == SFFT_BASIS_POLY);
     p->launches++;
     return cudaGetLastError();
 }
