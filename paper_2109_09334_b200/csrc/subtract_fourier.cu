@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(FftCfg<NH>::T * (FftCfg<NH>::T >= 128 ? 1 : 12
 k_rowfft_inverse_sub(const double2 *__restrict__ mhat, const double *__restrict__ S, double *__restrict__ D,
                      const double *__restrict__ coef, const double *__restrict__ xwt, const double *__restrict__ gB,
                      const int *__restrict__ bti, const int *__restrict__ btj, const double2 *__restrict__ twW,
-                     int H, int nimg, int nKa, int nBa, int FB, int n) {
+                     int H, int nimg, int nKa, int nBa, int FB, int n, int poly) {
     using C = FftCfg<NH>;
     constexpr int T = C::T, RPC = T >= 128 ? 1 : 128 / T, W = 2 * NH;
     extern __shared__ double2 sm2[];
@@ -215,11 +215,21 @@ k_rowfft_inverse_sub(const double2 *__restrict__ mhat, const double *__restrict_
         const int nn = tid + r * T;
         const double2 zz = buf[nn], sv = Sr[nn];
         double b0 = 0.0, b1 = 0.0;
-        for (int j = 0; j < nBa; ++j) {
-            const double2 g = __ldg(reinterpret_cast<const double2 *>(gB + (size_t)j * W) + nn);
-            const double c = cj[threadIdx.y][j];
-            b0 = fma(c, g.x, b0);
-            b1 = fma(c, g.y, b1);
+        if (poly) {      // g'_j(y) = u_y^j, u_y = (2y+1)/W - 1 exact: Horner in registers instead of nBa table reads
+            constexpr double invW = 1.0 / W;
+            const double u0 = (double)(4 * nn + 1) * invW - 1.0, u1 = (double)(4 * nn + 3) * invW - 1.0;
+            for (int j = nBa - 1; j >= 0; --j) {
+                const double c = cj[threadIdx.y][j];
+                b0 = fma(b0, u0, c);
+                b1 = fma(b1, u1, c);
+            }
+        } else {
+            for (int j = 0; j < nBa; ++j) {
+                const double2 g = __ldg(reinterpret_cast<const double2 *>(gB + (size_t)j * W) + nn);
+                const double c = cj[threadIdx.y][j];
+                b0 = fma(c, g.x, b0);
+                b1 = fma(c, g.y, b1);
+            }
         }
         Dr[nn] = make_double2(sv.x - zz.x * inv - b0, sv.y + zz.y * inv - b1);
     }
@@ -235,7 +245,7 @@ cudaError_t launch_inv(sfft_plan *p, const double *d_coef, const double *dS, dou
     if (e != cudaSuccess) return e;
     kern<<<dim3(p->H / RPC, p->nbatch), dim3(T, RPC), smem, p->stream>>>(
         p->rhat + (size_t)p->nKa * p->H * p->Nh, dS, dD, d_coef, p->dt.xwt, p->dt.gB, p->dt.bti, p->dt.btj, p->dt.twW,
-        p->H, p->nimg, p->nKa, p->nBa, p->FB, p->n);
+        p->H, p->nimg, p->nKa, p->nBa, p->FB, p->n, p->basis == SFFT_BASIS_POLY);
     p->launches++;
     return cudaGetLastError();
 }
