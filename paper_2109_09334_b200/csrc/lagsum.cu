@@ -17,11 +17,12 @@ namespace {
 
 template <int LP>
 __global__ void __launch_bounds__(128) k_lagsum_partial(const double2 *__restrict__ G, const double2 *__restrict__ lagtw,
-                                                        double *__restrict__ part, int Nh, int L, int E, int Sx, int nch) {
+                                                        double *__restrict__ part, int Nh, int L, int E, int Sx, int nch,
+                                                        int chunk) {
     __shared__ double2 tw[kLagChunk][LP];
     const int e = blockIdx.x * 128 + threadIdx.x, ch = blockIdx.y, bz = blockIdx.z;
-    const int mbeg = ch * kLagChunk, mcnt = min(kLagChunk, Nh + 1 - mbeg);
-    for (int i = threadIdx.x; i < kLagChunk * LP; i += 128) {
+    const int mbeg = ch * chunk, mcnt = min(chunk, Nh + 1 - mbeg);      // chunk <= kLagChunk, a multiple of 8
+    for (int i = threadIdx.x; i < chunk * LP; i += 128) {
         const int mm = i / LP, k = i % LP;
         tw[mm][k] = (mm < mcnt && k < L) ? __ldg(&lagtw[(size_t)(mbeg + mm) * L + k]) : make_double2(0.0, 0.0);
     }
@@ -82,7 +83,8 @@ __global__ void k_lagsum_final(const double *__restrict__ part, const LagUnit *_
 template <int LP>
 cudaError_t launch_partial(sfft_plan *p) {
     dim3 grid((p->E + 127) / 128, p->nch, p->nbatch);
-    k_lagsum_partial<LP><<<grid, 128, 0, p->stream>>>(p->G, p->dt.lagtw, p->lagpart, p->Nh, p->L, p->E, p->Sx, p->nch);
+    k_lagsum_partial<LP><<<grid, 128, 0, p->stream>>>(p->G, p->dt.lagtw, p->lagpart, p->Nh, p->L, p->E, p->Sx, p->nch,
+                                                     p->lagchunk);
     p->launches++;
     return cudaGetLastError();
 }

@@ -97,6 +97,11 @@ void choose_split(sfft_plan *p) {
         double cost = ceil(T / slots) / sx * (1.0 + 0.02 * sx);     // mild penalty: G traffic grows with sx
         if (cost < best) { best = cost; p->Sx = sx; }
     }
+    // column chunks of the y-direction partial sums (lagsum.cu): enough CTAs to fill the machine
+    p->lagchunk = kLagChunk;
+    while (p->lagchunk > 8 && (long)((p->E + 127) / 128) * ((p->Nh + p->lagchunk) / p->lagchunk) * p->nbatch < 2 * 148)
+        p->lagchunk /= 2;
+    p->nch = (p->Nh + 1 + p->lagchunk - 1) / p->lagchunk;
     // y-range splits of the first moment GEMM (moments.cu): enough CTAs to fill the machine
     const long tiles = (long)((p->H + 63) / 64) * ((p->NC + 63) / 64) * p->nbatch;
     p->ksq = 1;
@@ -213,7 +218,6 @@ void build_jobs(sfft_plan *p, const std::vector<double> &fK) {
         }
     p->NC = p->nKa * p->nBa * L;
     choose_split(p);
-    p->nch = (p->Nh + 1 + kLagChunk - 1) / kLagChunk;
     p->ksplit = std::max(1, std::min(32, p->H / 64));
 }
 

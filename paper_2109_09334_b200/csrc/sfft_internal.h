@@ -76,6 +76,7 @@ struct sfft_plan {
     int E = 0;           // G entries per spectrum column: nseq*nseq*L
     int Sx = 1;          // x-range splits of the correlation kernel (partial sums added by lagsum)
     int nlb = 0;         // 8-lag blocks: ceil((L-1)/8)
+    int lagchunk = sfft::kLagChunk;   // spectrum columns per partial sum (8, 16 or 32: enough CTAs to fill the machine)
     int nch = 0;         // column chunks of the lagsum partials
     int NC = 0;          // nKa*nBa*L columns of the moment GEMMs
     int ksplit = 1;      // K (x-range) splits of the second moment GEMM
