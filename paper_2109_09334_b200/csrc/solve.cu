@@ -14,6 +14,10 @@
 //           panel k-1 on the FP64 tensor cores (mma.sync.m8n8k4.f64: a dense contraction).
 //      P(k) needs only panel k-1 and the U updates of launch k-1, so the latency-bound panel
 //      chain (factor + triangular solve) overlaps the throughput-bound trailing update.
+//      Throughput regime (many trailing tiles: batches, n in the thousands): three launches per panel
+//      instead - one factoring CTA per system (k_chol_step with a single slab), lean slab CTAs that read
+//      W from global memory (k_chol_slab), and the trailing update by segments of tile rows with a
+//      cp.async double buffer and register-prefetched C tiles (k_chol_update_row).
 //   3. Backward substitution L^T y = z by a thread-block cluster of 8 CTAs per system: the owner
 //      of diagonal block b forms y_b = W_b^T z_b (W_b = L_bb^-1 from the factorisation), broadcasts it
 //      through distributed shared memory, and every CTA updates the columns it owns.  c = D y.
@@ -334,16 +338,6 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
     if (bx < ntiles) chol_update_tile(L, ldl, n, j1, jp0, bx, T0, T1);
 }
 
-// The trailing update alone (U CTAs of launch k), for batched / large systems where it is throughput bound:
-// without the panel code this kernel needs half the registers, so three CTAs share an SM and one CTA's tile
-// loads overlap another's MMAs.  grid.x = ntiles, grid.y = batch.
-__global__ void __launch_bounds__(256, 3) k_chol_update(double *__restrict__ Lf, int n, int ldl, int k) {
-    extern __shared__ double sm[];
-    double *L = Lf + (size_t)blockIdx.y * (n + 1) * ldl;
-    const int j0 = k * NB, nb = min(NB, n - j0);
-    chol_update_tile(L, ldl, n, j0 + nb, j0 - NB, blockIdx.x, sm, sm + NB * LDT);
-}
-
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
     const unsigned a = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(a), "l"(gmem));
@@ -363,7 +357,14 @@ __device__ __forceinline__ void tile_fetch_async(double *T, const double *L, int
 // Trailing update, throughput regime: one CTA per tile ROW ti of the lower triangle right of strip k.  The row's
 // own panel rows stay in shared memory; the column operands A_tj stream through a double buffer (cp.async) and
 // the C tile is fetched into registers before the MMAs, so loads of tile tj+1 overlap the MMAs of tile tj.
-// grid.x = nslab (row nslab-1-blockIdx.x: long rows first), grid.y = batch.
+// Rows are cut into segments of kRowSeg tiles so that work units are balanced; grid.x = number of segments
+// (long rows first), grid.y = batch.
+constexpr int kRowSeg = 16;
+__host__ __device__ inline int row_segments(int nslab) {
+    int s = 0;
+    for (int ti = 0; ti < nslab; ++ti) s += (ti + kRowSeg) / kRowSeg;
+    return s;
+}
 __global__ void __launch_bounds__(256, 2) k_chol_update_row(double *__restrict__ Lf, int n, int ldl, int k, int nslab) {
     extern __shared__ double sm[];
     double *Ti = sm, *Tj0 = sm + NB * LDT, *Tj1 = sm + 2 * NB * LDT;
@@ -371,16 +372,24 @@ __global__ void __launch_bounds__(256, 2) k_chol_update_row(double *__restrict__
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int r8 = lane >> 2, kq = lane & 3, wm = (warp >> 1) * 16, wn = (warp & 1) * 32;
     const int j0 = k * NB, nb = min(NB, n - j0), j1 = j0 + nb, jp0 = j0 - NB;
-    const int ti = nslab - 1 - blockIdx.x, i0 = j1 + ti * NB;
+    int ti = nslab - 1, seg = blockIdx.x;
+    for (;;) {
+        const int ns = (ti + kRowSeg) / kRowSeg;
+        if (seg < ns) break;
+        seg -= ns;
+        --ti;
+    }
+    const int i0 = j1 + ti * NB, tj0 = seg * kRowSeg, tj1 = min(ti, tj0 + kRowSeg - 1);     // tiles tj0..tj1 of row ti
     const int nri = max(0, min(NB, n + 1 - i0));
     if (nri <= 0) return;
     tile_fetch_async(Ti, L, ldl, i0, jp0, nri);
-    if (ti > 0) tile_fetch_async(Tj0, L, ldl, j1, jp0, min(NB, n - j1));
-    for (int tj = 0; tj <= ti; ++tj) {
+    if (tj0 < ti) tile_fetch_async((tj0 & 1) ? Tj1 : Tj0, L, ldl, j1 + tj0 * NB, jp0, max(0, min(NB, n - (j1 + tj0 * NB))));
+    for (int tj = tj0; tj <= tj1; ++tj) {
         const int c0 = j1 + tj * NB;
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();                 // tile tj (and Ti) visible; MMAs of tile tj-1 done by every warp
-        if (tj + 1 < ti) tile_fetch_async((tj & 1) ? Tj0 : Tj1, L, ldl, c0 + NB, jp0, max(0, min(NB, n - (c0 + NB))));
+        if (tj + 1 <= tj1 && tj + 1 < ti)
+            tile_fetch_async((tj & 1) ? Tj0 : Tj1, L, ldl, c0 + NB, jp0, max(0, min(NB, n - (c0 + NB))));
         // C tile into registers ahead of the MMAs
         double2 cv[2][4];
 #pragma unroll
@@ -561,7 +570,6 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     k_scale_copy<<<dim3((n + 127) / 128, n + 1, nbat), 128, 0, p->stream>>>(p->M, p->rhs, p->dscale, p->Lf, n, ldl);
     p->launches += 2;
     cudaError_t e = cudaFuncSetAttribute(k_chol_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStepSmem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUpdSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_update_row, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_slab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUpdSmem);
     if (e != cudaSuccess) return e;
@@ -577,9 +585,8 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
                 k_chol_slab<<<dim3(nslab - 1, nbat), 256, kUpdSmem, p->stream>>>(p->Lf, p->Winv, n, ldl, k, nblk);
                 p->launches++;
             }
-            // many systems: one CTA per tile row (operand reuse + software pipelining); few: one CTA per tile
-            if ((long)nslab * nbat >= 2048) k_chol_update_row<<<dim3(nslab, nbat), 256, kRowSmem, p->stream>>>(p->Lf, n, ldl, k, nslab);
-            else k_chol_update<<<dim3(ntiles, nbat), 256, kUpdSmem, p->stream>>>(p->Lf, n, ldl, k);
+            // one CTA per segment of a tile row (operand reuse + software pipelining)
+            k_chol_update_row<<<dim3(row_segments(nslab), nbat), 256, kRowSmem, p->stream>>>(p->Lf, n, ldl, k, nslab);
             p->launches += 2;
         } else {
             k_chol_step<<<dim3(nslab + ntiles, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, nslab,
