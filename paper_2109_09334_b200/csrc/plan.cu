@@ -325,8 +325,10 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
         }
     // moment-GEMM operands (moments.cu): products of a kernel and a shifted background basis function
     const int wl = p->w;
-    std::vector<double> cy((size_t)p->NC * W), fx((size_t)p->NC * H);
-    for (int jb = 0; jb < p->nKa; ++jb)
+    // (cy is the operand of the first moment contraction, used by the B-spline path only: the polynomial path
+    // replaces that contraction by row power moments, tables cq / cwr below)
+    std::vector<double> cy(basis == SFFT_BASIS_POLY ? 0 : (size_t)p->NC * W), fx((size_t)p->NC * H);
+    for (int jb = 0; jb < p->nKa && basis != SFFT_BASIS_POLY; ++jb)
         for (int j = 0; j < p->nBa; ++j)
             for (int b = 0; b < L; ++b) {
                 double *row = &cy[((size_t)(jb * p->nBa + j) * L + b) * W];

@@ -156,11 +156,9 @@ __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double
                 for (int bb = 0; bb < 4; ++bb) rb[tx + 16 * bb] = e[b][bb];
             }
             __syncthreads();
-            double piv = cb[k];
-            if (!(piv > 0.0)) {
-                if (store && tid == 0) atomicCAS(flag, -1, gidx0 + k);
-                piv = 1.0;
-            }
+            // the pivot test is taken off the per-column chain: pivots are recorded and checked once after the
+            // loop (a non-positive pivot makes everything after it garbage, which is reported, not used)
+            const double piv = cb[k];
             if (tid == 0) pivs[k] = piv;
             const double inv = fast_rcp(piv);
             // only the lower sub-blocks (a >= bb >= b) are ever read: the step is bound by FP64 issue
@@ -186,6 +184,13 @@ __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double
         }
     }
     __syncthreads();       // Dg fully consumed (registers), pivs complete
+    if (store && tid < nb && !(pivs[tid] > 0.0)) {
+        // first failing column of this block: the lowest index wins; an earlier block's failure (already in
+        // the flag from a previous launch) is kept by the compare-and-swap on -1 only
+        bool first = true;
+        for (int q = 0; q < tid; ++q) first = first && (pivs[q] > 0.0);
+        if (first) atomicCAS(flag, -1, gidx0 + tid);
+    }
     if (tid < NB) rs[tid] = (tid < nb) ? rsqrt(pivs[tid]) : 1.0;
     __syncthreads();
 #pragma unroll
