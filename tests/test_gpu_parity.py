@@ -381,4 +381,12 @@ def test_argument_and_state_errors(cuda_device):
     assert B.sfft_plan_set_workspace(h, ptr, B.sfft_plan_workspace_bytes(h)) == B.SFFT_OK
     assert B.sfft_solve(h, x.data_ptr()) == B.SFFT_ERR_STATE
     assert B.sfft_build_system(h, 0, x.data_ptr()) == B.SFFT_ERR_INVALID_ARG
+    assert B.sfft_plan_set_const_phot_ratio(h, 2) == B.SFFT_ERR_INVALID_ARG
+    assert B.sfft_plan_set_const_phot_ratio(h, 1) == B.SFFT_OK and B.sfft_plan_num_solved(h) == 148
+    assert B.sfft_plan_num_unknowns(h) == 150                      # coefficient vectors keep the full layout
+    assert B.sfft_plan_set_const_phot_ratio(h, 0) == B.SFFT_OK and B.sfft_plan_num_solved(h) == 150
+    assert B.sfft_run_host_async(h, 0, x.data_ptr(), 0, 0) == B.SFFT_ERR_INVALID_ARG
+    st2, h2 = B.sfft_plan_create(128, 128, 7, 1, 1, 0)
+    assert B.sfft_run_host_async(h2, x.data_ptr(), x.data_ptr(), 0, 0) == B.SFFT_ERR_WORKSPACE
+    B.sfft_plan_destroy(h2)
     B.sfft_plan_destroy(h)
