@@ -4,6 +4,7 @@ library routines (scipy.ndimage wrap-convolution, numpy lstsq, scipy BSpline), e
 rational arithmetic, and recovery of injected parameters.  CPU only.
 Each test names the plausible mistake it would catch.
 """
+import os
 from fractions import Fraction
 
 import numpy as np
@@ -41,8 +42,12 @@ def _rand_pair(H, W, seed):
 def test_term_order_and_counts():
     # i in [0,D], j in [0,D-i]  -> (D+1)(D+2)/2 terms; BASELINE unknown counts
     assert oracle.terms(POLY, 2) == [(0, 0), (0, 1), (0, 2), (1, 0), (1, 1), (2, 0)]
-    for L, DK, DB, n in [(7, 1, 1, 150), (11, 2, 2, 732), (15, 2, 2, 1356), (17, 2, 2, 1740)]:
+    golden = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "unknown_counts.txt")
+    rows = [tuple(int(v) for v in ln.split()) for ln in open(golden) if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 4
+    for L, DK, DB, n in rows:
         assert oracle.num_unknowns(L, POLY, DK, DB) == n
+        assert oracle.cpr_num_unknowns(L, POLY, DK, DB) == n - ((DK + 1) * (DK + 2) // 2 - 1)
     assert oracle.num_unknowns(11, BSPL, 4, 4) == 7808   # DESIGN g13: 8x8 functions
     assert oracle.terms(BSPL, 4)[9] == (1, 1)
 
