@@ -257,6 +257,10 @@ constexpr size_t kRowSmem = (size_t)(3 * NB * LDT) * sizeof(double);
 // One launch per panel k (see the header).  grid.x = nslab P CTAs, then ntiles U CTAs (k >= 1).
 __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, double *__restrict__ Winv, int *flag, int n,
                                                    int ldl, int k, int nslab, int ntiles, int nblk) {
+    // programmatic dependent launch: this grid may be scheduled while the previous panel's grid drains; nothing
+    // of the previous grid is read before the wait, and the next grid may be scheduled from here on
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;");
     extern __shared__ double sm[];
     double *T0 = sm, *T1 = sm + NB * LDT;                   // MMA operand tiles; later the factor / slab views
     double *colbuf = sm + 2 * NB * LDT, *rowbuf = colbuf + 2 * NB, *pivs = rowbuf + 2 * NB, *rs = pivs + NB;
@@ -594,8 +598,15 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
             k_chol_update_row<<<dim3(row_segments(nslab), nbat), 256, kRowSmem, p->stream>>>(p->Lf, n, ldl, k, nslab);
             p->launches += 2;
         } else {
-            k_chol_step<<<dim3(nslab + ntiles, nbat), 256, kStepSmem, p->stream>>>(p->Lf, p->Winv, p->flag, n, ldl, k, nslab,
-                                                                                   ntiles, nblk);
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(nslab + ntiles, nbat); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = kStepSmem;
+            cfg.stream = p->stream;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            at[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            e = cudaLaunchKernelEx(&cfg, k_chol_step, p->Lf, p->Winv, p->flag, n, ldl, k, nslab, ntiles, nblk);
+            if (e != cudaSuccess) return e;
             p->launches++;
         }
     }
