@@ -143,6 +143,7 @@ __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double
         }
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
+#pragma unroll
         for (int kk = 0; kk < 16; ++kk) {
             const int k = 16 * b + kk;
             if (k >= nb) break;                              // uniform
