@@ -150,11 +150,11 @@ __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double
             double *cb = colbuf + (k & 1) * NB, *rb = rowbuf + (k & 1) * NB;
             if (tx == kk) {
 #pragma unroll
-                for (int a = 0; a < 4; ++a) cb[ty + 16 * a] = t[a][b];
+                for (int a = b; a < 4; ++a) cb[ty + 16 * a] = t[a][b];      // rows above the block are never read
             }
             if (ty == kk) {
 #pragma unroll
-                for (int bb = 0; bb < 4; ++bb) rb[tx + 16 * bb] = e[b][bb];
+                for (int bb = 0; bb <= b; ++bb) rb[tx + 16 * bb] = e[b][bb];  // E is lower triangular
             }
             __syncthreads();
             // the pivot test is taken off the per-column chain: pivots are recorded and checked once after the
