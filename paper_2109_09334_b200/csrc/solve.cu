@@ -120,6 +120,34 @@ __device__ __forceinline__ void mma_64(const double *A, const double *B, double 
     }
 }
 
+// acc += A W^T for a LOWER-TRIANGULAR right operand W (64x64 tiles, stride LDT): column tile ct of the product
+// only needs k < 8 ct + 8, so each warp takes the column tiles {0,3,4,7} (HALF 0) or {1,2,5,6} (HALF 1) - 18 of
+// the 36 live (tile, k-block) pairs each, against 32 for the dense product.  Rows as in mma_64.
+// acc[a][c][q] <-> row 16*(w>>1) + 8a + (lane>>2), col 8*ct(c) + 2*(lane&3) + q
+template <int HALF>
+__device__ __forceinline__ int lower_tile(int c) { return HALF == 0 ? (c == 0 ? 0 : c == 1 ? 3 : c == 2 ? 4 : 7) : (c == 0 ? 1 : c == 1 ? 2 : c == 2 ? 5 : 6); }
+template <int HALF>
+__device__ __forceinline__ void mma_64_lowerB(const double *A, const double *W, double (&acc)[2][4][2]) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, r = lane >> 2, kq = lane & 3;
+    const double *ap = A + ((warp >> 1) * 16 + r) * LDT + kq;
+    const double *bp = W + r * LDT + kq;
+#pragma unroll
+    for (int k = 0; k < NB; k += 4) {
+        double af[2];
+#pragma unroll
+        for (int a = 0; a < 2; ++a) af[a] = ap[a * 8 * LDT + k];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int ct = lower_tile<HALF>(c);
+            if (k < 8 * ct + 8) {                    // compile-time after unrolling
+                const double bf = bp[ct * 8 * LDT + k];
+#pragma unroll
+                for (int a = 0; a < 2; ++a) dmma884(acc[a][c], af[a], bf);
+            }
+        }
+    }
+}
+
 // In-place Cholesky of the 64x64 block Dg (shared memory, stride LDX, lower triangle valid, identity
 // padded beyond nb) by all 256 threads, together with the inverse of its factor: the elimination is
 // run on the augmented block [A | I], which turns I into W = L^-1.  Every thread keeps 4x4 register
@@ -330,12 +358,13 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
         for (int a = 0; a < 2; ++a)
 #pragma unroll
             for (int c = 0; c < 4; ++c) accX[a][c][0] = accX[a][c][1] = 0.0;
-        mma_64(St, T0, accX);
+        if (warp & 1) mma_64_lowerB<1>(St, T0, accX); else mma_64_lowerB<0>(St, T0, accX);
 #pragma unroll
         for (int a = 0; a < 2; ++a)
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq;
+                const int ct = (warp & 1) ? lower_tile<1>(c) : lower_tile<0>(c);
+                const int r = wm + 8 * a + r8, cc = 8 * ct + 2 * kq;
                 if (r >= nr) continue;
                 double *dst = &L[(size_t)(r0 + r) * ldl + j0 + cc];
                 if (cc + 1 < nb) *reinterpret_cast<double2 *>(dst) = make_double2(accX[a][c][0], accX[a][c][1]);
@@ -486,12 +515,13 @@ __global__ void __launch_bounds__(256, 2) k_chol_slab(double *__restrict__ Lf, c
         }
     }
     __syncthreads();
-    mma_64(T1, T0, acc);
+    if (warp & 1) mma_64_lowerB<1>(T1, T0, acc); else mma_64_lowerB<0>(T1, T0, acc);
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
-            const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq;
+            const int ct = (warp & 1) ? lower_tile<1>(c) : lower_tile<0>(c);
+            const int r = wm + 8 * a + r8, cc = 8 * ct + 2 * kq;
             if (r >= nr) continue;
             double *dst = &L[(size_t)(r0 + r) * ldl + j0 + cc];
             if (cc + 1 < nb) *reinterpret_cast<double2 *>(dst) = make_double2(acc[a][c][0], acc[a][c][1]);
