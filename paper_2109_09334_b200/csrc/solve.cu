@@ -148,6 +148,40 @@ __device__ __forceinline__ void mma_64_lowerB(const double *A, const double *W, 
     }
 }
 
+// acc += A A^T restricted to the lower triangle (tile granularity 8): warp (RB, HALF) owns the row tiles {RB, 7-RB}
+// and the column tiles of lower_tile<HALF>, so every warp carries 4 or 5 live tiles of the 36 (8 for the dense
+// product).  acc[a][c][q] <-> row 8*rt(a) + (lane>>2), col 8*ct(c) + 2*(lane&3) + q, rt(0) = RB, rt(1) = 7 - RB.
+template <int RB, int HALF>
+__device__ __forceinline__ void mma_64_symlower(const double *A, double (&acc)[2][4][2]) {
+    const int lane = threadIdx.x & 31, r = lane >> 2, kq = lane & 3;
+    const double *ap = A + r * LDT + kq;
+#pragma unroll 4
+    for (int k = 0; k < NB; k += 4) {
+        const double a0 = ap[RB * 8 * LDT + k], a1 = ap[(7 - RB) * 8 * LDT + k];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int ct = lower_tile<HALF>(c);
+            if (ct <= 7 - RB) {                       // compile-time
+                const double bf = ap[ct * 8 * LDT + k];
+                if (ct <= RB) dmma884(acc[0][c], a0, bf);
+                dmma884(acc[1][c], a1, bf);
+            }
+        }
+    }
+}
+__device__ __forceinline__ void mma_64_symlower_dispatch(const double *A, double (&acc)[2][4][2]) {
+    switch (threadIdx.x >> 5) {          // warp-uniform
+        case 0: mma_64_symlower<0, 0>(A, acc); break;
+        case 1: mma_64_symlower<0, 1>(A, acc); break;
+        case 2: mma_64_symlower<1, 0>(A, acc); break;
+        case 3: mma_64_symlower<1, 1>(A, acc); break;
+        case 4: mma_64_symlower<2, 0>(A, acc); break;
+        case 5: mma_64_symlower<2, 1>(A, acc); break;
+        case 6: mma_64_symlower<3, 0>(A, acc); break;
+        default: mma_64_symlower<3, 1>(A, acc); break;
+    }
+}
+
 // In-place Cholesky of the 64x64 block Dg (shared memory, stride LDX, lower triangle valid, identity
 // padded beyond nb) by all 256 threads, together with the inverse of its factor: the elimination is
 // run on the augmented block [A | I], which turns I into W = L^-1.  Every thread keeps 4x4 register
@@ -317,7 +351,10 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
                     const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq + q;
-                    dv[a][c][q] = (r < nb && cc <= r) ? L[(size_t)(j0 + r) * ldl + j0 + cc] : ((r == cc) ? 1.0 : 0.0);
+                    // diagonal block in the layout of mma_64_symlower (row tiles {rb, 7-rb}, interleaved column tiles)
+                    const int rd = 8 * (a == 0 ? (warp >> 1) : 7 - (warp >> 1)) + r8;
+                    const int cd = 8 * ((warp & 1) ? lower_tile<1>(c) : lower_tile<0>(c)) + 2 * kq + q;
+                    dv[a][c][q] = (rd < nb && cd <= rd) ? L[(size_t)(j0 + rd) * ldl + j0 + cd] : ((rd == cd) ? 1.0 : 0.0);
                     xv[a][c][q] = (r < nr && cc < nb) ? L[(size_t)(r0 + r) * ldl + j0 + cc] : 0.0;
                 }
         if (k > 0) {
@@ -328,7 +365,7 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
             tile_store(T1, ts);
             __syncthreads();
             PROBE(k, 5);
-            mma_64(T0, T0, accD);
+            mma_64_symlower_dispatch(T0, accD);
             mma_64(T1, T0, accX);
             __syncthreads();
         }
@@ -342,8 +379,10 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
                     const int r = wm + 8 * a + r8, cc = wn + 8 * c + 2 * kq + q;
-                    const bool dl = (r < nb && cc <= r), xl = (r < nr && cc < nb);
-                    Dg[r * LDX + cc] = dl ? dv[a][c][q] - accD[a][c][q] : dv[a][c][q];
+                    const int rd = 8 * (a == 0 ? (warp >> 1) : 7 - (warp >> 1)) + r8;
+                    const int cd = 8 * ((warp & 1) ? lower_tile<1>(c) : lower_tile<0>(c)) + 2 * kq + q;
+                    const bool dl = (rd < nb && cd <= rd), xl = (r < nr && cc < nb);
+                    Dg[rd * LDX + cd] = dl ? dv[a][c][q] - accD[a][c][q] : dv[a][c][q];
                     St[r * LDT + cc] = xl ? xv[a][c][q] - accX[a][c][q] : 0.0;
                 }
         __syncthreads();
