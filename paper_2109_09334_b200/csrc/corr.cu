@@ -64,7 +64,8 @@ struct CorrCfg {
     static constexpr int ROWS = XT + 8 * NLB;              // staged x-rows per tile (largest lag offset + fragment extent)
     static constexpr int XS = ((ROWS + 7) / 16) * 16 + 8;  // plane stride, = 8 mod 16 (conflict-free staging stores)
     static constexpr int SS = 4 * XS + 4;                  // slot stride [part 2][col 2][XS] + 4 (conflict-free A loads)
-    static constexpr size_t SMEM = (size_t)kCorrSlots * SS * sizeof(double);
+    // operand planes + the raw cp.async staging buffer of one tile (16 bytes per item)
+    static constexpr size_t SMEM = (size_t)kCorrSlots * SS * sizeof(double) + (size_t)kCorrSlots * ROWS * kCorrCols * sizeof(double2);
 };
 
 // grid: x = column pair, y = job * Sx + xs, z = batch.  block: 256.
@@ -109,39 +110,70 @@ k_corr_mma(const double2 *__restrict__ rhat, const double *__restrict__ xwt, con
         for (int pt = 0; pt < 2; ++pt) acc[i][pt][0] = acc[i][pt][1] = 0.0;
 
     const int nitems = job.nstage * ROWS * kCorrCols;
-    for (int rg = 0; rg < job.nrange; ++rg) {
-        // this CTA's part of the range: Sx parts of whole 4-row steps
-        const int rb = job.xbeg[rg], re = job.xend[rg];
-        const int plen = (((re - rb) / 4 + Sx - 1) / Sx) * 4;
-        const int xbeg = rb + xs * plen, xend = min(re, xbeg + plen);
-        for (int x0 = xbeg; x0 < xend; x0 += XT) {
-            __syncthreads();
-            // ---- stage the tile: weighted sequences, split into Re / Im planes, x-contiguous ----
-            for (int i = tid; i < nitems; i += 256) {
-                const int c = i & 1, r = (i >> 1) % ROWS, si = (i >> 1) / ROWS;
-                const int x = (x0 + r) & (H - 1);
-                const Seq sq = sseq[si];
-                double2 v = __ldg(&rhat_b[((size_t)sq.img * H + x) * Nh + m0 + c]);
-                if (sq.xw >= 0) { const double wgt = __ldg(&xwt[(size_t)sq.xw * H + x]); v.x *= wgt; v.y *= wgt; }
-                double *pl = sm + job.stage_slot[si] * SS + c * XS + r;
-                pl[0] = v.x;
-                pl[2 * XS] = v.y;
-            }
-            __syncthreads();
-            // ---- MMAs ----
-            const int kmax = min(XT, xend - x0);
-            switch (nb) {               // warp-uniform
-                case 1: corr_tile_mma<1, XS>(acc, aA, aB, kmax); break;
-                case 2: corr_tile_mma<2, XS>(acc, aA, aB, kmax); break;
-                case 3: corr_tile_mma<3, XS>(acc, aA, aB, kmax); break;
-                case 4: corr_tile_mma<4, XS>(acc, aA, aB, kmax); break;
-                case 5: corr_tile_mma<5, XS>(acc, aA, aB, kmax); break;
-                case 6: corr_tile_mma<6, XS>(acc, aA, aB, kmax); break;
-                case 7: corr_tile_mma<7, XS>(acc, aA, aB, kmax); break;
-                case 8: corr_tile_mma<8, XS>(acc, aA, aB, kmax); break;
-                default: break;
-            }
+    // this CTA's part of each x-range: Sx parts of whole 4-row steps
+    int pb0, pe0, pb1 = 0, pe1 = 0;
+    {
+        const int rb = job.xbeg[0], re = job.xend[0], plen = (((re - rb) / 4 + Sx - 1) / Sx) * 4;
+        pb0 = rb + xs * plen; pe0 = min(re, pb0 + plen);
+        if (job.nrange > 1) {
+            const int rb1 = job.xbeg[1], re1 = job.xend[1], plen1 = (((re1 - rb1) / 4 + Sx - 1) / Sx) * 4;
+            pb1 = rb1 + xs * plen1; pe1 = min(re1, pb1 + plen1);
         }
+    }
+    // tile cursor (range, first row); range 2 = done
+    auto settle = [&](int &r, int &x) {
+        if (r == 0 && x >= pe0) { r = 1; x = pb1; }
+        if (r == 1 && x >= pe1) r = 2;
+    };
+    // The raw spectrum values of a tile are fetched with cp.async into a staging buffer while the MMAs of the
+    // previous tile run (no registers held across the MMA phase); each thread later converts the items it
+    // fetched itself (weight, Re/Im split) into the operand planes.
+    double2 *raw = reinterpret_cast<double2 *>(sm + kCorrSlots * SS);
+    auto prefetch = [&](int x0) {
+        for (int i = tid; i < nitems; i += 256) {
+            const int c = i & 1, r = (i >> 1) % ROWS, si = (i >> 1) / ROWS;
+            const int x = (x0 + r) & (H - 1);
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(&raw[i]);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst),
+                         "l"(&rhat_b[((size_t)sseq[si].img * H + x) * Nh + m0 + c]));
+        }
+        asm volatile("cp.async.commit_group;");
+    };
+    int crg = 0, cx = pb0;
+    settle(crg, cx);
+    __syncthreads();                    // sseq visible
+    if (crg < 2) prefetch(cx);
+    while (crg < 2) {
+        int nrg = crg, nx = cx + XT;
+        settle(nrg, nx);
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                // every warp is done with the planes of the previous tile
+        // ---- stage the tile: weighted sequences, split into Re / Im planes, x-contiguous ----
+        for (int i = tid; i < nitems; i += 256) {
+            const int c = i & 1, r = (i >> 1) % ROWS, si = (i >> 1) / ROWS;
+            const Seq sq = sseq[si];
+            double2 v = raw[i];
+            if (sq.xw >= 0) { const double wgt = __ldg(&xwt[(size_t)sq.xw * H + ((cx + r) & (H - 1))]); v.x *= wgt; v.y *= wgt; }
+            double *pl = sm + job.stage_slot[si] * SS + c * XS + r;
+            pl[0] = v.x;
+            pl[2 * XS] = v.y;
+        }
+        if (nrg < 2) prefetch(nx);      // own slots of the raw buffer only: no barrier needed before reuse
+        __syncthreads();
+        // ---- MMAs ----
+        const int kmax = min(XT, (crg == 0 ? pe0 : pe1) - cx);
+        switch (nb) {               // warp-uniform
+            case 1: corr_tile_mma<1, XS>(acc, aA, aB, kmax); break;
+            case 2: corr_tile_mma<2, XS>(acc, aA, aB, kmax); break;
+            case 3: corr_tile_mma<3, XS>(acc, aA, aB, kmax); break;
+            case 4: corr_tile_mma<4, XS>(acc, aA, aB, kmax); break;
+            case 5: corr_tile_mma<5, XS>(acc, aA, aB, kmax); break;
+            case 6: corr_tile_mma<6, XS>(acc, aA, aB, kmax); break;
+            case 7: corr_tile_mma<7, XS>(acc, aA, aB, kmax); break;
+            case 8: corr_tile_mma<8, XS>(acc, aA, aB, kmax); break;
+            default: break;
+        }
+        crg = nrg; cx = nx;
     }
 
     // ---- epilogue: combine the Re/Im row halves and store G[b][xs][m][e] ----
