@@ -64,8 +64,8 @@ struct CorrCfg {
     static constexpr int ROWS = XT + 8 * NLB;              // staged x-rows per tile (largest lag offset + fragment extent)
     static constexpr int XS = ((ROWS + 7) / 16) * 16 + 8;  // plane stride, = 8 mod 16 (conflict-free staging stores)
     static constexpr int SS = 4 * XS + 4;                  // slot stride [part 2][col 2][XS] + 4 (conflict-free A loads)
-    // operand planes + the raw cp.async staging buffer of one tile (16 bytes per item)
-    static constexpr size_t SMEM = (size_t)kCorrSlots * SS * sizeof(double) + (size_t)kCorrSlots * ROWS * kCorrCols * sizeof(double2);
+    // operand planes + the raw cp.async staging buffers of one tile (value 16 bytes + x-weight 8 bytes per item)
+    static constexpr size_t SMEM = (size_t)kCorrSlots * SS * sizeof(double) + (size_t)kCorrSlots * ROWS * kCorrCols * (sizeof(double2) + sizeof(double));
 };
 
 // grid: x = column pair, y = job * Sx + xs, z = batch.  block: 256.
@@ -129,13 +129,19 @@ k_corr_mma(const double2 *__restrict__ rhat, const double *__restrict__ xwt, con
     // previous tile run (no registers held across the MMA phase); each thread later converts the items it
     // fetched itself (weight, Re/Im split) into the operand planes.
     double2 *raw = reinterpret_cast<double2 *>(sm + kCorrSlots * SS);
+    double *raww = reinterpret_cast<double *>(raw + kCorrSlots * ROWS * kCorrCols);      // x-weight of every item
     auto prefetch = [&](int x0) {
         for (int i = tid; i < nitems; i += 256) {
             const int c = i & 1, r = (i >> 1) % ROWS, si = (i >> 1) / ROWS;
             const int x = (x0 + r) & (H - 1);
+            const Seq sq = sseq[si];
             const unsigned dst = (unsigned)__cvta_generic_to_shared(&raw[i]);
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst),
-                         "l"(&rhat_b[((size_t)sseq[si].img * H + x) * Nh + m0 + c]));
+                         "l"(&rhat_b[((size_t)sq.img * H + x) * Nh + m0 + c]));
+            if (sq.xw >= 0) {
+                const unsigned dw = (unsigned)__cvta_generic_to_shared(&raww[i]);
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dw), "l"(&xwt[(size_t)sq.xw * H + x]));
+            }
         }
         asm volatile("cp.async.commit_group;");
     };
@@ -153,7 +159,7 @@ k_corr_mma(const double2 *__restrict__ rhat, const double *__restrict__ xwt, con
             const int c = i & 1, r = (i >> 1) % ROWS, si = (i >> 1) / ROWS;
             const Seq sq = sseq[si];
             double2 v = raw[i];
-            if (sq.xw >= 0) { const double wgt = __ldg(&xwt[(size_t)sq.xw * H + ((cx + r) & (H - 1))]); v.x *= wgt; v.y *= wgt; }
+            if (sq.xw >= 0) { const double wgt = raww[i]; v.x *= wgt; v.y *= wgt; }
             double *pl = sm + job.stage_slot[si] * SS + c * XS + r;
             pl[0] = v.x;
             pl[2 * XS] = v.y;
