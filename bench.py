@@ -30,8 +30,8 @@ from paper_2109_09334_b200 import synth  # noqa: E402
 METRIC = "difference-image pairs/s at 4096^2 FP64 (build+solve+subtract, L=17, DK=DB=2)"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/clk x 2 flop x 1.965 GHz
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's dominant kernel at config 4, from the
-# `ncu --set full` capture summarised in profiles/r01_d_final_launches_and_ncu_full.md (bytes)
-NCU_TRAFFIC_CFG4 = {"corr": 542.6e6 + 46.2e6, "rowfft": 268.6e6 + 479.8e6, "subtract": 467.8e6 + 112.9e6}
+# `ncu --set full` capture summarised in profiles/r01_f_final.md (bytes)
+NCU_TRAFFIC_CFG4 = {"corr": 545.4e6 + 53.5e6, "rowfft": 268.5e6 + 478.8e6, "subtract": 467.5e6 + 112.4e6}
 
 
 def shard_units(nunits, rank, world):
