@@ -85,7 +85,8 @@ k_corr_mma(const double2 *__restrict__ rhat, const double *__restrict__ xwt, con
     const int m0 = blockIdx.x * kCorrCols;
 
     if (tid < (int)(sizeof(CorrJob) / sizeof(int))) reinterpret_cast<int *>(&job)[tid] = reinterpret_cast<const int *>(&jobs[jb])[tid];
-    for (int i = tid; i < kCorrSlots * SS; i += 256) sm[i] = 0.0;
+    // only the zero plane has to be cleared: every staged plane is rewritten in full (rows < ROWS) for each tile
+    for (int i = tid; i < SS; i += 256) sm[kCorrZero * SS + i] = 0.0;
     __syncthreads();
     if (tid < job.nstage) sseq[tid] = seqs[job.stage_seq[tid]];
 
