@@ -1,18 +1,21 @@
 #!/usr/bin/env python
 """Benchmark of the SFFT hot path (build_system -> solve -> subtract) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C] [--no-compare]
 
 One step = one pass of the whole hot path over one seeded
 synthetic image pair per GPU.  Default workload: BASELINE.json config 4 (4096x4096 FP64 pair,
 17x17 delta-basis kernel, DK=DB=2, 1740 unknowns).  Prints ONE JSON line (contract in the task
 statement): whole-job pairs/s with inputs resident in HBM (`value`), the same through the C ABI's
 host-buffer entry point with the copies inside the timed region (`e2e`), the roofline of the
-dominant kernel, and the CPU oracle timed on a bounded sample (`cpu_baseline`).
-For N > 1 (torchrun) every rank processes its own independent pair (weak scaling, no collective
-in the data path).
+dominant kernel, the CPU oracle timed on the full pair (`cpu_baseline`), and library comparison
+points (cuFFT / cuSOLVER through torch, never linked into libsfft_b200.so) under `comparison`.
+For N > 1 (torchrun): configs 1-4, every rank processes its own independent pair (weak scaling);
+config 5, the 64 sub-fields of the batch are cut into contiguous slices, one per rank (strong
+scaling).  No collective in the data path either way.
 """
 import argparse
+import ctypes
 import json
 import os
 import sys
@@ -25,13 +28,23 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2109_09334_b200 import synth  # noqa: E402
+import synth  # noqa: E402
 
-METRIC = "difference-image pairs/s at 4096^2 FP64 (build+solve+subtract, L=17, DK=DB=2)"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/clk x 2 flop x 1.965 GHz
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's dominant kernel at config 4, from the
-# `ncu --set full` capture summarised in profiles/r01_f_final.md (bytes)
-NCU_TRAFFIC_CFG4 = {"corr": 545.4e6 + 53.5e6, "rowfft": 268.5e6 + 478.8e6, "subtract": 467.5e6 + 112.4e6}
+# committed `ncu --set full` capture named in NCU_TRAFFIC_SOURCE (bytes).  Not measured by this run: the line
+# carries the source beside the number.
+NCU_TRAFFIC_CFG4 = {"rowfft": 268.5e6 + 478.8e6, "subtract": 467.5e6 + 112.4e6}
+NCU_TRAFFIC_SOURCE = {"rowfft": "profiles/r01_f_final.md (round-1 kernel)",
+                      "subtract": "profiles/r01_f_final.md (k_fir_x, round-1 kernel)"}
+REFERENCE_BUDGET_S = 200.0      # wall-clock cap of the --impl reference arm (the oracle is slow by construction)
+
+
+def metric_name(cfg_index):
+    c = synth.CONFIGS[cfg_index]
+    size = f"{c['H']}x{c['W']}" if c["H"] != c["W"] else f"{c['H']}^2"
+    what = "difference-image pairs/s" if c["batch"] == 1 else f"sub-field pairs/s (batch of {c['batch']} per call)"
+    return f"{what} at {size} FP64 (build+solve+subtract, L={c['L']}, {c['basis']} DK={c['DK']} DB={c['DB']})"
 
 
 def shard_units(nunits, rank, world):
@@ -39,6 +52,16 @@ def shard_units(nunits, rank, world):
     base, rem = divmod(nunits, world)
     lo = rank * base + min(rank, rem)
     return lo, lo + base + (1 if rank < rem else 0)
+
+
+def rank_units(cfg_index, rank, world):
+    """Units (pairs / sub-fields) rank `rank` of `world` processes per step, as (first, count, scaling):
+    a single-pair config gives every rank its own pair (weak); the config-5 batch is sliced (strong)."""
+    nb = synth.CONFIGS[cfg_index]["batch"]
+    if nb == 1:
+        return rank, 1, "weak"
+    lo, hi = shard_units(nb, rank, world)
+    return lo, hi - lo, "strong"
 
 
 def workload_name(cfg_index):
@@ -99,15 +122,28 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.sm)}
 
 
-def oracle_sample(cfg_index, pair, crop=1024):
-    """The oracle as it stands on a bounded sample of the workload: lag tables + difference on a
-    crop x crop corner (cost is linear in pixels -> scaled to the full frame) plus the full-size solve
-    of that crop's system (n is the full n).  Returns (seconds per full pair, description, cores)."""
+def oracle_pass(cfg_index, pair, crop=None):
+    """One pass of the oracle as it stands (direct pixel sums, no FFT: normal system, solve, full difference image).
+    crop = None: the FULL pair (single-pair configs) -- a measurement, not an extrapolation.  crop = c: a c x c corner,
+    its pixel-proportional parts scaled to the full frame plus the full-n solve (labelled fallback for the
+    batch-of-64 config, whose full oracle pass takes hours).  Returns (seconds per unit of the workload,
+    description, cores)."""
     import oracle
     c = synth.CONFIGS[cfg_index]
     bid = oracle.POLY if c["basis"] == "poly" else oracle.BSPLINE
     R = pair.R if pair.R.ndim == 2 else pair.R[0]
     S = pair.S if pair.S.ndim == 2 else pair.S[0]
+    if crop is None:
+        t0 = time.perf_counter()
+        M, rhs = oracle.normal_from_lags(R, S, c["L"], bid, c["DK"], c["DB"])
+        t1 = time.perf_counter()
+        coef = oracle.solve(M, rhs)
+        t2 = time.perf_counter()
+        oracle.difference(R, S, coef, c["L"], bid, c["DK"], c["DB"])
+        t3 = time.perf_counter()
+        desc = (f"oracle (direct pixel sums, no FFT) on the FULL {c['H']}x{c['W']} pair: normal system {t1 - t0:.2f}s, "
+                f"n={M.shape[0]} solve {t2 - t1:.2f}s, difference image {t3 - t2:.2f}s")
+        return t3 - t0, desc, oracle.num_threads()
     ch, cw = min(crop, c["H"]), min(crop, c["W"])
     Rc, Sc = np.ascontiguousarray(R[:ch, :cw]), np.ascontiguousarray(S[:ch, :cw])
     scale = (c["H"] * c["W"]) / float(ch * cw)
@@ -118,35 +154,125 @@ def oracle_sample(cfg_index, pair, crop=1024):
     t2 = time.perf_counter()
     oracle.difference(Rc, Sc, coef, c["L"], bid, c["DK"], c["DB"])
     t3 = time.perf_counter()
-    per_pair = (t1 - t0) * scale + (t2 - t1) + (t3 - t2) * scale
-    desc = (f"oracle (direct pixel sums, no FFT) on a {ch}x{cw} crop of the pair: normal system {t1 - t0:.2f}s and "
-            f"difference {t3 - t2:.2f}s scaled x{scale:.0f} to the full frame, plus the full n={M.shape[0]} solve {t2 - t1:.2f}s")
-    return per_pair * c["batch"], desc, oracle.num_threads()
+    per_unit = (t1 - t0) * scale + (t2 - t1) + (t3 - t2) * scale
+    desc = (f"EXTRAPOLATED: oracle on a {ch}x{cw} crop of one sub-field: normal system {t1 - t0:.2f}s and difference "
+            f"{t3 - t2:.2f}s scaled x{scale:.0f} to the full frame, plus the full n={M.shape[0]} solve {t2 - t1:.2f}s")
+    return per_unit, desc, oracle.num_threads()
+
+
+def oracle_crop_for(cfg_index):
+    return None if synth.CONFIGS[cfg_index]["batch"] == 1 else 256
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle (this tier has no reference implementation) on the same config."""
+    """--impl reference: the CPU oracle (this tier has no reference implementation) on the same config.
+    A step is one full oracle pass over the pair; the oracle is slow by construction, so the arm stops after
+    REFERENCE_BUDGET_S of wall clock and prints the number of steps and warm-ups it ACTUALLY ran."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     cfg = args.config
-    pair = synth.make_pair(cfg) if synth.CONFIGS[cfg]["batch"] == 1 else synth.make_pair(cfg, subfield=0)
-    times, desc, cores = [], "", 1
-    for i in range(args.warmup + args.steps):
-        sec, desc, cores = oracle_sample(cfg, pair, crop=args.ref_crop)
-        if i >= args.warmup:
-            times.append(sec)
+    single = synth.CONFIGS[cfg]["batch"] == 1
+    pair = synth.make_pair(cfg) if single else synth.make_pair(cfg, subfield=0)
+    crop = args.ref_crop if args.ref_crop > 0 else oracle_crop_for(cfg)
+    t_begin = time.perf_counter()
+    times, warm_done = [], 0
+    t0 = time.perf_counter()
+    sec, desc, cores = oracle_pass(cfg, pair, crop)
+    wall = time.perf_counter() - t0           # wall clock of one pass (what the budget is counted in)
+    if args.warmup > 0 and 3.0 * wall < REFERENCE_BUDGET_S:
+        warm_done = 1                          # the first pass was a warm-up: more passes still fit
+        while warm_done < args.warmup and wall < 10.0 and (time.perf_counter() - t_begin) + 2.0 * wall < REFERENCE_BUDGET_S:
+            oracle_pass(cfg, pair, crop)       # further warm-ups only while passes are short
+            warm_done += 1
+    else:
+        times.append(sec)                      # a pass is so long that the first one is the measurement
+    while len(times) < args.steps and (not times or (time.perf_counter() - t_begin) + wall < REFERENCE_BUDGET_S):
+        sec, desc, cores = oracle_pass(cfg, pair, crop)
+        times.append(sec)
     sec = float(np.mean(times))
     val = 1.0 / sec
     line = {
-        "impl": "reference", "metric": METRIC, "value": val, "unit": "pairs/s", "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": {"workload": workload_name(cfg)},
+        "impl": "reference", "metric": metric_name(cfg), "value": val, "unit": "pairs/s", "n_gpus": args.gpus,
+        "steps": len(times), "warmup": warm_done, "steps_requested": args.steps, "warmup_requested": args.warmup,
+        "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak" if single else "strong",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": {"workload": workload_name(cfg)},
         "cpu_baseline": {"value": val, "unit": "pairs/s", "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": val, "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
+
+
+def load_bench_lib():
+    """libsfft_bench.so: FP64 peak probes and flop counters (csrc/bench/, measurement support only)."""
+    from paper_2109_09334_b200 import build as libbuild
+    L = ctypes.CDLL(libbuild.build_bench_library())
+    L.sfft_bench_fp64_peak.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+    L.sfft_bench_corr_flops.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+    return L
+
+
+def time_cuda(torch, fn, reps=5, warm=2):
+    """Median device time (ms) of fn() by CUDA events on the current stream."""
+    for _ in range(warm):
+        fn()
+    ts = []
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        e1.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    return float(np.median(ts))
+
+
+def library_comparison(torch, dev, c, nb, n, stage_ms):
+    """Vendor-library comparison points in the same run, same clocks (SURVEY.md 8(d) "Timing protocol"):
+    cuFFT batched D2Z / Z2D of the row-transform shape and cuSOLVER potrf + potrs at the solve's size,
+    both through torch (comparison only; nothing here is linked into or called by libsfft_b200.so)."""
+    out = {"note": "cuFFT / cuSOLVER via torch.fft / torch.linalg, timed with CUDA events; comparison points only"}
+    nKa = (c["DK"] + 1) if c["basis"] == "poly" else (c["DK"] + 4)
+    try:
+        nimg = min(nKa + 1, 8) * min(nb, 8)
+        x = torch.randn((nimg, c["H"], c["W"]), dtype=torch.float64, device=dev)
+        t_f = time_cuda(torch, lambda: torch.fft.rfft(x, dim=-1))
+        X = torch.fft.rfft(x, dim=-1)
+        t_i = time_cuda(torch, lambda: torch.fft.irfft(X[:1], n=c["W"], dim=-1))
+        byts = nimg * c["H"] * c["W"] * 8 * 2.0
+        out["cufft_d2z_rows"] = {"shape": [nimg, c["H"], c["W"]], "ms": t_f, "gbs": byts / (t_f * 1e-3) / 1e9,
+                                 "ours_ms_same_transform_count": float(stage_ms[0]) * nimg / ((nKa + 1) * nb),
+                                 "note": "unweighted batched 1-D D2Z; ours also applies the y-weights and writes "
+                                         "nKa+1 spectra from 2 images"}
+        out["cufft_z2d_rows"] = {"shape": [1, c["H"], c["W"]], "ms": t_i,
+                                 "note": "one image; ours fuses D = S - model - background into this transform"}
+        del x, X
+    except Exception as e:   # a comparison point must never take the benchmark down
+        out["cufft_error"] = repr(e)[:200]
+    try:
+        try:
+            torch.backends.cuda.preferred_linalg_library("cusolver")
+        except Exception:
+            pass
+        k = nb if nb * n * n * 8.0 * 3 < 60e9 else 1
+        g = torch.Generator(device=dev).manual_seed(7)
+        A = torch.randn((k, n, n + 16), dtype=torch.float64, device=dev, generator=g)
+        Msp = A @ A.transpose(-1, -2)
+        b = torch.randn((k, n, 1), dtype=torch.float64, device=dev, generator=g)
+        del A
+
+        def potrf_potrs():
+            Lc = torch.linalg.cholesky(Msp)
+            return torch.cholesky_solve(b, Lc)
+
+        t_s = time_cuda(torch, potrf_potrs, reps=3, warm=1)
+        out["cusolver_potrf_potrs"] = {"n": n, "systems": k, "ms": t_s, "ms_per_system": t_s / k,
+                                       "ours_ms_per_system": float(stage_ms[5]) / nb}
+        del Msp, b
+    except Exception as e:
+        out["cusolver_error"] = repr(e)[:200]
+    return out
 
 
 def main():
@@ -156,9 +282,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
-    ap.add_argument("--ref-crop", type=int, default=1024)
+    ap.add_argument("--ref-crop", type=int, default=0, help="time the oracle on a crop (0: full pair; config 5: 256)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-pipelined", action="store_true")
+    ap.add_argument("--no-compare", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -181,12 +308,16 @@ def main():
 
     cfg = args.config
     c = synth.CONFIGS[cfg]
-    nb = c["batch"]
-    # every rank owns one independent unit (pair, or batch of sub-fields) per step: weak scaling
-    lo, hi = shard_units(world, rank, world)
-    assert hi - lo == 1
-    pair = synth.make_pair(cfg) if nb == 1 else synth.make_batch(cfg)
-    plan = B.Plan(c["H"], c["W"], c["L"], c["DK"], c["DB"], c["basis"], nbatch=nb, device=dev)
+    first, nb, scaling = rank_units(cfg, rank, world)
+    total_units = world if c["batch"] == 1 else c["batch"]
+    if nb < 1:
+        raise SystemExit(f"bench.py: rank {rank} of {world} has no unit of config {cfg}")
+    if c["batch"] == 1:
+        pair = synth.make_pair(cfg)
+    else:
+        pair = synth.make_batch(cfg, nbatch=nb, first=first, workers=min(16, os.cpu_count() or 1))
+    # fit and apply on the same pair: the subtract may reuse the build's row spectra (explicit opt-in)
+    plan = B.Plan(c["H"], c["W"], c["L"], c["DK"], c["DB"], c["basis"], nbatch=nb, device=dev, reuse_spectra=True)
     dR = torch.from_numpy(np.ascontiguousarray(pair.R)).to(dev)
     dS = torch.from_numpy(np.ascontiguousarray(pair.S)).to(dev)
     dD = torch.empty_like(dS)
@@ -233,15 +364,16 @@ def main():
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_step = float(t.item()) / args.steps
-    value = world * nb / (ms_step * 1e-3)
+    value = total_units / (ms_step * 1e-3)
 
     # ---- two pairs in flight (informational, not the headline): a second plan on a second stream, so that one
-    # pair's latency-bound solve overlaps the other's tensor-bound lag correlation ----
+    # pair's latency-bound solve overlaps the other's FP64-bound lag correlation ----
     pipelined = None
-    if nb == 1 and not args.no_pipelined:
+    if c["batch"] == 1 and not args.no_pipelined:
         s2 = torch.cuda.Stream(device=dev)
         with torch.cuda.stream(s2):
-            plan2 = B.Plan(c["H"], c["W"], c["L"], c["DK"], c["DB"], c["basis"], nbatch=nb, device=dev)
+            plan2 = B.Plan(c["H"], c["W"], c["L"], c["DK"], c["DB"], c["basis"], nbatch=nb, device=dev,
+                           reuse_spectra=True)
             dR2, dS2, dD2, coef2 = dR.clone(), dS.clone(), torch.empty_like(dS), torch.empty_like(coef)
 
         def step2():
@@ -263,6 +395,7 @@ def main():
             dist.all_reduce(tp, op=dist.ReduceOp.MAX)
         plan2.status()
         plan2.close()
+        del dR2, dS2, dD2
         pipelined = {"pairs_in_flight": 2, "value": world * 2 * nb / float(tp.item()), "unit": "pairs/s",
                      "note": "two plans on two streams, wall clock around K double steps; not the headline value"}
 
@@ -272,6 +405,7 @@ def main():
     hD = torch.empty_like(hR).pin_memory()
     hC = torch.empty((nb, plan.n), dtype=torch.float64).pin_memory()
     e2e_steps = max(3, min(args.steps, 20))
+    plan.ensure_host_staging()
 
     def e2e_submit():
         st = B.sfft_run_host_async(plan.h, hR.data_ptr(), hS.data_ptr(), hD.data_ptr(), hC.data_ptr())
@@ -303,8 +437,8 @@ def main():
         st = B.sfft_run_host(plan.h, hR.data_ptr(), hS.data_ptr(), hD.data_ptr(), hC.data_ptr())
         if st != B.SFFT_OK:
             raise B.SfftError(st, "sfft_run_host")
-    e2e_sync_val = world * nb / ((time.perf_counter() - t0) / 3)
-    e2e_val = world * nb / float(e2e_s.item())
+    e2e_sync_val = total_units / ((time.perf_counter() - t0) / 3)
+    e2e_val = total_units / float(e2e_s.item())
     img_bytes = nb * c["H"] * c["W"] * 8
 
     if rank == 0:
@@ -324,28 +458,39 @@ def main():
         hbm_peak = peaks.get("hbm_gbs", 6650.0)
         peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback"
         alg = {
-            # row FFT: read R (nKa times, L2-served after the first) + S, write nKa+1 half spectra
+            # row FFT: read R and S once, write nKa+1 half spectra
             "rowfft": ("hbm", (2 * P * 8 + (nKa + 1) * P * 8) * nb / 1e9, hbm_peak, "GB/s"),
             # lag correlation: SURVEY 8(d) pruned-FFT figure ~ (FK(FK+1)/2 + FK) maps x columns x 5 N log2 N x 0.6
             "corr": ("alu", (FK * (FK + 1) // 2 + FK) * (c["W"] // 2 + 1) * 5.0 * c["H"] * np.log2(c["H"]) * 0.6 * nb / 1e12,
                      FP64_PEAK_TFLOPS, "TFLOP/s"),
+            # gather: one write of the n x n matrix
+            "gather": ("hbm", plan.ns * plan.ns * 8.0 * nb / 1e9, hbm_peak, "GB/s"),
             # subtract: SURVEY 8(d) Fourier-route figure, L*FK complex MACs per spectrum point (8 flop each)
             "subtract": ("alu", 8.0 * L * FK * c["H"] * (c["W"] // 2) * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
-            "solve": ("alu", (plan.n ** 3 / 3.0) * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
+            "solve": ("alu", (plan.ns ** 3 / 3.0) * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
         }
         tname = names[top]
         bound, work, peak, unit = alg.get(tname, ("hbm", 0.0, hbm_peak, "GB/s"))
         achieved = work / (stage_ms[top] * 1e-3)
         roofline = {"kernel": tname, "bound": bound, "achieved": achieved, "peak": peak, "unit": unit,
                     "frac": achieved / peak, "traffic": NCU_TRAFFIC_CFG4.get(tname) if cfg == 4 else None,
+                    "traffic_source": NCU_TRAFFIC_SOURCE.get(tname) if cfg == 4 else None,
                     "ms": float(stage_ms[top]),
                     "peak_source": peak_src if bound == "hbm" else "derived: 148 SM x 64 FP64 FMA/clk x 1.965 GHz"}
-        if tname == "corr":
-            # the x-direction is executed as direct lag sums on the FP64 tensor cores: DMMA flops actually issued
-            ex = plan.corr_executed_flops() * nb
-            st_dm, dmma = B.sfft_measure_fp64_peak(1)
-            roofline["executed_tflops"] = ex / 1e12 / (stage_ms[top] * 1e-3)
-            roofline["dmma_peak_measured_tflops"] = dmma if st_dm == B.SFFT_OK else None
+        blib = None
+        try:
+            blib = load_bench_lib()
+        except Exception as e:
+            roofline["bench_lib_error"] = repr(e)[:200]
+        if blib is not None:
+            ex, tc = ctypes.c_double(0.0), ctypes.c_double(0.0)
+            if blib.sfft_bench_corr_flops(plan.h, ctypes.byref(ex), ctypes.byref(tc)) == 0:
+                t_corr = stage_ms[names.index("corr")] * 1e-3
+                roofline["corr_executed_tflops"] = ex.value * nb / 1e12 / t_corr
+                roofline["corr_executed_gflop"] = ex.value * nb / 1e9
+            pk = ctypes.c_double(0.0)
+            for kind, key in ((0, "dfma_peak_measured_tflops"), (1, "dmma_peak_measured_tflops")):
+                roofline[key] = pk.value if blib.sfft_bench_fp64_peak(kind, ctypes.byref(pk)) == 0 else None
         rf_all = {}
         for nm, (bd, wk, pk, un) in alg.items():
             t_ms = stage_ms[names.index(nm)]
@@ -353,11 +498,13 @@ def main():
                 rf_all[nm] = {"bound": bd, "achieved": round(wk / (t_ms * 1e-3), 3), "peak": round(pk, 1), "unit": un,
                               "frac": round(wk / (t_ms * 1e-3) / pk, 4)}
         line = {
-            "metric": METRIC, "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "metric": metric_name(cfg), "value": value, "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": scaling,
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(cfg), "l2": "inputs and intermediates (>= 0.8 GB per step) exceed the 126 MB L2",
-                       "unknowns": plan.n, "pairs_per_step_per_gpu": nb},
+            "config": {"workload": workload_name(cfg),
+                       "l2": "inputs and intermediates (>= 0.8 GB per step) exceed the 126 MB L2",
+                       "unknowns": plan.n, "pairs_per_step_per_gpu": nb,
+                       "reuse_spectra": "on (sfft_plan_set_reuse_spectra: fit and apply on the same pair)"},
             "e2e": {"value": e2e_val, "unit": "pairs/s", "h2d_bytes_per_step": 2 * img_bytes,
                     "d2h_bytes_per_step": img_bytes + nb * plan.n * 8, "steps": e2e_steps,
                     "api": "sfft_run_host_async x steps + sfft_run_host_wait (two staging slots, copy streams)",
@@ -369,8 +516,12 @@ def main():
             "pipelined": pipelined,
             "stage_ms": stages,
         }
+        if not args.no_compare and world == 1:
+            del hR, hS, hD
+            line["comparison"] = library_comparison(torch, dev, c, nb, plan.ns, stage_ms)
         if not args.no_cpu_baseline and world == 1:
-            sec, desc, cores = oracle_sample(cfg, pair, crop=args.ref_crop)
+            crop = args.ref_crop if args.ref_crop > 0 else oracle_crop_for(cfg)
+            sec, desc, cores = oracle_pass(cfg, pair, crop)
             line["cpu_baseline"] = {"value": 1.0 / sec, "unit": "pairs/s", "cores": cores, "kind": "oracle", "sample": desc}
         print(json.dumps(line))
     plan.close()

@@ -28,7 +28,8 @@
  * buffer, including the workspace; the plan owns only small constant tables.  Calls enqueue
  * work on the plan's CUDA stream and return without synchronising unless stated.  Every call
  * returns an SFFT_* status; nothing throws or aborts.  There is no CPU fallback: without a
- * CUDA device every compute call returns SFFT_ERR_CUDA.
+ * CUDA device every compute call returns SFFT_ERR_CUDA.  A plan belongs to the CUDA device that was
+ * current when it was created; calling it with another device current returns SFFT_ERR_STATE.
  */
 #ifndef SFFT_H_
 #define SFFT_H_
@@ -76,12 +77,10 @@ int sfft_plan_num_solved(const sfft_plan *plan);
 /* n = F_K*L*L + F_B (Eq. 18's dimension), or -1 for a null plan. */
 int sfft_plan_num_unknowns(const sfft_plan *plan);
 int sfft_plan_num_kernel_terms(const sfft_plan *plan);     /* F_K */
-/* Measurement support: FP64 tensor-core flops (mma.sync.m8n8k4.f64, 512 each) one sfft_build_system issues
- * per batch entry in the x-direction lag correlation (steps a3+a4), counted from the plan's job list. */
-double sfft_plan_corr_executed_flops(const sfft_plan *plan);
 int sfft_plan_num_background_terms(const sfft_plan *plan); /* F_B */
 
-/* Bytes of device workspace the plan needs for its current batch size. */
+/* Bytes of device workspace the plan needs for its current batch size (build / solve / subtract on device
+ * pointers; the image staging area of the host-buffer entry points is a separate buffer, see below). */
 size_t sfft_plan_workspace_bytes(const sfft_plan *plan);
 
 /* Lend a device buffer (>= workspace_bytes, 256-byte aligned) to the plan.  The caller keeps
@@ -96,19 +95,24 @@ int sfft_plan_set_workspace(sfft_plan *plan, void *d_ws, size_t bytes);
  * and joined back into the plan's stream with events: ordering on the plan's stream is all a caller sees. */
 int sfft_build_system(sfft_plan *plan, const double *d_R, const double *d_S);
 
-/* Device pointers to the assembled system (valid until the next build): M is [nbatch][n][ld]
- * row-major, FULL symmetric (both triangles), ld = n; rhs is [nbatch][n].  For parity tests. */
+/* Device pointers to the assembled system (valid until the next build): M is [nbatch][ns][ld] row-major,
+ * FULL symmetric (both triangles), ld = ns = sfft_plan_num_solved() (= n unless the photometric ratio is
+ * constrained); rhs is [nbatch][ns].  For parity tests. */
 int sfft_get_system(const sfft_plan *plan, const double **d_M, const double **d_rhs, int *ld);
 
 /* Device pointer to the lag tables of the last build, for parity tests.  which: 0 = Omega
- * [nbatch][npairs][2L-1][2L-1] over pairs (tb <= t) in row-major pair order, 1 = Theta
- * [nbatch][F_K][L][L], 2 = Lambda [nbatch][F_K][F_B][L][L], 3 = Delta [nbatch][F_B].
- * count receives the number of doubles per batch entry. */
-int sfft_get_lag_table(const sfft_plan *plan, int which, const double **d_table, size_t *count);
+ * [npairs][2L-1][2L-1] over pairs (tb <= t) in row-major pair order, 1 = Theta [F_K][L][L],
+ * 2 = Lambda [F_K][F_B][L][L], 3 = Delta [F_B].  *d_table points at the table of batch entry 0; the
+ * same table of batch entry b starts *batch_stride doubles further per entry.  count receives the number
+ * of doubles of the table (per batch entry).  count and batch_stride may be NULL. */
+int sfft_get_lag_table(const sfft_plan *plan, int which, const double **d_table, size_t *count, size_t *batch_stride);
 
 /* Step a6: solve M c = rhs (Jacobi-scaled blocked FP64 Cholesky; DESIGN g11) and write
- * c to d_coef [nbatch][n].  A non-positive pivot raises a device flag reported by
- * sfft_plan_status as SFFT_ERR_NOT_SPD; d_coef is then undefined. */
+ * c to d_coef [nbatch][n].  A diagonal entry that is not positive and finite, or a pivot of the
+ * Jacobi-scaled matrix (unit diagonal) that is not finite or falls below 64 n eps (eps = 2^-52: the level
+ * at which a pivot is rounding noise of the assembled entries, i.e. the system is numerically
+ * rank-deficient), raises a device flag reported by sfft_plan_status as SFFT_ERR_NOT_SPD; d_coef is then
+ * undefined. */
 int sfft_solve(sfft_plan *plan, double *d_coef);
 
 /* Steps a7-a8: D = S - sum_t sum_ab k_{t,ab} R^t((x-a)%H,(y-b)%W) - sum_s b_s T'_s  (Eqs. 1, 12)
@@ -117,19 +121,34 @@ int sfft_solve(sfft_plan *plan, double *d_coef);
  * original).  d_D [nbatch][H][W] may alias d_S; no other aliasing.
  * Two routes, chosen by the plan from its sizes: the direct tensor-core contraction, or (wide
  * kernels on rows of >= 1024 pixels) a FIR filter along x on the row spectra followed by one
- * inverse row transform.  The second route reuses the row spectra of d_R computed by the last
- * sfft_build_system when d_R is the very pointer passed to it: in that case the contents of
- * d_R must not have changed since that call (pass another buffer, or call sfft_build_system
- * again, otherwise).  It overwrites the workspace slot holding the row spectrum of S. */
+ * inverse row transform.  The second route needs the row spectra of d_R: by default it transforms
+ * d_R again on every call (whatever was passed to sfft_build_system); see sfft_plan_set_reuse_spectra
+ * for the opt-in that skips this.  It overwrites the workspace slot holding the row spectrum of S. */
 int sfft_subtract(sfft_plan *plan, const double *d_coef, const double *d_R, const double *d_S, double *d_D);
 
+/* Opt-in for the Fourier-route subtract: on = 1 is the caller's PROMISE that every following sfft_subtract is
+ * given, as d_R, an image with the same contents as the d_R of the last sfft_build_system (the unmasked flow:
+ * fit and apply on the same pair); the row spectra computed by that build are then reused instead of
+ * transforming d_R again.  Pointer values play no role in either mode.  Default 0: always transform again,
+ * which is what the paper's masked flow needs (fit on the masked pair, apply to the original).
+ * The host-buffer entry points below fit and apply on the same staged pair and always reuse. */
+int sfft_plan_set_reuse_spectra(sfft_plan *plan, int on);
+
 /* Synchronise the plan's stream and report numerical status.  On SFFT_ERR_NOT_SPD, *info =
- * batch*n + index of the first failing pivot; otherwise *info = -1.  info may be NULL. */
+ * batch*ns + index of the first failing pivot in the order of the solved system (ns =
+ * sfft_plan_num_solved(): the reduced layout under the constant photometric ratio); otherwise
+ * *info = -1.  info may be NULL. */
 int sfft_plan_status(sfft_plan *plan, int *info);
+
+/* Device staging area of the host-buffer entry points (two slots of R, S, D images and coefficients):
+ * size for the current batch, and the call that lends a caller-owned device buffer (>= that size, 256-byte
+ * aligned) to the plan.  Callers that only use device pointers never need it. */
+size_t sfft_plan_host_staging_bytes(const sfft_plan *plan);
+int sfft_plan_set_host_staging(sfft_plan *plan, void *d_buf, size_t bytes);
 
 /* End-to-end convenience with HOST buffers: copies h_R, h_S ([nbatch][H][W]) to the device,
  * runs build -> solve -> subtract, copies D and the coefficients back, synchronises.
- * Needs the workspace (sfft_plan_workspace_bytes already includes the image staging area).
+ * Needs the workspace and the staging area (SFFT_ERR_WORKSPACE otherwise).
  * h_D [nbatch][H][W], h_coef [nbatch][n] (either may be NULL to skip that copy). */
 int sfft_run_host(sfft_plan *plan, const double *h_R, const double *h_S, double *h_D, double *h_coef);
 
@@ -160,11 +179,6 @@ void sfft_plan_destroy(sfft_plan *plan);
 const char *sfft_strerror(int status);
 const char *sfft_last_cuda_error(const sfft_plan *plan);
 const char *sfft_version(void);
-
-/* Measurement support (not on the hot path): achieved FP64 throughput of the current device in TFLOP/s from a
- * register-resident probe kernel, kind 0 = plain FMA pipe (DFMA), kind 1 = FP64 tensor cores (mma.sync.m8n8k4.f64).
- * These are the denominators of the "alu" rooflines in DESIGN.md / bench.py.  Synchronous; best of 3 timed runs. */
-int sfft_measure_fp64_peak(int kind, double *tflops);
 
 #ifdef __cplusplus
 }

@@ -9,7 +9,7 @@ file only compiles it with gcc and marshals numpy arrays through ctypes.
 """
 from .binding import (  # noqa: F401
     POLY, BSPLINE, build_library, num_threads, num_terms, num_axis, terms, axis_table,
-    num_unknowns, design_matrix, gram, normal_bruteforce, lag_tables, gather,
+    num_unknowns, design_matrix, gram, normal_bruteforce, diag_and_rhs, lag_tables, gather,
     normal_from_lags, solve, difference, difference_at, corr_diff_one, weighted_ref,
     cpr_num_unknowns, cpr_constrain, cpr_expand,
 )

@@ -44,6 +44,7 @@ def _load():
     L.orc_design_matrix.argtypes = [_ci] * 6 + [_D, _D]
     L.orc_gram.argtypes = [_ci, ctypes.c_long, _D, _D, _D, _D]
     L.orc_lag_tables.argtypes = [_ci] * 6 + [_D] * 10
+    L.orc_diag_and_rhs.argtypes = [_ci] * 6 + [_D] * 4
     L.orc_gather.argtypes = [_ci] * 3 + [_D] * 10
     L.orc_solve.argtypes = [_ci, _D, _D, _D, _ci]
     L.orc_difference.argtypes = [_ci] * 6 + [_D] * 4
@@ -113,6 +114,16 @@ def gram(Phi, S):
 def normal_bruteforce(R, S, L, basis, DK, DB):
     """Tier A normal system from the materialised design matrix."""
     return gram(design_matrix(R, L, basis, DK, DB), S)
+
+
+def diag_and_rhs(R, S, L, basis, DK, DB):
+    """(diag(M), rhs) from the column definitions, without the rest of the normal matrix."""
+    R, S = _c(R), _c(S)
+    H, W = R.shape
+    n = num_unknowns(L, basis, DK, DB)
+    diag, rhs = np.zeros(n), np.zeros(n)
+    _load().orc_diag_and_rhs(H, W, L, basis, DK, DB, R, S, diag, rhs)
+    return diag, rhs
 
 
 def lag_tables(R, S, L, basis, DK, DB):

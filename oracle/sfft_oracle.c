@@ -177,6 +177,64 @@ void orc_gram(int n, long P, const double *Phi, const double *S, double *M, doub
     }
 }
 
+/* diag[k] = sum_p Phi_k(p)^2 and rhs[k] = sum_p Phi_k(p) S(p) for every unknown k, straight from the column
+ * definitions of orc_design_matrix (Eqs. 3-4, 11-12) without materialising Phi: the diagonal of the normal
+ * matrix and the whole right-hand side at 2 n P multiply-adds, cheap enough to check every entry of a large
+ * batch (config 5: all 64 sub-fields).  Row partial sums in double, rows combined in long double. */
+void orc_diag_and_rhs(int H, int W, int L, int basis, int DK, int DB, const double *R, const double *S,
+                      double *diag, double *rhs) {
+    orc_basis b; basis_make(&b, H, W, basis, DK, DB);
+    int w = (L - 1) / 2, LL = L * L; size_t P = (size_t)H * W;
+    double *Rt = (double *)malloc(sizeof(double) * P);
+    for (int t = 0; t < b.FK; ++t) {
+        weighted_image(H, W, b.fK + (size_t)b.kti[t] * H, b.gK + (size_t)b.ktj[t] * W, R, Rt);
+        /* rows outermost (each image row is read once per term), all L*L lags per row; per-thread long-double
+         * accumulators of double row partial sums, combined at the end */
+        long double *acc2 = (long double *)calloc((size_t)LL, sizeof(long double));
+        long double *accs = (long double *)calloc((size_t)LL, sizeof(long double));
+#pragma omp parallel
+        {
+            long double *l2 = (long double *)calloc((size_t)LL, sizeof(long double));
+            long double *ls = (long double *)calloc((size_t)LL, sizeof(long double));
+            double *sh = (double *)malloc(sizeof(double) * W);       /* sh[y] = R^t((x-al)%H, (y-be)%W) */
+#pragma omp for schedule(static)
+            for (int x = 0; x < H; ++x) {
+                const double *own = Rt + (size_t)x * W, *sr = S + (size_t)x * W;
+                for (int a = 0; a < LL; ++a) {
+                    int al = a / L - w, be = a % L - w, centre = (al == 0 && be == 0);
+                    const double *src = Rt + (size_t)wrap(x - al, H) * W;
+                    int o = wrap(-be, W);                     /* sh[y] = src[(y + o) % W], in two runs */
+                    for (int y = 0; y < W - o; ++y) sh[y] = src[y + o];
+                    for (int y = W - o; y < W; ++y) sh[y] = src[y + o - W];
+                    double r2 = 0.0, rs = 0.0, cm = centre ? 0.0 : 1.0;
+#pragma omp simd reduction(+ : r2, rs)
+                    for (int y = 0; y < W; ++y) {
+                        double v = sh[y] - cm * own[y];
+                        r2 += v * v; rs += v * sr[y];
+                    }
+                    l2[a] += r2; ls[a] += rs;
+                }
+            }
+#pragma omp critical
+            for (int a = 0; a < LL; ++a) { acc2[a] += l2[a]; accs[a] += ls[a]; }
+            free(l2); free(ls); free(sh);
+        }
+        for (int a = 0; a < LL; ++a) { diag[(size_t)t * LL + a] = (double)acc2[a]; rhs[(size_t)t * LL + a] = (double)accs[a]; }
+        free(acc2); free(accs);
+    }
+    for (int s = 0; s < b.FB; ++s) {
+        const double *fx = b.fB + (size_t)b.bti[s] * H, *gy = b.gB + (size_t)b.btj[s] * W;
+        long double a2 = 0.0L, as = 0.0L;
+        for (int x = 0; x < H; ++x) {
+            double r2 = 0.0, rs = 0.0;
+            for (int y = 0; y < W; ++y) { double v = fx[x] * gy[y]; r2 += v * v; rs += v * S[(size_t)x * W + y]; }
+            a2 += r2; as += rs;
+        }
+        diag[(size_t)b.FK * LL + s] = (double)a2; rhs[(size_t)b.FK * LL + s] = (double)as;
+    }
+    free(Rt); basis_free(&b);
+}
+
 /* ---------------------------------------------------------------- Tier B */
 
 /* Direct-sum correlation in difference form, all lags |rho|,|eps| <= wl:

@@ -15,14 +15,14 @@ from . import build as _build
 SFFT_BASIS_POLY, SFFT_BASIS_BSPLINE = 0, 1
 SFFT_OK, SFFT_ERR_INVALID_ARG, SFFT_ERR_STATE, SFFT_ERR_WORKSPACE, SFFT_ERR_CUDA, SFFT_ERR_NOT_SPD = range(6)
 
-# every symbol include/sfft.h declares (checked against the built library by tests/test_abi.py)
+# every symbol include/sfft.h declares (checked against the built library by tests/test_abi_and_host.py)
 EXPORTS = [
     "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
-    "sfft_plan_num_kernel_terms", "sfft_plan_corr_executed_flops", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
+    "sfft_plan_num_kernel_terms", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
-    "sfft_subtract", "sfft_plan_status", "sfft_run_host", "sfft_run_host_async", "sfft_run_host_wait", "sfft_plan_launch_count", "sfft_plan_destroy",
+    "sfft_subtract", "sfft_plan_set_reuse_spectra", "sfft_plan_status", "sfft_plan_host_staging_bytes", "sfft_plan_set_host_staging",
+    "sfft_run_host", "sfft_run_host_async", "sfft_run_host_wait", "sfft_plan_launch_count", "sfft_plan_destroy",
     "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
-    "sfft_measure_fp64_peak",
 ]
 SFFT_NUM_STAGES = 8
 STAGE_NAMES = ["rowfft", "corr", "lagsum", "moments", "gather", "solve", "subtract_prep", "subtract"]
@@ -46,10 +46,10 @@ def load_library(build_if_missing=True):
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(_build.LIB):
-        if not build_if_missing:
-            raise FileNotFoundError(f"{_build.LIB} is missing: run __graft_entry__.build()")
-        _build.build_library()
+    if not os.path.exists(_build.LIB) and not build_if_missing:
+        raise FileNotFoundError(f"{_build.LIB} is missing: run __graft_entry__.build()")
+    if build_if_missing:
+        _build.build_library()          # no-op unless the library is missing or older than its sources
     L = ctypes.CDLL(_build.LIB)
     vp, ci, cs = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
     pvp, pci = ctypes.POINTER(ctypes.c_void_p), ctypes.POINTER(ctypes.c_int)
@@ -61,16 +61,18 @@ def load_library(build_if_missing=True):
         "sfft_plan_num_solved": (ci, [vp]),
         "sfft_plan_num_unknowns": (ci, [vp]),
         "sfft_plan_num_kernel_terms": (ci, [vp]),
-        "sfft_plan_corr_executed_flops": (ctypes.c_double, [vp]),
         "sfft_plan_num_background_terms": (ci, [vp]),
         "sfft_plan_workspace_bytes": (cs, [vp]),
         "sfft_plan_set_workspace": (ci, [vp, vp, cs]),
         "sfft_build_system": (ci, [vp, vp, vp]),
         "sfft_get_system": (ci, [vp, pvp, pvp, pci]),
-        "sfft_get_lag_table": (ci, [vp, ci, pvp, ctypes.POINTER(cs)]),
+        "sfft_get_lag_table": (ci, [vp, ci, pvp, ctypes.POINTER(cs), ctypes.POINTER(cs)]),
         "sfft_solve": (ci, [vp, vp]),
         "sfft_subtract": (ci, [vp, vp, vp, vp, vp]),
+        "sfft_plan_set_reuse_spectra": (ci, [vp, ci]),
         "sfft_plan_status": (ci, [vp, pci]),
+        "sfft_plan_host_staging_bytes": (cs, [vp]),
+        "sfft_plan_set_host_staging": (ci, [vp, vp, cs]),
         "sfft_run_host": (ci, [vp, vp, vp, vp, vp]),
         "sfft_run_host_async": (ci, [vp, vp, vp, vp, vp]),
         "sfft_run_host_wait": (ci, [vp]),
@@ -81,7 +83,6 @@ def load_library(build_if_missing=True):
         "sfft_version": (ctypes.c_char_p, []),
         "sfft_plan_profile": (ci, [vp, ci]),
         "sfft_plan_profile_read": (ci, [vp, vp, pci]),
-        "sfft_measure_fp64_peak": (ci, [ci, ctypes.POINTER(ctypes.c_double)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -98,12 +99,6 @@ def sfft_strerror(status):
 
 def sfft_version():
     return load_library().sfft_version().decode()
-
-
-def sfft_measure_fp64_peak(kind):
-    v = ctypes.c_double(0.0)
-    st = load_library().sfft_measure_fp64_peak(int(kind), ctypes.byref(v))
-    return st, v.value
 
 
 def sfft_plan_create(H, W, L, DK, DB, basis):
@@ -151,9 +146,9 @@ def sfft_get_system(plan):
 
 
 def sfft_get_lag_table(plan, which):
-    t, cnt = ctypes.c_void_p(), ctypes.c_size_t()
-    st = load_library().sfft_get_lag_table(plan, which, ctypes.byref(t), ctypes.byref(cnt))
-    return st, t.value, cnt.value
+    t, cnt, stride = ctypes.c_void_p(), ctypes.c_size_t(), ctypes.c_size_t()
+    st = load_library().sfft_get_lag_table(plan, which, ctypes.byref(t), ctypes.byref(cnt), ctypes.byref(stride))
+    return st, t.value, cnt.value, stride.value
 
 
 def sfft_solve(plan, d_coef):
@@ -163,6 +158,18 @@ def sfft_solve(plan, d_coef):
 def sfft_subtract(plan, d_coef, d_R, d_S, d_D):
     return load_library().sfft_subtract(plan, ctypes.c_void_p(d_coef), ctypes.c_void_p(d_R), ctypes.c_void_p(d_S),
                                         ctypes.c_void_p(d_D))
+
+
+def sfft_plan_set_reuse_spectra(plan, on):
+    return load_library().sfft_plan_set_reuse_spectra(plan, int(on))
+
+
+def sfft_plan_host_staging_bytes(plan):
+    return load_library().sfft_plan_host_staging_bytes(plan)
+
+
+def sfft_plan_set_host_staging(plan, dptr, nbytes):
+    return load_library().sfft_plan_set_host_staging(plan, ctypes.c_void_p(dptr), nbytes)
 
 
 def sfft_plan_status(plan):
@@ -219,7 +226,8 @@ def _basis_id(basis):
 class Plan:
     """sfft_plan handle + workspace tensor on the current CUDA device and stream."""
 
-    def __init__(self, H, W, L, DK, DB, basis="poly", nbatch=1, device="cuda:0", const_phot_ratio=False):
+    def __init__(self, H, W, L, DK, DB, basis="poly", nbatch=1, device="cuda:0", const_phot_ratio=False,
+                 reuse_spectra=False):
         import torch
         if not torch.cuda.is_available():
             raise SfftError(SFFT_ERR_CUDA, "Plan", "no CUDA device: libsfft_b200 has no CPU fallback")
@@ -240,6 +248,16 @@ class Plan:
         self._check(sfft_plan_set_workspace(self.h, ptr, self.ws_bytes), "sfft_plan_set_workspace")
         self.stream = torch.cuda.current_stream(self.device)
         self._check(sfft_plan_set_stream(self.h, self.stream.cuda_stream), "sfft_plan_set_stream")
+        self._check(sfft_plan_set_reuse_spectra(self.h, reuse_spectra), "sfft_plan_set_reuse_spectra")
+        self.staging = None
+
+    def ensure_host_staging(self):
+        """Allocate the staging area of the host-buffer entry points on first use."""
+        if self.staging is None:
+            nbytes = sfft_plan_host_staging_bytes(self.h)
+            self.staging = self.torch.empty(nbytes + 256, dtype=self.torch.uint8, device=self.device)
+            ptr = (self.staging.data_ptr() + 255) & ~255
+            self._check(sfft_plan_set_host_staging(self.h, ptr, nbytes), "sfft_plan_set_host_staging")
 
     def _check(self, st, where):
         if st != SFFT_OK:
@@ -280,21 +298,25 @@ class Plan:
             raise SfftError(st, "sfft_plan_status", f"info={info}")
         return st, info
 
-    def system(self):
-        """Copies of (M [b][n][n], rhs [b][n]) as torch tensors (parity tests)."""
+    def system(self, batch=None):
+        """Copies of (M [b][ns][ns], rhs [b][ns]) as torch tensors (parity tests); one batch entry if `batch` is given."""
         st, pM, pr, ld = sfft_get_system(self.h)
         self._check(st, "sfft_get_system")
         self.status()
+        if batch is not None:
+            return (self._ws_view(pM + 8 * batch * self.ns * ld, (self.ns, ld)),
+                    self._ws_view(pr + 8 * batch * self.ns, (self.ns,)))
         return self._ws_view(pM, (self.nbatch, self.ns, ld)), self._ws_view(pr, (self.nbatch, self.ns))
 
-    def lag_table(self, which):
-        st, pt, cnt = sfft_get_lag_table(self.h, which)
+    def lag_table(self, which, batch=0):
+        st, pt, cnt, stride = sfft_get_lag_table(self.h, which)
         self._check(st, "sfft_get_lag_table")
         self.status()
-        return self._ws_view(pt, (cnt,))
+        return self._ws_view(pt + 8 * stride * batch, (cnt,))
 
     def run_host(self, R_host, S_host):
         """End to end with host (numpy) buffers through sfft_run_host.  Returns (D, coef) numpy arrays."""
+        self.ensure_host_staging()
         D = np.empty_like(R_host)
         coef = np.empty((self.nbatch, self.n))
         st = sfft_run_host(self.h, R_host.ctypes.data, S_host.ctypes.data, D.ctypes.data, coef.ctypes.data)
@@ -308,9 +330,6 @@ class Plan:
         st, ms = sfft_plan_profile_read(self.h, nsteps)
         self._check(st, "sfft_plan_profile_read")
         return ms
-
-    def corr_executed_flops(self):
-        return load_library().sfft_plan_corr_executed_flops(self.h)
 
     def launch_count(self):
         return sfft_plan_launch_count(self.h)

@@ -1,8 +1,10 @@
-// FP64 throughput probes (measurement support for bench.py, not on the hot path): the peak of the plain
+// Measurement support for bench.py (libsfft_bench.so; never linked into libsfft_b200.so).
+// FP64 throughput probes: the peak of the plain
 // FP64 FMA pipe (DFMA) and of the FP64 tensor-core path (mma.sync.m8n8k4.f64 -> DMMA) on this device,
 // the denominators of the "alu" rooflines in DESIGN.md.  Register-resident operands, 8 independent
 // accumulator chains per thread / warp, no memory traffic.
-#include "sfft_internal.h"
+#include "../sfft_internal.h"
+#include "sfft_bench.h"
 
 namespace sfft {
 namespace {
@@ -41,7 +43,7 @@ __global__ void __launch_bounds__(256) k_peak_dmma(double *out, int iters, doubl
 }  // namespace
 }  // namespace sfft
 
-extern "C" int sfft_measure_fp64_peak(int kind, double *tflops) {
+extern "C" int sfft_bench_fp64_peak(int kind, double *tflops) {
     if (!tflops || (kind != 0 && kind != 1)) return SFFT_ERR_INVALID_ARG;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
@@ -71,4 +73,16 @@ extern "C" int sfft_measure_fp64_peak(int kind, double *tflops) {
     cudaFree(d);
     *tflops = best;
     return e == cudaSuccess ? SFFT_OK : SFFT_ERR_CUDA;
+}
+
+extern "C" int sfft_bench_corr_flops(const sfft_plan *p, double *executed, double *tensor) {
+    if (!p || !executed || !tensor) return SFFT_ERR_INVALID_ARG;
+    double f = 0.0;
+    for (const sfft::CorrJob &j : p->jobs) {
+        int rows = 0;
+        for (int r = 0; r < j.nrange; ++r) rows += j.xend[r] - j.xbeg[r];
+        f += 2.0 * (j.nblk[0] + j.nblk[1]) * 2.0 * 512.0 * (rows / 4) * p->Nh;    // 2 row blocks x blocks x (Re, Im) per 4 rows per column
+    }
+    *executed = f; *tensor = f;
+    return SFFT_OK;
 }

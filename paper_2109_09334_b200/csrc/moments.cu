@@ -19,12 +19,6 @@ namespace {
 
 constexpr int BM = 64, BN = 64, BK = 16, LDS_ = BK + 4;   // smem row stride = 4 mod 16 doubles: conflict-free fragments
 
-__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-        : "+d"(c[0]), "+d"(c[1])
-        : "d"(a), "d"(b));
-}
-
 // grid: x = N tile, y = M tile, z = problem * ksplit + kpart.  block: 128 (2x2 warps of 32x32).
 template <bool BT>
 __global__ void __launch_bounds__(128) k_dgemm(GemmArgs g) {

@@ -236,12 +236,13 @@ void free_tables(sfft_plan *p) {
 }
 
 struct WsLayout {
-    size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, coefr, kfold, ctab, khat, flag, stR[2], stS[2], stD[2], stC[2], total;
+    size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, coefr, kfold, ctab, khat, flag, total;
 };
+struct StagingLayout { size_t stR[2], stS[2], stD[2], stC[2], total; };
 
 WsLayout ws_layout(const sfft_plan *p) {
     WsLayout l{};
-    size_t nb = p->nbatch, P = (size_t)p->H * p->W, n = p->n, off = 0;
+    size_t nb = p->nbatch, n = p->n, off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
     l.rhat = take(nb * p->nimg * (size_t)p->H * p->Nh * sizeof(double2));
     l.G = take(nb * p->Sx * (size_t)(p->Nh + 1) * p->E * sizeof(double2));
@@ -258,17 +259,34 @@ WsLayout ws_layout(const sfft_plan *p) {
     l.dscale = take(nb * n * sizeof(double));
     l.coefr = take(nb * n * sizeof(double));
     l.kfold = take(nb * (size_t)p->FK * p->L * p->L * sizeof(double));
-    l.ctab = take(nb * (size_t)p->H * p->L * p->LT * sizeof(double));
+    // only the subtract route the plan takes gets its table
+    l.ctab = take(subtract_use_fourier(p) ? 0 : nb * (size_t)p->H * p->L * p->LT * sizeof(double));
     l.khat = take(subtract_use_fourier(p) ? nb * (size_t)p->L * p->FK * p->Nh * sizeof(double2) : 0);
     l.flag = take(nb * sizeof(int) * 2);
+    l.total = off;
+    return l;
+}
+
+// staging area of the host-buffer entry points: two slots of (R, S, D, coefficients)
+StagingLayout staging_layout(const sfft_plan *p) {
+    StagingLayout l{};
+    size_t nb = p->nbatch, P = (size_t)p->H * p->W, off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
     for (int q = 0; q < 2; ++q) {
         l.stR[q] = take(nb * P * sizeof(double));
         l.stS[q] = take(nb * P * sizeof(double));
         l.stD[q] = take(nb * P * sizeof(double));
-        l.stC[q] = take(nb * n * sizeof(double));
+        l.stC[q] = take(nb * (size_t)p->n * sizeof(double));
     }
     l.total = off;
     return l;
+}
+
+// a plan is tied to the device it was created on
+bool wrong_device(const sfft_plan *p) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return true; }
+    return dev != p->device;
 }
 
 }  // namespace
@@ -287,6 +305,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
 
     sfft_plan *p = new (std::nothrow) sfft_plan();
     if (!p) return SFFT_ERR_INVALID_ARG;
+    if (cudaGetDevice(&p->device) != cudaSuccess) { cudaGetLastError(); delete p; return SFFT_ERR_CUDA; }
     p->H = H; p->W = W; p->L = L; p->w = (L - 1) / 2; p->DK = DK; p->DB = DB; p->basis = basis;
     p->Nh = W / 2;
     p->nKa = num_axis(basis, DK); p->nBa = num_axis(basis, DB);
@@ -409,6 +428,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
 int sfft_plan_set_batch(sfft_plan *p, int nbatch) {
     if (!p || nbatch < 1 || nbatch > 65535) return SFFT_ERR_INVALID_ARG;
     p->nbatch = nbatch; p->ws = nullptr; p->ws_bytes = 0; p->built = p->solved = false;
+    p->staging = nullptr; p->staging_bytes = 0;
     choose_split(p);
     return SFFT_OK;
 }
@@ -431,16 +451,6 @@ int sfft_plan_set_stream(sfft_plan *p, void *stream) {
 
 int sfft_plan_num_unknowns(const sfft_plan *p) { return p ? p->n : -1; }
 int sfft_plan_num_kernel_terms(const sfft_plan *p) { return p ? p->FK : -1; }
-double sfft_plan_corr_executed_flops(const sfft_plan *p) {
-    if (!p) return -1.0;
-    double f = 0.0;
-    for (const CorrJob &j : p->jobs) {
-        int rows = 0;
-        for (int r = 0; r < j.nrange; ++r) rows += j.xend[r] - j.xbeg[r];
-        f += 2.0 * (j.nblk[0] + j.nblk[1]) * 2.0 * 512.0 * (rows / 4) * p->Nh;    // 2 row blocks x blocks x (Re, Im) per 4 rows per column
-    }
-    return f;
-}
 int sfft_plan_num_background_terms(const sfft_plan *p) { return p ? p->FB : -1; }
 
 size_t sfft_plan_workspace_bytes(const sfft_plan *p) { return p ? ws_layout(p).total : 0; }
@@ -455,19 +465,37 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     p->Q = (double *)(b + l.Q); p->QS = (double *)(b + l.QS); p->LamC = (double *)(b + l.LamC); p->mu = (double *)(b + l.mu);
     p->M = (double *)(b + l.M); p->rhs = (double *)(b + l.rhs); p->Lf = (double *)(b + l.Lf); p->Winv = (double *)(b + l.Winv);
     p->dscale = (double *)(b + l.dscale); p->coefr = (double *)(b + l.coefr); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
+    p->built = p->solved = false;
+    p->rhat_from_build = false;
+    return SFFT_OK;
+}
+
+size_t sfft_plan_host_staging_bytes(const sfft_plan *p) { return p ? staging_layout(p).total : 0; }
+
+int sfft_plan_set_host_staging(sfft_plan *p, void *d_buf, size_t bytes) {
+    if (!p || !d_buf) return SFFT_ERR_INVALID_ARG;
+    StagingLayout l = staging_layout(p);
+    if (bytes < l.total || ((uintptr_t)d_buf & 255)) return SFFT_ERR_WORKSPACE;
+    char *b = (char *)d_buf;
+    p->staging = d_buf; p->staging_bytes = bytes;
     for (int q = 0; q < 2; ++q) {
         p->stageR[q] = (double *)(b + l.stR[q]); p->stageS[q] = (double *)(b + l.stS[q]);
         p->stageD[q] = (double *)(b + l.stD[q]); p->stageC[q] = (double *)(b + l.stC[q]);
     }
     p->host_slot = 0;
-    p->built = p->solved = false;
-    p->rhat_valid = false;
+    return SFFT_OK;
+}
+
+int sfft_plan_set_reuse_spectra(sfft_plan *p, int on) {
+    if (!p || (on != 0 && on != 1)) return SFFT_ERR_INVALID_ARG;
+    p->reuse_spectra = on;
     return SFFT_OK;
 }
 
 int sfft_build_system(sfft_plan *p, const double *d_R, const double *d_S) {
     if (!p || !d_R || !d_S) return SFFT_ERR_INVALID_ARG;
     if (!p->ws) return SFFT_ERR_WORKSPACE;
+    if (wrong_device(p)) return SFFT_ERR_STATE;
     p->built = p->solved = false;
     cudaError_t e = cudaMemsetAsync(p->flag, 0xff, sizeof(int) * 2 * p->nbatch, p->stream);  // -1 = no failure
     if (p->prof_steps > 0) p->prof_cur = p->prof_cur + 1;   // a build opens the next profiled step
@@ -488,7 +516,7 @@ int sfft_build_system(sfft_plan *p, const double *d_R, const double *d_S) {
         if (e == cudaSuccess) e = cudaEventRecord(p->ev_join, p->side);
     }
     if (e == cudaSuccess) e = launch_rowfft_forward(p, d_R, d_S);
-    p->rhat_src = d_R; p->rhat_valid = (e == cudaSuccess);
+    p->rhat_from_build = (e == cudaSuccess);
     prof_mark(p, 1);
     if (e == cudaSuccess) e = launch_corr(p);
     prof_mark(p, 2);
@@ -545,19 +573,19 @@ int sfft_get_system(const sfft_plan *p, const double **d_M, const double **d_rhs
     return SFFT_OK;
 }
 
-int sfft_get_lag_table(const sfft_plan *p, int which, const double **d_table, size_t *count) {
+int sfft_get_lag_table(const sfft_plan *p, int which, const double **d_table, size_t *count, size_t *batch_stride) {
     if (!p || which < 0 || which > 3) return SFFT_ERR_INVALID_ARG;
     if (!p->built) return SFFT_ERR_STATE;
-    if (p->nbatch != 1 && d_table) { /* tables of batch entry b start at b*tab_size; expose entry 0 */ }
     size_t off[5] = {p->off_om, p->off_th, p->off_la, p->off_de, p->tab_size};
     if (d_table) *d_table = p->tab + off[which];
     if (count) *count = off[which + 1] - off[which];
+    if (batch_stride) *batch_stride = p->tab_size;
     return SFFT_OK;
 }
 
 int sfft_solve(sfft_plan *p, double *d_coef) {
     if (!p || !d_coef) return SFFT_ERR_INVALID_ARG;
-    if (!p->built) return SFFT_ERR_STATE;
+    if (!p->built || wrong_device(p)) return SFFT_ERR_STATE;
     prof_mark(p, 6);
     cudaError_t e = launch_solve(p, d_coef);
     prof_mark(p, 7);
@@ -569,6 +597,7 @@ int sfft_solve(sfft_plan *p, double *d_coef) {
 int sfft_subtract(sfft_plan *p, const double *d_coef, const double *d_R, const double *d_S, double *d_D) {
     if (!p || !d_coef || !d_R || !d_S || !d_D) return SFFT_ERR_INVALID_ARG;
     if (!p->ws) return SFFT_ERR_WORKSPACE;
+    if (wrong_device(p)) return SFFT_ERR_STATE;
     prof_mark(p, 8);
     cudaError_t e = launch_subtract(p, d_coef, d_R, d_S, d_D);
     prof_mark(p, 10);
@@ -587,7 +616,7 @@ int sfft_plan_status(sfft_plan *p, int *info) {
     if (e != cudaSuccess) return fail_cuda(p, e);
     for (int b = 0; b < p->nbatch; ++b)
         if (h[2 * b] >= 0) {
-            if (info) *info = b * p->n + h[2 * b];
+            if (info) *info = b * p->ns + h[2 * b];
             return SFFT_ERR_NOT_SPD;
         }
     return SFFT_OK;
@@ -595,7 +624,8 @@ int sfft_plan_status(sfft_plan *p, int *info) {
 
 int sfft_run_host_async(sfft_plan *p, const double *h_R, const double *h_S, double *h_D, double *h_coef) {
     if (!p || !h_R || !h_S) return SFFT_ERR_INVALID_ARG;
-    if (!p->ws) return SFFT_ERR_WORKSPACE;
+    if (!p->ws || !p->staging) return SFFT_ERR_WORKSPACE;
+    if (wrong_device(p)) return SFFT_ERR_STATE;
     const int q = p->host_slot;
     p->host_slot ^= 1;
     const size_t img = (size_t)p->nbatch * p->H * p->W * sizeof(double);
@@ -610,7 +640,9 @@ int sfft_run_host_async(sfft_plan *p, const double *h_R, const double *h_S, doub
     if (e != cudaSuccess) return fail_cuda(p, e);
     int st = sfft_build_system(p, p->stageR[q], p->stageS[q]);
     if (st == SFFT_OK) st = sfft_solve(p, p->stageC[q]);
+    p->host_call = true;        // the subtract sees the very pair the build transformed: its spectra are reused
     if (st == SFFT_OK) st = sfft_subtract(p, p->stageC[q], p->stageR[q], p->stageS[q], p->stageD[q]);
+    p->host_call = false;
     if (st != SFFT_OK) return st;
     e = cudaEventRecord(p->ev_done[q], p->stream);
     // D2H on the other copy stream
@@ -668,6 +700,6 @@ const char *sfft_strerror(int s) {
 }
 
 const char *sfft_last_cuda_error(const sfft_plan *p) { return p ? p->cuda_err.c_str() : ""; }
-const char *sfft_version(void) { return "sfft_b200 0.1 (sm_100a)"; }
+const char *sfft_version(void) { return "sfft_b200 0.2 (sm_100a)"; }
 
 }  // extern "C"

@@ -10,6 +10,16 @@
 
 namespace sfft {
 
+#ifdef __CUDACC__
+// One FP64 tensor-core MMA (DMMA on sm_100a): C[8x8] += A[8x4] B[4x8].  Fragments: a = A[lane>>2][lane&3],
+// b = B[lane&3][lane>>2], c[q] = C[lane>>2][2*(lane&3) + q].
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c[0]), "+d"(c[1])
+        : "d"(a), "d"(b));
+}
+#endif
+
 constexpr int kProfMarks = 11;     // event marks per profiled step (see sfft_plan_profile_read)
 constexpr int kCorrCols = 2;       // spectrum columns (m) per CTA of the correlation kernel
 constexpr int kCorrNSlots = 8;     // N-side (shifted) sequence planes per correlation job: slots 0..7
@@ -98,8 +108,10 @@ struct sfft_plan {
     double *Q = nullptr, *QS = nullptr, *LamC = nullptr, *mu = nullptr;
     double *M = nullptr, *rhs = nullptr, *Lf = nullptr, *Winv = nullptr, *dscale = nullptr, *kfold = nullptr, *ctab = nullptr;
     double2 *khat = nullptr;                    // [b][L*FK][Nh] row spectra of the pixel kernels (Fourier-route subtract)
-    const double *rhat_src = nullptr;           // device buffer whose weighted row spectra rhat[0..nKa) currently holds
-    bool rhat_valid = false;
+    bool rhat_from_build = false;               // rhat[0..nKa) holds the spectra of the R given to the last build
+    int reuse_spectra = 0;                      // caller's promise (sfft_plan_set_reuse_spectra): subtract R == build R
+    bool host_call = false;                     // inside sfft_run_host*: build and subtract see the same staged pair
+    int device = 0;                             // CUDA device the plan was created on
     double *coefr = nullptr;                    // [b][ns] reduced solution (cpr) before expansion to the full layout
     // host-call staging: two slots so that the copies of one pair overlap the compute of another (sfft_run_host_async)
     double *stageR[2] = {nullptr, nullptr}, *stageS[2] = {nullptr, nullptr}, *stageD[2] = {nullptr, nullptr},
@@ -107,6 +119,7 @@ struct sfft_plan {
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;           // plan-owned copy streams
     cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
     int host_slot = 0;                                       // next staging slot (round robin)
+    void *staging = nullptr; size_t staging_bytes = 0;       // caller-owned staging buffer (sfft_plan_set_host_staging)
     int *flag = nullptr;
     cudaStream_t stream = nullptr;
     cudaStream_t side = nullptr;                // plan-owned stream: the moment stage (HBM bound) runs beside the

@@ -21,7 +21,9 @@
 //   3. Backward substitution L^T y = z by a thread-block cluster of 8 CTAs per system: the owner
 //      of diagonal block b forms y_b = W_b^T z_b (W_b = L_bb^-1 from the factorisation), broadcasts it
 //      through distributed shared memory, and every CTA updates the columns it owns.  c = D y.
-// A non-positive pivot writes its index to flag[2*b] (reported as SFFT_ERR_NOT_SPD).
+// A diagonal entry that is not positive and finite, or a pivot of the scaled matrix (unit diagonal) that is not
+// finite or lies below kPivotFloor * n (rounding-noise level of the assembled entries: the system is numerically
+// rank-deficient even where the noise happens to be positive), writes its index to flag[2*b] (SFFT_ERR_NOT_SPD).
 #include <cooperative_groups.h>
 
 #include <algorithm>
@@ -30,14 +32,6 @@
 
 namespace cg = cooperative_groups;
 
-// In-kernel phase timestamps for the development probe (compiled out of the library).
-#ifdef SFFT_PROBE
-__device__ long long g_probe[64 * 8];
-#define PROBE(k, i) do { if (blockIdx.x == 0 && threadIdx.x == 0) g_probe[(k) * 8 + (i)] = clock64(); } while (0)
-#else
-#define PROBE(k, i) do { } while (0)
-#endif
-
 namespace sfft {
 namespace {
 
@@ -45,18 +39,15 @@ constexpr int NB = 64;        // panel width = tile size
 constexpr int LDT = NB + 4;   // smem stride of MMA operand tiles (= 4 mod 16: conflict-free fragments)
 constexpr int LDX = NB + 1;   // smem stride of the factor / solve views (conflict-free row-per-thread access)
 constexpr int CS = 8;         // cluster size of the back substitution
+constexpr double kPivotFloor = 64.0 * 2.220446049250313e-16;   // x n: smallest pivot of the scaled matrix taken as non-zero
 
-__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-        : "+d"(c[0]), "+d"(c[1])
-        : "d"(a), "d"(b));
-}
+__device__ __forceinline__ bool pivot_ok(double p, double pmin) { return p > pmin && p < 1e300; }
 
 __global__ void k_scale_diag(const double *__restrict__ M, double *__restrict__ dscale, int *flag, int n) {
     int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
     if (i >= n) return;
     double d = M[((size_t)b * n + i) * n + i];
-    if (!(d > 0.0)) { atomicCAS(&flag[2 * b], -1, i); d = 1.0; }
+    if (!(d > 0.0 && d < 1e300)) { atomicCAS(&flag[2 * b], -1, i); d = 1.0; }
     dscale[(size_t)b * n + i] = rsqrt(d);
 }
 
@@ -193,7 +184,7 @@ __device__ __forceinline__ void mma_64_symlower_dispatch(const double *A, double
 // reads it (the back substitution uses W), and the other P CTAs of this launch - which may be scheduled
 // after this one has finished when the grid exceeds one wave - still read the unfactored block from Lf.
 __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double *colbuf, double *rowbuf, double *pivs,
-                                            double *rs, int nb, int *flag, int gidx0, bool store, double *Wg) {
+                                            double *rs, int nb, int *flag, int gidx0, bool store, double *Wg, double pmin) {
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
     double t[4][4], e[4][4];
 #pragma unroll
@@ -247,11 +238,11 @@ __device__ __forceinline__ void chol_inv_64(const double *Dg, double *Wt, double
         }
     }
     __syncthreads();       // Dg fully consumed (registers), pivs complete
-    if (store && tid < nb && !(pivs[tid] > 0.0)) {
+    if (store && tid < nb && !pivot_ok(pivs[tid], pmin)) {
         // first failing column of this block: the lowest index wins; an earlier block's failure (already in
         // the flag from a previous launch) is kept by the compare-and-swap on -1 only
         bool first = true;
-        for (int q = 0; q < tid; ++q) first = first && (pivs[q] > 0.0);
+        for (int q = 0; q < tid; ++q) first = first && pivot_ok(pivs[q], pmin);
         if (first) atomicCAS(flag, -1, gidx0 + tid);
     }
     if (tid < NB) rs[tid] = (tid < nb) ? rsqrt(pivs[tid]) : 1.0;
@@ -337,7 +328,6 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
         // ------------------------------ P: panel k ------------------------------
         const int r0 = j1 + bx * NB, nr = max(0, min(NB, n + 1 - r0));
         double accD[2][4][2], accX[2][4][2];
-        PROBE(k, 0);
 #pragma unroll
         for (int a = 0; a < 2; ++a)
 #pragma unroll
@@ -364,12 +354,10 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
             tile_store(T0, td);
             tile_store(T1, ts);
             __syncthreads();
-            PROBE(k, 5);
             mma_64_symlower_dispatch(T0, accD);
             mma_64(T1, T0, accX);
             __syncthreads();
         }
-        PROBE(k, 1);
         // strip values minus the look-ahead update -> factor view Dg (T0, stride LDX) and slab operand tile S (T1)
         double *Dg = T0, *St = T1;
 #pragma unroll
@@ -386,11 +374,9 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
                     St[r * LDT + cc] = xl ? xv[a][c][q] - accX[a][c][q] : 0.0;
                 }
         __syncthreads();
-        PROBE(k, 2);
         // factor the diagonal block and invert its factor; W replaces Dg in T0 as an MMA operand tile
         chol_inv_64(Dg, T0, colbuf, rowbuf, pivs, rs, nb, &flag[2 * b], j0, bx == 0,
-                    Winv + ((size_t)b * nblk + k) * NB * NB);
-        PROBE(k, 3);
+                    Winv + ((size_t)b * nblk + k) * NB * NB, kPivotFloor * n);
         if (nr <= 0) return;
         // slab solve X L11^T = S as the dense contraction X = S W^T
 #pragma unroll
@@ -409,7 +395,6 @@ __global__ void __launch_bounds__(256) k_chol_step(double *__restrict__ Lf, doub
                 if (cc + 1 < nb) *reinterpret_cast<double2 *>(dst) = make_double2(accX[a][c][0], accX[a][c][1]);
                 else if (cc < nb) dst[0] = accX[a][c][0];
             }
-        PROBE(k, 4);
         return;
     }
     bx -= nslab;

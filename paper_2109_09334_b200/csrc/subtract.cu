@@ -23,12 +23,6 @@
 namespace sfft {
 namespace {
 
-__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-        : "+d"(c[0]), "+d"(c[1])
-        : "d"(a), "d"(b));
-}
-
 __global__ void k_fold_coef(const double *__restrict__ coef, double *__restrict__ kfold, int n, int FK, int LL) {
     const int t = blockIdx.x, b = blockIdx.y, a0 = LL / 2;
     const double *c = coef + (size_t)b * n + (size_t)t * LL;

@@ -289,11 +289,12 @@ cudaError_t launch_subtract_fourier(sfft_plan *p, const double *d_coef, const do
     k_kernel_spectrum<<<dim3((p->Nh + 127) / 128, p->L * p->FK, p->nbatch), 128, 0, p->stream>>>(p->kfold, p->dt.twW, p->khat,
                                                                                               p->Nh, p->L, p->FK);
     p->launches++;
-    // row spectra of g_j R: reuse those of the last build when it transformed this very buffer
-    if (!(p->rhat_valid && p->rhat_src == dR)) {
+    // row spectra of g_j R: transformed again unless the caller promised that this R is the one the last
+    // build transformed (sfft_plan_set_reuse_spectra), or the call comes from sfft_run_host* (same staged pair)
+    if (!((p->reuse_spectra || p->host_call) && p->rhat_from_build)) {
         e = launch_rowfft_forward(p, dR, nullptr);
         if (e != cudaSuccess) return e;
-        p->rhat_src = dR; p->rhat_valid = true;
+        p->rhat_from_build = false;
     }
     prof_mark(p, 9);
     // x-ranges: whole waves of 2 CTAs per SM, each warp pays a halo of 2w + pad source rows

@@ -182,10 +182,43 @@ def make_pair(config, subfield=None, H=None, W=None, stars=None, seed=None, nois
     return Pair(R=R, S=S, H=H, W=W, L=L, DK=c["DK"], DB=c["DB"], basis=c["basis"], sigma=SIGMA_BKG, config=config)
 
 
-def make_batch(config=5, nbatch=None, H=None, W=None, stars=None):
-    """Config 5: stack of independent sub-field pairs, images [B][H][W]."""
+_WORKER = """
+import sys, numpy as np
+sys.path.insert(0, {root!r})
+import synth
+config, lo, hi, H, W, stars, out = {args!r}
+ps = [synth.make_pair(config, subfield=e, H=H, W=W, stars=stars) for e in range(lo, hi)]
+np.save(out + "_R.npy", np.stack([p.R for p in ps])); np.save(out + "_S.npy", np.stack([p.S for p in ps]))
+"""
+
+
+def make_batch(config=5, nbatch=None, H=None, W=None, stars=None, first=0, workers=0):
+    """Config 5: stack of independent sub-field pairs first .. first+nbatch-1, images [B][H][W].
+    workers > 1 renders slices of the batch in that many child interpreters (identical arrays: every
+    sub-field has its own seed); used by the full-size batch-of-64 test and bench only."""
     nb = CONFIGS[config]["batch"] if nbatch is None else nbatch
-    pairs = [make_pair(config, subfield=e, H=H, W=W, stars=stars) for e in range(nb)]
+    if workers > 1 and nb > 1:
+        import os
+        import subprocess
+        import sys
+        import tempfile
+        root = os.path.dirname(os.path.abspath(__file__))
+        nw = min(workers, nb)
+        cuts = [first + (nb * q) // nw for q in range(nw + 1)]
+        with tempfile.TemporaryDirectory() as tmp:
+            procs = []
+            for q in range(nw):
+                args = (config, cuts[q], cuts[q + 1], H, W, stars, os.path.join(tmp, f"part{q}"))
+                procs.append(subprocess.Popen([sys.executable, "-c", _WORKER.format(root=root, args=args)]))
+            for pr in procs:
+                if pr.wait() != 0:
+                    raise RuntimeError("synth.make_batch: a rendering child failed")
+            R = np.concatenate([np.load(os.path.join(tmp, f"part{q}_R.npy")) for q in range(nw)])
+            S = np.concatenate([np.load(os.path.join(tmp, f"part{q}_S.npy")) for q in range(nw)])
+        c = CONFIGS[config]
+        return Pair(R=R, S=S, H=R.shape[1], W=R.shape[2], L=c["L"], DK=c["DK"], DB=c["DB"], basis=c["basis"],
+                    sigma=SIGMA_BKG, config=config)
+    pairs = [make_pair(config, subfield=first + e, H=H, W=W, stars=stars) for e in range(nb)]
     p0 = pairs[0]
     return Pair(R=np.stack([p.R for p in pairs]), S=np.stack([p.S for p in pairs]), H=p0.H, W=p0.W, L=p0.L,
                 DK=p0.DK, DB=p0.DB, basis=p0.basis, sigma=p0.sigma, config=config)

@@ -61,7 +61,7 @@ def test_product_path_does_not_import_the_oracle():
 
 
 def test_generator_is_deterministic_and_shaped():
-    from paper_2109_09334_b200 import synth
+    import synth
     a, b = synth.make_pair(1), synth.make_pair(1)
     assert np.array_equal(a.R, b.R) and np.array_equal(a.S, b.S)
     assert a.R.shape == (128, 128) and (a.L, a.DK, a.DB, a.basis) == (7, 1, 1, "poly")
@@ -98,6 +98,16 @@ rank = dist.get_rank()
 lo, hi = bench.shard_units(5, rank, 2)            # 5 independent pairs over 2 ranks, no data-path collective
 mine = torch.zeros(5); mine[lo:hi] = 1.0
 dist.all_reduce(mine)                             # test-only: every unit owned exactly once
+# config 5 (batch of 64 sub-fields): contiguous slices of the batch axis per rank, strong scaling (SURVEY 8(e));
+# the sub-fields a rank renders are exactly those of the one-process batch at its slice
+import numpy as np, synth
+first, cnt, scaling = bench.rank_units(5, rank, 2)
+own = torch.zeros(64); own[first:first + cnt] = 1.0
+dist.all_reduce(own)
+assert scaling == "strong" and cnt == 32 and first == 32 * rank and torch.equal(own, torch.ones(64))
+assert bench.rank_units(4, rank, 2) == (rank, 1, "weak")
+part = synth.make_batch(5, nbatch=2, first=first, H=64, W=64)
+assert np.array_equal(part.R[1], synth.make_pair(5, subfield=first + 1, H=64, W=64).R)
 t = torch.tensor([1.0 + rank])                    # bench's max-over-ranks timing reduction
 dist.all_reduce(t, op=dist.ReduceOp.MAX)
 assert torch.equal(mine, torch.ones(5)) and t.item() == 2.0

@@ -318,6 +318,50 @@ def test_normal_equation_orthogonality_and_sampled_difference():
     np.testing.assert_allclose(oracle.difference_at(R, S, c, L, POLY, 1, 1, px, py), D[px, py], rtol=0, atol=1e-10)
 
 
+def _numpy_design(R, L, basis, DK, DB):
+    """Design matrix rebuilt with np.roll (Eqs. 3-4, 11), weights from closed forms (POLY) or scipy (BSPLINE)."""
+    H, W = R.shape
+    w = (L - 1) // 2
+    if basis == POLY:
+        TK, TB = _poly_T(H, W, DK), _poly_T(H, W, DB)
+    else:
+        def ax(N, m):
+            knots = np.r_[np.zeros(4), np.arange(1, m + 1) / (m + 1.0), np.ones(4)]
+            return scipy.interpolate.BSpline.design_matrix((np.arange(N) + 0.5) / N, knots, 3).toarray().T
+        fK, gK, fB, gB = ax(H, DK), ax(W, DK), ax(H, DB), ax(W, DB)
+        TK = [np.outer(fK[i], gK[j]) for i in range(DK + 4) for j in range(DK + 4)]
+        TB = [np.outer(fB[i], gB[j]) for i in range(DB + 4) for j in range(DB + 4)]
+    cols = []
+    for T in TK:
+        Rt = T * R
+        for al in range(-w, w + 1):
+            for be in range(-w, w + 1):
+                sh = np.roll(Rt, (al, be), axis=(0, 1))
+                cols.append((sh if (al, be) == (0, 0) else sh - Rt).ravel())
+    cols += [T.ravel() for T in TB]
+    return np.array(cols)
+
+
+@pytest.mark.parametrize("H,W,L,basis,DK,DB", [(20, 24, 5, POLY, 2, 1), (24, 20, 5, BSPL, 1, 0), (16, 16, 7, BSPL, 0, 1)])
+def test_difference_at_on_borders_and_diag_rhs_vs_numpy(H, W, L, basis, DK, DB):
+    """orc_difference_at (the sampled form the full-size configs rest on) against D = S - Phi^T c with Phi rebuilt
+    in numpy, at pixels whose kernel footprint wraps in x, in y and in both (all four corners), under both bases;
+    catches a wrong wrap direction, a transposed weight table or a missing centre correction.
+    orc_diag_and_rhs against the same Phi (catches a wrong shift sign or a dropped '- R^t' term)."""
+    R, S = _rand_pair(H, W, 21)
+    Phi = _numpy_design(R, L, basis, DK, DB)
+    rng = np.random.default_rng(22)
+    c = rng.standard_normal(Phi.shape[0])
+    D = (S.ravel() - c @ Phi).reshape(H, W)
+    px = np.array([0, 0, H - 1, H - 1, 1, H - 2, H // 2, 0, H - 1, 3])
+    py = np.array([0, W - 1, 0, W - 1, W - 2, 1, W // 2, W // 2, 2, 0])
+    np.testing.assert_allclose(oracle.difference_at(R, S, c, L, basis, DK, DB, px, py), D[px, py], rtol=0, atol=2e-10)
+    np.testing.assert_allclose(oracle.difference(R, S, c, L, basis, DK, DB), D, rtol=0, atol=2e-10)
+    diag, rhs = oracle.diag_and_rhs(R, S, L, basis, DK, DB)
+    np.testing.assert_allclose(diag, np.sum(Phi * Phi, axis=1), rtol=1e-12, atol=1e-9)
+    np.testing.assert_allclose(rhs, Phi @ S.ravel(), rtol=1e-12, atol=1e-7)
+
+
 def test_affine_coordinate_invariance_of_difference():
     """DESIGN g8: the total-degree polynomial space is affine invariant, so D fitted with raw pixel
     indices (the paper's T = x^p y^q) equals D fitted with normalised coordinates."""
