@@ -74,6 +74,13 @@ int sfft_plan_set_stream(sfft_plan *plan, void *cuda_stream);
 int sfft_plan_set_const_phot_ratio(sfft_plan *plan, int on);
 int sfft_plan_num_solved(const sfft_plan *plan);
 
+/* Route of the x-direction lag correlation (steps a3+a4): 0 = chosen by the plan (default), 1 = direct lag sums
+ * on the FP64 tensor cores, 2 = sectioned (overlap-save) correlation with 64-point FFTs along x, available for
+ * polynomial bases with at most 8 column sequences (F_K + 1 <= 8), SFFT_ERR_INVALID_ARG otherwise.  Both routes
+ * evaluate the same sums (App. B); the setter exists so that parity tests and benchmarks can
+ * run either on the same input.  Invalidates the workspace (call before sfft_plan_workspace_bytes). */
+int sfft_plan_set_corr_route(sfft_plan *plan, int route);
+
 /* n = F_K*L*L + F_B (Eq. 18's dimension), or -1 for a null plan. */
 int sfft_plan_num_unknowns(const sfft_plan *plan);
 int sfft_plan_num_kernel_terms(const sfft_plan *plan);     /* F_K */

@@ -17,7 +17,7 @@ SFFT_OK, SFFT_ERR_INVALID_ARG, SFFT_ERR_STATE, SFFT_ERR_WORKSPACE, SFFT_ERR_CUDA
 
 # every symbol include/sfft.h declares (checked against the built library by tests/test_abi_and_host.py)
 EXPORTS = [
-    "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
+    "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_set_corr_route", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
     "sfft_plan_num_kernel_terms", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
     "sfft_subtract", "sfft_plan_set_reuse_spectra", "sfft_plan_status", "sfft_plan_host_staging_bytes", "sfft_plan_set_host_staging",
@@ -58,6 +58,7 @@ def load_library(build_if_missing=True):
         "sfft_plan_set_batch": (ci, [vp, ci]),
         "sfft_plan_set_stream": (ci, [vp, vp]),
         "sfft_plan_set_const_phot_ratio": (ci, [vp, ci]),
+        "sfft_plan_set_corr_route": (ci, [vp, ci]),
         "sfft_plan_num_solved": (ci, [vp]),
         "sfft_plan_num_unknowns": (ci, [vp]),
         "sfft_plan_num_kernel_terms": (ci, [vp]),
@@ -117,6 +118,10 @@ def sfft_plan_set_stream(plan, stream_ptr):
 
 def sfft_plan_set_const_phot_ratio(plan, on):
     return load_library().sfft_plan_set_const_phot_ratio(plan, int(on))
+
+
+def sfft_plan_set_corr_route(plan, route):
+    return load_library().sfft_plan_set_corr_route(plan, int(route))
 
 
 def sfft_plan_num_solved(plan):
@@ -227,7 +232,7 @@ class Plan:
     """sfft_plan handle + workspace tensor on the current CUDA device and stream."""
 
     def __init__(self, H, W, L, DK, DB, basis="poly", nbatch=1, device="cuda:0", const_phot_ratio=False,
-                 reuse_spectra=False):
+                 reuse_spectra=False, corr_route=0):
         import torch
         if not torch.cuda.is_available():
             raise SfftError(SFFT_ERR_CUDA, "Plan", "no CUDA device: libsfft_b200 has no CPU fallback")
@@ -240,6 +245,8 @@ class Plan:
         self.H, self.W, self.L, self.nbatch = H, W, L, nbatch
         self._check(sfft_plan_set_batch(self.h, nbatch), "sfft_plan_set_batch")
         self._check(sfft_plan_set_const_phot_ratio(self.h, const_phot_ratio), "sfft_plan_set_const_phot_ratio")
+        if corr_route:
+            self._check(sfft_plan_set_corr_route(self.h, corr_route), "sfft_plan_set_corr_route")
         self.n = sfft_plan_num_unknowns(self.h)
         self.ns = sfft_plan_num_solved(self.h)
         self.ws_bytes = sfft_plan_workspace_bytes(self.h)

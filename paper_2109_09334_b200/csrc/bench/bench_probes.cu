@@ -3,6 +3,8 @@
 // FP64 FMA pipe (DFMA) and of the FP64 tensor-core path (mma.sync.m8n8k4.f64 -> DMMA) on this device,
 // the denominators of the "alu" rooflines in DESIGN.md.  Register-resident operands, 8 independent
 // accumulator chains per thread / warp, no memory traffic.
+#include <algorithm>
+
 #include "../sfft_internal.h"
 #include "sfft_bench.h"
 
@@ -77,6 +79,20 @@ extern "C" int sfft_bench_fp64_peak(int kind, double *tflops) {
 
 extern "C" int sfft_bench_corr_flops(const sfft_plan *p, double *executed, double *tensor) {
     if (!p || !executed || !tensor) return SFFT_ERR_INVALID_ARG;
+    if (p->corr_os) {
+        // sectioned kernel: per CTA (column slot, x-range part) steps of 4 hops, each 2 FFT64 per sequence and hop
+        // (5 N log2 N = 1920 flop) and 4 DMMA (512 flop) per frequency bin
+        const int HOP = p->os_hop, hops = (p->H + HOP - 1) / HOP, hpp = (hops + p->Sx - 1) / p->Sx;
+        double steps = 0.0;
+        for (int xs = 0; xs < p->Sx; ++xs) {
+            const int xb = std::min(p->H, xs * hpp * HOP), xe = std::min(p->H, xb + hpp * HOP);
+            steps += (xe - xb + 4 * HOP - 1) / (4 * HOP);
+        }
+        const double ctas = (double)(p->Nh + 1);
+        *tensor = ctas * steps * 64.0 * 4.0 * 512.0;
+        *executed = *tensor + ctas * steps * (p->nseq * 4.0 * 2.0 * 1920.0) + ctas * p->Sx * 64.0 * 1920.0;
+        return SFFT_OK;
+    }
     double f = 0.0;
     for (const sfft::CorrJob &j : p->jobs) {
         int rows = 0;

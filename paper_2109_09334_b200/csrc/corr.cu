@@ -235,6 +235,7 @@ cudaError_t launch_x(sfft_plan *p) {
 }  // namespace
 
 cudaError_t launch_corr(sfft_plan *p) {
+    if (corr_use_os(p)) return launch_corr_os(p);
     return (p->H / p->Sx) >= 64 ? launch_x<64>(p) : launch_x<32>(p);
 }
 

@@ -114,8 +114,18 @@ __device__ __forceinline__ void fft_core(double2 (&v)[16], double2 *buf, const d
     const int k2 = tid & 15;
 #pragma unroll
     for (int r = 0; r < 16; ++r) { const int i = tid + r * T; v[r] = buf[i + (i >> 4)]; }
-#pragma unroll
-    for (int r = 1; r < 16; ++r) v[r] = cmulf(v[r], tw2[r * 16 + k2]);
+    {
+        // twiddles exp(-2 pi i k2 r / 256) = w^r from ONE table read by a shallow product tree (depth 4): the kernels
+        // using this are bound by the shared-memory data pipe, not by FP64 issue, so 14 complex products are
+        // cheaper than 14 more 16-byte shared loads per thread
+        const double2 w1 = tw2[16 + k2], w2 = cmulf(w1, w1), w3 = cmulf(w2, w1), w4 = cmulf(w2, w2);
+        const double2 w5 = cmulf(w4, w1), w6 = cmulf(w4, w2), w7 = cmulf(w4, w3), w8 = cmulf(w4, w4);
+        v[1] = cmulf(v[1], w1); v[2] = cmulf(v[2], w2); v[3] = cmulf(v[3], w3); v[4] = cmulf(v[4], w4);
+        v[5] = cmulf(v[5], w5); v[6] = cmulf(v[6], w6); v[7] = cmulf(v[7], w7); v[8] = cmulf(v[8], w8);
+        v[9] = cmulf(v[9], cmulf(w8, w1)); v[10] = cmulf(v[10], cmulf(w8, w2)); v[11] = cmulf(v[11], cmulf(w8, w3));
+        v[12] = cmulf(v[12], cmulf(w8, w4)); v[13] = cmulf(v[13], cmulf(w8, w5)); v[14] = cmulf(v[14], cmulf(w8, w6));
+        v[15] = cmulf(v[15], cmulf(w8, w7));
+    }
     fft_reg<16>(v);
     __syncthreads();
 #pragma unroll

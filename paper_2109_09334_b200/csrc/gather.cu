@@ -96,6 +96,60 @@ __global__ void k_gather(const double *__restrict__ tab, const double *__restric
     }
 }
 
+// Kernel-kernel part of M for the unconstrained system, block by block: CTA (t, tb, chunk) fills kGatherRows rows of
+// the L^2 x L^2 block M[(tb, .)][(t, .)] from the Omega table of the pair (min, max)(tb, t) staged in shared memory
+// (one table read per CTA instead of four L2 reads per entry; rows leave in 256-byte runs).  Entries are formed from
+// the (lower, higher)-ordered unknown pair exactly as in m_entry, so M stays exactly symmetric.
+constexpr int kGatherRows = 32;
+__global__ void __launch_bounds__(256) k_gather_kk(const double *__restrict__ tab, double *__restrict__ M, GatherDims d,
+                                                   int nchunk) {
+    extern __shared__ double som[];                       // [nO][nO] Omega of the ordered pair, then int dec[LL]
+    int *dec = reinterpret_cast<int *>(som + d.nO * d.nO);
+    const int t = blockIdx.x, tb = blockIdx.y, b = blockIdx.z / nchunk, chunk = blockIdx.z - b * nchunk;
+    const int tlo = min(tb, t), thi = max(tb, t), pair = tlo * d.FK - tlo * (tlo - 1) / 2 + (thi - tlo);
+    const double *om = tab + (size_t)b * d.tab_size + d.off_om + (size_t)pair * d.nO * d.nO;
+    for (int i = threadIdx.x; i < d.nO * d.nO; i += 256) som[i] = __ldg(&om[i]);
+    for (int a = threadIdx.x; a < d.LL; a += 256) dec[a] = ((a / d.L - d.w) << 16) | ((a % d.L - d.w) & 0xffff);
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, c0 = (d.L - 1) * d.nO + (d.L - 1);   // index of lag (0,0)
+    const double o0 = som[c0];
+    const int r1 = min(d.LL, (chunk + 1) * kGatherRows);
+    for (int ab = chunk * kGatherRows + warp; ab < r1; ab += 8) {
+        const int kb = tb * d.LL + ab;
+        double *row = M + ((size_t)b * d.ns + kb) * d.ns + (size_t)t * d.LL;
+        for (int a = lane; a < d.LL; a += 32) {
+            const int k = t * d.LL + a;
+            // (first, second) = the unknowns in increasing index order
+            const int fa = kb <= k ? ab : a, sa = kb <= k ? a : ab;
+            const int df = dec[fa], ds = dec[sa];
+            const int alb = df >> 16, beb = (short)(df & 0xffff), al = ds >> 16, be = (short)(ds & 0xffff);
+            const bool cb = (alb == 0 && beb == 0), c = (al == 0 && be == 0);
+            double v;
+            if (cb && c) v = o0;
+            else if (c) v = som[c0 + alb * d.nO + beb] - o0;
+            else if (cb) v = som[c0 - al * d.nO - be] - o0;
+            else v = (som[c0 + (alb - al) * d.nO + (beb - be)] - som[c0 + alb * d.nO + beb]) - (som[c0 - al * d.nO - be] - o0);
+            row[a] = v;
+        }
+    }
+}
+
+// Background part of the unconstrained system: columns and rows of the F_B background unknowns (B7/B9, B11), and the
+// right-hand side (B13, B15).  thread = unknown i, blockIdx.y = background term s; both M[i][na+s] and M[na+s][i].
+__global__ void __launch_bounds__(128) k_gather_bg(const double *__restrict__ tab, const double *__restrict__ phi0,
+                                                   const int *__restrict__ kdec, double *__restrict__ M,
+                                                   double *__restrict__ rhs, GatherDims d) {
+    const int i = blockIdx.x * 128 + threadIdx.x, s = blockIdx.y, b = blockIdx.z;
+    if (i >= d.n) return;
+    const double *tb_ = tab + (size_t)b * d.tab_size;
+    const double *om = tb_ + d.off_om, *th = tb_ + d.off_th, *la = tb_ + d.off_la, *de = tb_ + d.off_de;
+    const int k = d.FK * d.LL + s;
+    const double v = m_entry(om, la, phi0, kdec, d, min(i, k), max(i, k));
+    M[((size_t)b * d.ns + i) * d.ns + k] = v;
+    M[((size_t)b * d.ns + k) * d.ns + i] = v;
+    if (s == 0) rhs[(size_t)b * d.ns + i] = rhs_entry(th, de, d, i);
+}
+
 // c = C c': reduced solution -> full coefficient layout (constrained centre entries filled in)
 __global__ void k_expand_coef(const double *__restrict__ cr, double *__restrict__ c, GatherDims d, int poly) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
@@ -123,6 +177,15 @@ static GatherDims gather_dims(const sfft_plan *p) {
 
 cudaError_t launch_gather(sfft_plan *p) {
     GatherDims d = gather_dims(p);
+    if (!p->cpr) {
+        const int nchunk = (d.LL + kGatherRows - 1) / kGatherRows;
+        const size_t smem = (size_t)d.nO * d.nO * sizeof(double) + (size_t)d.LL * sizeof(int);
+        k_gather_kk<<<dim3(p->FK, p->FK, p->nbatch * nchunk), 256, smem, p->stream>>>(p->tab, p->M, d, nchunk);
+        k_gather_bg<<<dim3((p->n + 127) / 128, p->FB, p->nbatch), 128, 0, p->stream>>>(p->tab, p->dt.phi0, p->dt.kdec, p->M,
+                                                                                     p->rhs, d);
+        p->launches += 2;
+        return cudaGetLastError();
+    }
     dim3 grid((p->ns + 127) / 128, p->ns, p->nbatch);
     k_gather<<<grid, 128, 0, p->stream>>>(p->tab, p->dt.phi0, p->dt.kdec, p->M, p->rhs, d);
     p->launches++;

@@ -97,6 +97,8 @@ void choose_split(sfft_plan *p) {
         double cost = ceil(T / slots) / sx * (1.0 + 0.02 * sx);     // mild penalty: G traffic grows with sx
         if (cost < best) { best = cost; p->Sx = sx; }
     }
+    p->corr_os = corr_use_os(p);
+    if (p->corr_os) { p->Sx = corr_os_split(p); p->os_hop = corr_os_hop(p); }
     // column chunks of the y-direction partial sums (lagsum.cu): enough CTAs to fill the machine
     p->lagchunk = kLagChunk;
     while (p->lagchunk > 8 && (long)((p->E + 127) / 128) * ((p->Nh + p->lagchunk) / p->lagchunk) * p->nbatch < 2 * 148)
@@ -442,6 +444,15 @@ int sfft_plan_set_const_phot_ratio(sfft_plan *p, int on) {
 }
 
 int sfft_plan_num_solved(const sfft_plan *p) { return p ? p->ns : -1; }
+
+int sfft_plan_set_corr_route(sfft_plan *p, int route) {
+    if (!p || route < 0 || route > 2) return SFFT_ERR_INVALID_ARG;
+    p->corr_route = route;
+    if (route == 2 && !corr_use_os(p)) { p->corr_route = 0; return SFFT_ERR_INVALID_ARG; }
+    p->ws = nullptr; p->ws_bytes = 0; p->built = p->solved = false;      // the workspace partition depends on the split
+    choose_split(p);
+    return SFFT_OK;
+}
 
 int sfft_plan_set_stream(sfft_plan *p, void *stream) {
     if (!p) return SFFT_ERR_INVALID_ARG;

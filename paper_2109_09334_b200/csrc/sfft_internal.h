@@ -79,6 +79,8 @@ struct DeviceTables {
 struct sfft_plan {
     int H = 0, W = 0, L = 0, w = 0, DK = 0, DB = 0, basis = 0, nbatch = 1;
     int FK = 0, FB = 0, nKa = 0, nBa = 0, n = 0, Nh = 0;
+    bool corr_os = false; int os_hop = 0;   // the build takes the sectioned correlation (set by choose_split), its hop length
+    int corr_route = 0;  // 0: chosen by the plan, 1: direct lag sums (corr.cu), 2: sectioned FFT64 correlation (corr_os.cu)
     int cpr = 0;         // constant photometric ratio: centre coefficients of the terms t >= 1 not free
     int ns = 0;          // solved unknowns: n, or n - (FK - 1) under cpr
     int nimg = 0;        // spectrum stack depth per batch entry: nKa weighted-y images + S
@@ -135,6 +137,10 @@ namespace sfft {
 // stage launchers (each returns cudaError_t of the launch); all enqueue on p->stream
 cudaError_t launch_rowfft_forward(sfft_plan *p, const double *dR, const double *dS);   // dS == nullptr: R rows only
 cudaError_t launch_corr(sfft_plan *p);
+bool corr_use_os(const sfft_plan *p);        // sectioned (overlap-save FFT64) lag correlation instead of direct lag sums
+int corr_os_split(const sfft_plan *p);       // its x-range parts
+int corr_os_hop(const sfft_plan *p);
+cudaError_t launch_corr_os(sfft_plan *p);
 cudaError_t launch_lagsum(sfft_plan *p);
 cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS);
 cudaError_t launch_gather(sfft_plan *p);

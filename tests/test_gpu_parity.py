@@ -40,12 +40,12 @@ def _check_coef(c, co, na):
     assert np.max(np.abs(c[na:] - co[na:])) <= TOL_C * np.max(np.abs(co[na:]))
 
 
-def _gpu_all(torch, p, L, basis, DK, DB, R=None, S=None):
+def _gpu_all(torch, p, L, basis, DK, DB, R=None, S=None, corr_route=0):
     R = p.R if R is None else R
     S = p.S if S is None else S
     nb = 1 if R.ndim == 2 else R.shape[0]
     H, W = R.shape[-2:]
-    plan = B.Plan(H, W, L, DK, DB, basis, nbatch=nb)
+    plan = B.Plan(H, W, L, DK, DB, basis, nbatch=nb, corr_route=corr_route)
     dR, dS = torch.from_numpy(np.ascontiguousarray(R)).cuda(), torch.from_numpy(np.ascontiguousarray(S)).cuda()
     plan.build_system(dR, dS)
     coef = plan.solve()
@@ -90,6 +90,48 @@ def test_parity_small(cuda_device, cfg, H, W, L, basis, DK, DB):
     M, rhs, c, D = _gpu_all(torch, p, L, basis, DK, DB)
     _check_system(M[0], rhs[0], Mo, ro, p.S)
     _check_coef(c[0], co, Mo.shape[0] - oracle.num_terms(_bid(basis), DB))
+    assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
+
+
+@pytest.mark.parametrize("cfg,H,W,L,DK,DB", [
+    (1, None, None, None, None, None),      # config 1
+    (3, 64, 256, 15, None, None),           # 29 lags on a small frame
+    (4, 256, 128, 17, None, None),          # L = 17: lag-0 block + two 8-lag blocks
+    (2, 128, 128, 9, 1, 2),
+    (2, 64, 64, 1, 2, 1),                   # L = 1
+])
+def test_parity_direct_corr_route(cuda_device, cfg, H, W, L, DK, DB):
+    """The polynomial cases take the sectioned FFT64 lag correlation by default; the direct tensor-core lag sums
+    (the route of the many-term bases) must give the same system on the same input (sfft_plan_set_corr_route)."""
+    import torch
+    p = synth.make_pair(cfg, H=H, W=W)
+    L = p.L if L is None else L
+    DK = p.DK if DK is None else DK
+    DB = p.DB if DB is None else DB
+    Mo, ro, co, Do = _oracle_all(p.R, p.S, L, "poly", DK, DB)
+    M, rhs, c, D = _gpu_all(torch, p, L, "poly", DK, DB, corr_route=1)
+    _check_system(M[0], rhs[0], Mo, ro, p.S)
+    _check_coef(c[0], co, Mo.shape[0] - oracle.num_terms(oracle.POLY, DB))
+    assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
+
+
+def test_parity_many_polynomial_terms_and_routes(cuda_device):
+    """DK = 3: 10 kernel terms + S = 11 column sequences -> beyond the sectioned kernel's 8, the plan falls back to
+    the direct lag sums by itself and refuses route 2; x-range splits of the sectioned route on a tall frame."""
+    import torch
+    p = synth.make_pair(2, H=128, W=128)
+    Mo, ro, co, Do = _oracle_all(p.R, p.S, 5, "poly", 3, 1)
+    M, rhs, c, D = _gpu_all(torch, p, 5, "poly", 3, 1)
+    _check_system(M[0], rhs[0], Mo, ro, p.S)
+    st, h = B.sfft_plan_create(128, 128, 5, 3, 1, 0)
+    assert st == B.SFFT_OK and B.sfft_plan_set_corr_route(h, 2) == B.SFFT_ERR_INVALID_ARG
+    assert B.sfft_plan_set_corr_route(h, 1) == B.SFFT_OK and B.sfft_plan_set_corr_route(h, 3) == B.SFFT_ERR_INVALID_ARG
+    B.sfft_plan_destroy(h)
+    p = synth.make_pair(2, H=2048, W=64)                       # few columns, many rows: the x axis is split in parts
+    Mo, ro, co, Do = _oracle_all(p.R, p.S, 7, "poly", 2, 2)
+    M, rhs, c, D = _gpu_all(torch, p, 7, "poly", 2, 2, corr_route=2)
+    _check_system(M[0], rhs[0], Mo, ro, p.S)
+    _check_coef(c[0], co, Mo.shape[0] - 6)
     assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
 
 
