@@ -17,13 +17,14 @@
 // a dense contraction with K = hops, run on the FP64 tensor cores (mma.sync.m8n8k4.f64, K = 4 hops per step):
 //   Re ACC += Pr^T Qr + Pi^T Qi,   Im ACC += Pr^T Qi - Pi^T Qr        (4 DMMA per bin per 4 hops).
 //
-// CTA = 16 warps, one spectrum column, warp specialised:
-//   warps 0..7  (producers): warp s owns sequence s, its four 8-lane groups own the 4 hops of a step; each group
-//               runs the P and Q transforms of its (sequence, hop) in registers (radix 8 x 8, one padded
-//               shared-memory exchange) and writes the spectra in MMA fragment order [bin][sequence][hop];
-//   warps 8..15 (consumers): warp j owns bins 8j..8j+7 and keeps their ACC (Re, Im: 8 x 8 each) in registers;
-//   two spectrum buffers, named barriers full[2] / empty[2]; the raw column values and x-weights of the next step
-//   are fetched with cp.async while the current one is transformed.
+// CTA = 16 warps, one spectrum column, one barrier per step of 4 hops:
+//   transform phase: warp w < 2 nseq owns the Q (w even) or P (w odd) transforms of sequence w/2, its four 8-lane
+//                    groups the 4 hops; a group runs its 64-point transform in registers (radix 8 x 8) and does the
+//                    one exchange IN PLACE in the 64 spectrum slots it is about to fill (skewed, conflict-free),
+//                    then writes the spectrum in MMA fragment order [bin][sequence][hop];
+//   MMA phase:       warp j owns bins 4j..4j+3 and keeps their ACC (Re, Im: 8 x 8 each) in registers.
+// Spectra are double buffered, so warps that finish their MMAs start the next step's transforms at once; the raw
+// column values and x-weights are fetched two steps ahead with cp.async.
 // The packed DC/Nyquist slot (column 0 holds (X[0], X[W/2]), both real) is run as two real columns (grid.x = Nh+1).
 #include "fft_regs.cuh"
 #include "sfft_internal.h"
@@ -32,49 +33,86 @@ namespace sfft {
 namespace {
 
 constexpr int kOsHops = 4;                       // hops per step = K of one DMMA
-constexpr int kOsBinStride = 36;                 // double2 per bin of a spectrum buffer: 8 seq x 4 hops + 4 pad
+constexpr int kOsBinStride = 33;                 // double2 per bin of a spectrum buffer: 8 seq x 4 hops + 1 (odd: conflict-free)
 constexpr int kOsSpec = 64 * kOsBinStride;       // double2 per spectrum buffer (P or Q)
-constexpr int kOsEx = 72;                        // double2 per FFT group exchange buffer (8 x 9, padded)
-constexpr int kOsMaxImg = 4, kOsMaxXw = 3;
+constexpr int kOsEx = 72;                        // double2 per exchange buffer of the final inverse transforms (8 x 9)
+constexpr int kOsMaxImg = 4, kOsMaxXw = 3;     // images of the spectrum stack; x-weight powers u^0 .. u^2
 
-struct OsDims { int H, Nh, nimg, nKa, nseq, L, E, Sx, HOP, RS; };
+#ifdef SFFT_OS_PROBE
+__device__ long long g_osp[16 * 8];
+#define OSP(i) do { if (blockIdx.x == 700 && s == 10 && (threadIdx.x & 31) == 0) g_osp[(threadIdx.x >> 5) * 8 + (i)] = clock64(); } while (0)
+#else
+#define OSP(i) do { } while (0)
+#endif
 
-__device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-__device__ __forceinline__ void bar_arrive(int id, int n) {
-    __threadfence_block();
-    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory");
-}
+struct OsDims { int H, Nh, nimg, nseq, L, E, Sx, HOP, RS; };
 
 // 64-point forward DFT by a group of 8 lanes (t = lane & 7).  In: v[r] = x[t + 8 r].  Out: v[k2] = X[t + 8 k2].
-// ex: the group's exchange buffer (kOsEx entries); tw[k1] = exp(-2 pi i t k1 / 64).
-__device__ __forceinline__ void fft64_group(double2 (&v)[8], double2 *ex, const double2 *tw, int t) {
+// ex(i): the group's 64 exchange slots; tw[k1] = exp(-2 pi i t k1 / 64).  The slot of Y_t[k1] is skewed by k1 so
+// that both the stores (lanes = t) and the loads (lanes = k1) of a quarter warp fall in eight different 16-byte banks
+// whatever (odd) stride the slots have.
+template <class Slot>
+__device__ __forceinline__ void fft64_group(double2 (&v)[8], Slot ex, const double2 *tw, int t) {
     fft_reg<8>(v);                                            // Y_t[k1] = sum_r x[t + 8r] w8^(r k1)
 #pragma unroll
     for (int k1 = 1; k1 < 8; ++k1) v[k1] = cmulf(v[k1], tw[k1]);
 #pragma unroll
-    for (int k1 = 0; k1 < 8; ++k1) ex[t * 9 + k1] = v[k1];
+    for (int k1 = 0; k1 < 8; ++k1) *ex(k1 * 8 + ((t + k1) & 7)) = v[k1];
     __syncwarp();
 #pragma unroll
-    for (int tt = 0; tt < 8; ++tt) v[tt] = ex[tt * 9 + t];    // lane k1 = t gathers Y_tt[k1] w64^(tt k1)
+    for (int tt = 0; tt < 8; ++tt) v[tt] = *ex(t * 8 + ((tt + t) & 7));    // lane k1 = t gathers Y_tt[k1] w64^(tt k1)
     __syncwarp();
     fft_reg<8>(v);                                            // X[k1 + 8 k2] = sum_tt (.) w8^(tt k2)
 }
 
+// Transform phase of one step for one lane: rows t + 8r of the hop starting at staged row r0 (image row x0).
+//   MODE : 0 complex column, 1 DC part (.x) and 2 Nyquist part (.y) of the packed column 0, run as real columns
+//   SIDE : 0 = Q (64-row window), 1 = P (only the nkeep first rows, the rest of the window zero)
+//   XP   : power of the x-weight f_i(x) = u_x^i, u_x = (2x+1)/H - 1 (exact in double; DESIGN g8).  Computed here
+//          instead of read from the plan's table: u is exact and u*u is its correctly rounded square, which is
+//          what the table holds, so both routes weight with the very same numbers (a1).
+template <int MODE, int SIDE, int XP>
+__device__ __forceinline__ void os_transform(const double2 *rw, double2 *dst, const double2 *tw, int t, int nkeep, int x0,
+                                             int hmask, double uscale, double uoff) {
+    double2 v[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        double2 a = rw[t + 8 * r];
+        if (MODE == 1) a.y = 0.0;
+        if (MODE == 2) { a.x = a.y; a.y = 0.0; }
+        if (XP > 0) {
+            const double u = fma((double)((x0 + t + 8 * r) & hmask), uscale, uoff), w = XP == 1 ? u : u * u;
+            a.x *= w;
+            if (MODE == 0) a.y *= w;
+        }
+        if (SIDE == 1 && t + 8 * r >= nkeep) a = make_double2(0.0, 0.0);
+        v[r] = a;
+    }
+    fft64_group(v, [dst](int i) { return dst + i * kOsBinStride; }, tw, t);
+#pragma unroll
+    for (int k2 = 0; k2 < 8; ++k2) dst[(t + 8 * k2) * kOsBinStride] = v[k2];
+}
+
+template <int MODE, int SIDE>
+__device__ __forceinline__ void os_transform_xp(int xp, const double2 *rw, double2 *dst, const double2 *tw, int t, int nkeep,
+                                                int x0, int hmask, double uscale, double uoff) {
+    if (xp <= 0) os_transform<MODE, SIDE, 0>(rw, dst, tw, t, nkeep, x0, hmask, uscale, uoff);
+    else if (xp == 1) os_transform<MODE, SIDE, 1>(rw, dst, tw, t, nkeep, x0, hmask, uscale, uoff);
+    else os_transform<MODE, SIDE, 2>(rw, dst, tw, t, nkeep, x0, hmask, uscale, uoff);
+}
+
 // grid: x = column slot c (0: DC of packed column 0, Nh: its Nyquist part, else column c), y = x-range part, z = batch
-__global__ void __launch_bounds__(512, 1)
-k_corr_os(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const Seq *__restrict__ seqs,
-          double2 *__restrict__ G, OsDims d) {
-    extern __shared__ double2 smo[];
-    double2 *SP = smo;                                   // [2][64][36]  spectra of the zero-padded hops (conj side)
-    double2 *SQ = smo + 2 * kOsSpec;                     // [2][64][36]  spectra of the 64-row windows
+template <int MODE>
+__device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, const Seq *__restrict__ seqs,
+                                             double2 *__restrict__ G, const OsDims &d, double2 *smo) {
+    double2 *SQ = smo;                                   // [2][64][33]  spectra of the 64-row windows
+    double2 *SP = smo + 2 * kOsSpec;                     // [2][64][33]  spectra of the zero-padded hops (conj side)
     double2 *raw = smo + 4 * kOsSpec;                    // [2][nimg][RS] column values of the staged rows
-    double2 *exb = raw + 2 * kOsMaxImg * d.RS;           // [8 warps][4 groups][72]
-    double *wts = reinterpret_cast<double *>(exb + 8 * 4 * kOsEx);   // [2][nKa][RS] x-weights of the staged rows
     __shared__ double2 tw64[64];
     __shared__ Seq sseq[8];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int c = blockIdx.x, xs = blockIdx.y, bz = blockIdx.z;
-    const int mode = (c == 0) ? 1 : (c == d.Nh ? 2 : 0), col = (c == d.Nh) ? 0 : c;
+    const int col = (MODE == 2) ? 0 : c;
     const int H = d.H, HOP = d.HOP, RS = d.RS, STEP = kOsHops * d.HOP;
 
     if (tid < 64) {
@@ -89,122 +127,115 @@ k_corr_os(const double2 *__restrict__ rhat, const double *__restrict__ xwt, cons
     const int xb = min(H, xs * hpp * HOP), xe = min(H, xb + hpp * HOP);
     const int nsteps = (xe - xb + STEP - 1) / STEP;
     const double2 *rb = rhat + (size_t)bz * d.nimg * H * d.Nh + col;
+
+    // The staged rows are fetched by all threads, one or two 16-byte items each (a warp keeps only a few scattered
+    // cp.async in flight: two dedicated fetch warps took 3700 cycles per step to issue the 832 items)
+    constexpr int npf = 512;
+    const int img0 = tid / RS, rr0 = tid - img0 * RS;
+    auto prefetch = [&](int s) {
+        const int x0 = xb + s * STEP;
+        double2 *rbuf = raw + (s & 1) * kOsMaxImg * RS;
+        for (int img = img0, r = rr0; img < d.nimg;) {
+            const int x = (x0 + r) & (H - 1);
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(&rbuf[img * RS + r]);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(&rb[((size_t)img * H + x) * d.Nh]));
+            r += npf;
+            while (r >= RS) { r -= RS; ++img; }
+        }
+    };
+    if (nsteps > 0) prefetch(0);
+    if (nsteps > 1) prefetch(1);
+    asm volatile("cp.async.commit_group;");
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
 
-    if (warp < 8) {
-        // ------------------------------------------------ producers ------------------------------------------------
-        const int hop = lane >> 3, t = lane & 7, seq = warp;
-        double2 *ex = exb + (warp * 4 + hop) * kOsEx;
-        const bool live = seq < d.nseq;
-        const Seq sq = live ? sseq[seq] : Seq{0, -1};
-        double2 tw[8];
+    // transform role: sequence, side (0: Q = 64-row window, 1: P = zero-padded hop), hop, lane of the group
+    const int seq = warp >> 1, side = warp & 1, hop = lane >> 3, t = lane & 7;
+    const bool live = seq < d.nseq;
+    const Seq sq = live ? sseq[seq] : Seq{0, -1};
+    const double uscale = 2.0 / H, uoff = 1.0 / H - 1.0;
+    double2 tw[8];
 #pragma unroll
-        for (int k1 = 0; k1 < 8; ++k1) tw[k1] = tw64[(t * k1) & 63];
-        auto prefetch = [&](int s) {
-            const int x0 = xb + s * STEP, b = s & 1;
-            for (int i = tid; i < d.nimg * RS; i += 256) {
-                const int img = i / RS, r = i - img * RS, x = (x0 + r) & (H - 1);
-                const unsigned dst = (unsigned)__cvta_generic_to_shared(&raw[(b * kOsMaxImg + img) * RS + r]);
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(&rb[((size_t)img * H + x) * d.Nh]));
-            }
-            for (int i = tid; i < d.nKa * RS; i += 256) {
-                const int f = i / RS, r = i - f * RS, x = (x0 + r) & (H - 1);
-                const unsigned dst = (unsigned)__cvta_generic_to_shared(&wts[(b * kOsMaxXw + f) * RS + r]);
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(&xwt[(size_t)f * H + x]));
-            }
-            asm volatile("cp.async.commit_group;");
-        };
-        if (nsteps > 0) prefetch(0);
-        for (int s = 0; s < nsteps; ++s) {
-            const int b = s & 1;
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
-            bar_sync(5, 256);                              // raw[b] of every producer thread landed; step s-1 fully read
-            if (s + 1 < nsteps) prefetch(s + 1);
-            if (s >= 2) bar_sync(3 + b, 512);              // empty[b]: the consumers are done with the spectra of step s-2
-            if (live) {
-                const int r0 = hop * HOP;
-                const double2 *rw = raw + (b * kOsMaxImg + sq.img) * RS + r0;
-                const double *wt = wts + (b * kOsMaxXw + (sq.xw >= 0 ? sq.xw : 0)) * RS + r0;
-                double2 v[8], q[8];
+    for (int k1 = 0; k1 < 8; ++k1) tw[k1] = tw64[(t * k1) & 63];
+    double are[4][2], aim[4][2];
 #pragma unroll
-                for (int r = 0; r < 8; ++r) {
-                    double2 a = rw[t + 8 * r];
-                    if (mode == 1) a.y = 0.0;
-                    else if (mode == 2) { a.x = a.y; a.y = 0.0; }
-                    if (sq.xw >= 0) { const double w = wt[t + 8 * r]; a.x *= w; a.y *= w; }
-                    q[r] = a;
-                    // the conj side keeps only the HOP rows of this hop that lie inside the CTA's x-range
-                    const bool keep = (t + 8 * r < HOP) && (xb + s * STEP + r0 + t + 8 * r < xe);
-                    v[r] = keep ? a : make_double2(0.0, 0.0);
-                }
-                fft64_group(q, ex, tw, t);
-                double2 *dq = SQ + b * kOsSpec + seq * 4 + hop;
-#pragma unroll
-                for (int k2 = 0; k2 < 8; ++k2) dq[(t + 8 * k2) * kOsBinStride] = q[k2];
-                fft64_group(v, ex, tw, t);
-                double2 *dp = SP + b * kOsSpec + seq * 4 + hop;
-#pragma unroll
-                for (int k2 = 0; k2 < 8; ++k2) dp[(t + 8 * k2) * kOsBinStride] = v[k2];
-            }
-            bar_arrive(1 + b, 512);                        // full[b]
+    for (int i = 0; i < 4; ++i) are[i][0] = are[i][1] = aim[i][0] = aim[i][1] = 0.0;
+
+    for (int s = 0; s < nsteps; ++s) {
+        const int b = s & 1;
+        OSP(0);
+        if (live) {
+            const int r0 = hop * HOP, x0 = xb + s * STEP + r0;
+            const double2 *rw = raw + (b * kOsMaxImg + sq.img) * RS + r0;
+            double2 *dst = (side ? SP : SQ) + b * kOsSpec + seq * 4 + hop;
+            // the conj side keeps only the HOP rows of this hop that lie inside the CTA's x-range
+            if (side) os_transform_xp<MODE, 1>(sq.xw, rw, dst, tw, t, min(HOP, xe - x0), x0, H - 1, uscale, uoff);
+            else os_transform_xp<MODE, 0>(sq.xw, rw, dst, tw, t, 64, x0, H - 1, uscale, uoff);
         }
-    } else {
-        // ------------------------------------------------ consumers ------------------------------------------------
-        const int j = warp - 8;
-        double are[8][2], aim[8][2];
+        OSP(1);
+        asm volatile("cp.async.wait_group 0;" ::: "memory");      // the rows of step s+1 (fetched during step s-1) landed
+        OSP(2);
+        __syncthreads();                                           // spectra of step s complete; raw[b] and S[b^1] free
+        OSP(3);
+        if (s + 2 < nsteps) prefetch(s + 2);
+        asm volatile("cp.async.commit_group;");
+        OSP(4);
+        const double2 *sp = SP + b * kOsSpec + (4 * warp) * kOsBinStride + lane;
+        const double2 *sq2 = SQ + b * kOsSpec + (4 * warp) * kOsBinStride + lane;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) are[i][0] = are[i][1] = aim[i][0] = aim[i][1] = 0.0;
-        for (int s = 0; s < nsteps; ++s) {
-            const int b = s & 1;
-            bar_sync(1 + b, 512);                          // full[b]
-            const double2 *sp = SP + b * kOsSpec + (8 * j) * kOsBinStride + lane;
-            const double2 *sq2 = SQ + b * kOsSpec + (8 * j) * kOsBinStride + lane;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const double2 p = sp[i * kOsBinStride], q = sq2[i * kOsBinStride];
-                dmma884(are[i], p.x, q.x);
-                dmma884(are[i], p.y, q.y);
-                dmma884(aim[i], p.x, q.y);
-                dmma884(aim[i], -p.y, q.x);
-            }
-            if (s + 2 < nsteps) bar_arrive(3 + b, 512);    // empty[b]
+        for (int i = 0; i < 4; ++i) {
+            const double2 p = sp[i * kOsBinStride], q = sq2[i * kOsBinStride];
+            dmma884(are[i], p.x, q.x);
+            dmma884(are[i], p.y, q.y);
+            dmma884(aim[i], p.x, q.y);
+            dmma884(aim[i], -p.y, q.x);
         }
-        // ACC -> shared, [q*8 + p][bin] with a padded pair stride, over the spectrum buffers: the producers wrote
-        // them for the last time before the last full[] barrier; every consumer must have read its last operands
-        bar_sync(6, 256);
+        OSP(5);
+    }
+    // ACC -> shared, [q*8 + p][bin] with a padded pair stride, over the spectrum buffers
+    __syncthreads();
+    {
         double2 *accs = smo;
         const int p = lane >> 2, q0 = 2 * (lane & 3);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            accs[(q0 * 8 + p) * 65 + 8 * j + i] = make_double2(are[i][0], aim[i][0]);
-            accs[((q0 + 1) * 8 + p) * 65 + 8 * j + i] = make_double2(are[i][1], aim[i][1]);
+        for (int i = 0; i < 4; ++i) {
+            accs[(q0 * 8 + p) * 65 + 4 * warp + i] = make_double2(are[i][0], aim[i][0]);
+            accs[((q0 + 1) * 8 + p) * 65 + 4 * warp + i] = make_double2(are[i][1], aim[i][1]);
         }
     }
     __syncthreads();
     // ---- inverse 64-point transform of every pair's ACC, stored at the lags rho < L:  G = conj(FFT(conj ACC)) / 64 ----
     {
-        const int g = tid >> 3, t = tid & 7, q = g >> 3, p = g & 7;
-        double2 *ex2 = smo + 64 * 65 + g * kOsEx;
-        double2 tw[8];
-#pragma unroll
-        for (int k1 = 0; k1 < 8; ++k1) tw[k1] = tw64[(t * k1) & 63];
+        const int g = tid >> 3, q = g >> 3, p = g & 7;
+        double2 *ex2 = smo + 64 * 65 + g * kOsEx;          // past the ACC copy (runs on into the raw staging area)
         double2 v[8];
 #pragma unroll
         for (int r = 0; r < 8; ++r) { const double2 a = smo[g * 65 + t + 8 * r]; v[r] = make_double2(a.x, -a.y); }
-        fft64_group(v, ex2, tw, t);
+        fft64_group(v, [ex2](int i) { return ex2 + i + (i >> 3); }, tw, t);
         if (p < d.nseq && q < d.nseq) {
             double2 *Gm = G + (((size_t)bz * d.Sx + xs) * (d.Nh + 1) + c) * d.E + (size_t)(p * d.nseq + q) * d.L;
 #pragma unroll
             for (int k2 = 0; k2 < 8; ++k2) {
                 const int rho = t + 8 * k2;
-                if (rho < d.L) Gm[rho] = make_double2(v[k2].x * (1.0 / 64.0), mode ? 0.0 : -v[k2].y * (1.0 / 64.0));
+                if (rho < d.L) Gm[rho] = make_double2(v[k2].x * (1.0 / 64.0), MODE ? 0.0 : -v[k2].y * (1.0 / 64.0));
             }
         }
     }
 }
 
+__global__ void __launch_bounds__(512, 1)
+k_corr_os(const double2 *__restrict__ rhat, const Seq *__restrict__ seqs, double2 *__restrict__ G, OsDims d) {
+    extern __shared__ double2 smo[];
+    const int c = blockIdx.x;                            // uniform per CTA
+    if (c == 0) corr_os_body<1>(rhat, seqs, G, d, smo);
+    else if (c == d.Nh) corr_os_body<2>(rhat, seqs, G, d, smo);
+    else corr_os_body<0>(rhat, seqs, G, d, smo);
+}
+
 size_t corr_os_smem(const OsDims &d) {
-    return (size_t)(4 * kOsSpec + 2 * kOsMaxImg * d.RS + 8 * 4 * kOsEx) * sizeof(double2) + (size_t)2 * kOsMaxXw * d.RS * sizeof(double);
+    const size_t main_loop = (size_t)(4 * kOsSpec + 2 * kOsMaxImg * d.RS) * sizeof(double2);
+    const size_t epilogue = (size_t)(64 * 65 + 64 * kOsEx) * sizeof(double2);      // ACC copy + 64 exchange buffers
+    return main_loop > epilogue ? main_loop : epilogue;
 }
 
 }  // namespace
@@ -233,15 +264,21 @@ int corr_os_split(const sfft_plan *p) {
 }
 
 cudaError_t launch_corr_os(sfft_plan *p) {
-    OsDims d{p->H, p->Nh, p->nimg, p->nKa, p->nseq, p->L, p->E, p->Sx, corr_os_hop(p), 0};
+    OsDims d{p->H, p->Nh, p->nimg, p->nseq, p->L, p->E, p->Sx, corr_os_hop(p), 0};
     d.RS = (kOsHops - 1) * d.HOP + 64;
     const size_t smem = corr_os_smem(d);
     cudaError_t e = cudaFuncSetAttribute(k_corr_os, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid(p->Nh + 1, p->Sx, p->nbatch);
-    k_corr_os<<<grid, 512, smem, p->stream>>>(p->rhat, p->dt.xwt, p->dt.seqs, p->G, d);
+    k_corr_os<<<grid, 512, smem, p->stream>>>(p->rhat, p->dt.seqs, p->G, d);
     p->launches++;
     return cudaGetLastError();
 }
 
 }  // namespace sfft
+
+#ifdef SFFT_OS_PROBE
+extern "C" int sfft_os_probe_read(long long *out) {
+    return (int)cudaMemcpyFromSymbol(out, sfft::g_osp, sizeof(long long) * 16 * 8);
+}
+#endif
