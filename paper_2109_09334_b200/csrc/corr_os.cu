@@ -24,7 +24,8 @@
 //                    then writes the spectrum in MMA fragment order [bin][sequence][hop];
 //   MMA phase:       warp j owns bins 4j..4j+3 and keeps their ACC (Re, Im: 8 x 8 each) in registers.
 // Spectra are double buffered, so warps that finish their MMAs start the next step's transforms at once; the raw
-// column values and x-weights are fetched two steps ahead with cp.async.
+// column values are fetched two steps ahead with cp.async (by all threads: a warp keeps only a few scattered copies
+// in flight); the polynomial x-weights are computed in registers.
 // The packed DC/Nyquist slot (column 0 holds (X[0], X[W/2]), both real) is run as two real columns (grid.x = Nh+1).
 #include "fft_regs.cuh"
 #include "sfft_internal.h"
@@ -37,13 +38,6 @@ constexpr int kOsBinStride = 33;                 // double2 per bin of a spectru
 constexpr int kOsSpec = 64 * kOsBinStride;       // double2 per spectrum buffer (P or Q)
 constexpr int kOsEx = 72;                        // double2 per exchange buffer of the final inverse transforms (8 x 9)
 constexpr int kOsMaxImg = 4, kOsMaxXw = 3;     // images of the spectrum stack; x-weight powers u^0 .. u^2
-
-#ifdef SFFT_OS_PROBE
-__device__ long long g_osp[16 * 8];
-#define OSP(i) do { if (blockIdx.x == 700 && s == 10 && (threadIdx.x & 31) == 0) g_osp[(threadIdx.x >> 5) * 8 + (i)] = clock64(); } while (0)
-#else
-#define OSP(i) do { } while (0)
-#endif
 
 struct OsDims { int H, Nh, nimg, nseq, L, E, Sx, HOP, RS; };
 
@@ -163,7 +157,6 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
 
     for (int s = 0; s < nsteps; ++s) {
         const int b = s & 1;
-        OSP(0);
         if (live) {
             const int r0 = hop * HOP, x0 = xb + s * STEP + r0;
             const double2 *rw = raw + (b * kOsMaxImg + sq.img) * RS + r0;
@@ -172,14 +165,10 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
             if (side) os_transform_xp<MODE, 1>(sq.xw, rw, dst, tw, t, min(HOP, xe - x0), x0, H - 1, uscale, uoff);
             else os_transform_xp<MODE, 0>(sq.xw, rw, dst, tw, t, 64, x0, H - 1, uscale, uoff);
         }
-        OSP(1);
         asm volatile("cp.async.wait_group 0;" ::: "memory");      // the rows of step s+1 (fetched during step s-1) landed
-        OSP(2);
         __syncthreads();                                           // spectra of step s complete; raw[b] and S[b^1] free
-        OSP(3);
         if (s + 2 < nsteps) prefetch(s + 2);
         asm volatile("cp.async.commit_group;");
-        OSP(4);
         const double2 *sp = SP + b * kOsSpec + (4 * warp) * kOsBinStride + lane;
         const double2 *sq2 = SQ + b * kOsSpec + (4 * warp) * kOsBinStride + lane;
 #pragma unroll
@@ -190,7 +179,6 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
             dmma884(aim[i], p.x, q.y);
             dmma884(aim[i], -p.y, q.x);
         }
-        OSP(5);
     }
     // ACC -> shared, [q*8 + p][bin] with a padded pair stride, over the spectrum buffers
     __syncthreads();
@@ -277,8 +265,3 @@ cudaError_t launch_corr_os(sfft_plan *p) {
 
 }  // namespace sfft
 
-#ifdef SFFT_OS_PROBE
-extern "C" int sfft_os_probe_read(long long *out) {
-    return (int)cudaMemcpyFromSymbol(out, sfft::g_osp, sizeof(long long) * 16 * 8);
-}
-#endif
