@@ -53,6 +53,9 @@ def _load():
     L.orc_corr_diff_one.restype = ctypes.c_double
     L.orc_weighted_ref.argtypes = [_ci] * 5 + [_D, _D]
     L.orc_num_threads.restype = _ci
+    L.orc_mask_fill.argtypes = [_ci, _ci, _D, _D, ctypes.c_double, ctypes.c_double, _ci, _ci, _D, _D,
+                                np.ctypeslib.ndpointer(dtype=np.uint8, flags="C_CONTIGUOUS")]
+    L.orc_mask_fill.restype = ctypes.c_long
     L.orc_cpr_num_unknowns.argtypes = [_ci] * 4
     L.orc_cpr_constrain.argtypes = [_ci] * 4 + [_D] * 4
     L.orc_cpr_expand.argtypes = [_ci] * 4 + [_D] * 2
@@ -221,3 +224,13 @@ def cpr_expand(cr, L, basis, DK, DB):
     c = np.zeros(num_unknowns(L, basis, DK, DB))
     _load().orc_cpr_expand(L, basis, DK, DB, cr, c)
     return c
+
+
+def mask_fill(R, S, sat_R, sat_S, rd, rb):
+    """NEXT-2 (DESIGN g21): joint saturation mask grown by rd, masked pixels replaced by the mean of the
+    unmasked pixels in the (2 rb + 1)^2 neighbourhood.  Returns (Rm, Sm, mask uint8)."""
+    R, S = _c(R), _c(S)
+    H, W = R.shape
+    Rm, Sm, mask = np.zeros((H, W)), np.zeros((H, W)), np.zeros((H, W), np.uint8)
+    _load().orc_mask_fill(H, W, R, S, float(sat_R), float(sat_S), int(rd), int(rb), Rm, Sm, mask)
+    return Rm, Sm, mask

@@ -573,3 +573,52 @@ int orc_num_threads(void) {
     return 1;
 #endif
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * NEXT-2: crowded-flavor preprocessing.  "The crowded-flavor SFFT will automatically mask the
+ * pixels affected by the saturated sources in the field and replace them with the neighboring background."
+ * The paper fixes neither the mask growth nor the background estimate; reading DESIGN g21:
+ *   seed(x,y)  = R(x,y) >= sat_R  or  S(x,y) >= sat_S                 (one joint mask for the pair)
+ *   mask(x,y)  = 1 iff some seed lies within Chebyshev distance rd     (square (2 rd + 1)^2 window)
+ *   fill       : every masked pixel of an image <- mean of the UNMASKED pixels of that image inside the square
+ *                (2 rb + 1)^2 window centred on it; if that window holds no unmasked pixel, the mean of all
+ *                unmasked pixels of the image; unmasked pixels are copied.
+ * Indices wrap around (the method is circular everywhere, DESIGN g12).  Plain loops, the definition itself.
+ * Returns the number of masked pixels. */
+long orc_mask_fill(int H, int W, const double *R, const double *S, double sat_R, double sat_S, int rd, int rb,
+                   double *Rm, double *Sm, unsigned char *mask) {
+    size_t P = (size_t)H * W;
+    long nmask = 0;
+    for (int x = 0; x < H; ++x)
+        for (int y = 0; y < W; ++y) {
+            int m = 0;
+            for (int dx = -rd; dx <= rd && !m; ++dx)
+                for (int dy = -rd; dy <= rd; ++dy) {
+                    size_t q = (size_t)wrap(x + dx, H) * W + wrap(y + dy, W);
+                    if (R[q] >= sat_R || S[q] >= sat_S) { m = 1; break; }
+                }
+            mask[(size_t)x * W + y] = (unsigned char)m;
+            nmask += m;
+        }
+    const double *src[2] = {R, S};
+    double *dst[2] = {Rm, Sm};
+    for (int im = 0; im < 2; ++im) {
+        long double gs = 0.0L; long gc = 0;
+        for (size_t p = 0; p < P; ++p) if (!mask[p]) { gs += src[im][p]; ++gc; }
+        double gmean = gc > 0 ? (double)(gs / gc) : 0.0;
+#pragma omp parallel for schedule(dynamic, 8)
+        for (int x = 0; x < H; ++x)
+            for (int y = 0; y < W; ++y) {
+                size_t p = (size_t)x * W + y;
+                if (!mask[p]) { dst[im][p] = src[im][p]; continue; }
+                long double s = 0.0L; long c = 0;
+                for (int dx = -rb; dx <= rb; ++dx)
+                    for (int dy = -rb; dy <= rb; ++dy) {
+                        size_t q = (size_t)wrap(x + dx, H) * W + wrap(y + dy, W);
+                        if (!mask[q]) { s += src[im][q]; ++c; }
+                    }
+                dst[im][p] = c > 0 ? (double)(s / c) : gmean;
+            }
+    }
+    return nmask;
+}

@@ -449,3 +449,71 @@ def test_cpr_recovers_constant_scale_with_varying_kernel():
     assert abs(cr[a0] - 1.25) <= 1e-9
     c = oracle.cpr_expand(cr, L, POLY, DK, DB)
     assert np.max(np.abs(oracle.difference(R, S, c, L, POLY, DK, DB))) <= 1e-8
+
+
+# --------------------------------------------------------------------------- NEXT-2: crowded-flavor mask + fill
+
+def _saturated_pair(H, W, seed, sat=600.0):
+    rng = np.random.default_rng(seed)
+    R = 100.0 + 20.0 * rng.random((H, W))
+    S = 110.0 + 20.0 * rng.random((H, W))
+    for (x, y, a) in [(5, 7, 900.0), (H - 1, 0, 1500.0), (H // 2, W - 1, 700.0)]:      # two of them wrap around the frame
+        R[x, y] = a
+    S[3, W // 2] = 2000.0
+    S[5, 7] = 650.0
+    return R, S, sat
+
+
+def test_mask_fill_golden_9x9():
+    """Hand-computed example (tests/golden/mask_fill_9x9.txt, DESIGN g21): catches a wrong window size,
+    masked pixels leaking into the mean, or a transposed axis."""
+    x, y = np.meshgrid(np.arange(9.0), np.arange(9.0), indexing="ij")
+    I = x + 10.0 * y
+    I[4, 4] = 1000.0
+    Rm, Sm, mask = oracle.mask_fill(I, np.zeros_like(I), 500.0, 500.0, 1, 2)
+    expect = np.zeros((9, 9), np.uint8); expect[3:6, 3:6] = 1
+    assert np.array_equal(mask, expect)
+    golden = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "mask_fill_9x9.txt")
+    rows = [ln.split() for ln in open(golden) if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 5
+    for gx, gy, val in rows:
+        assert abs(Rm[int(gx), int(gy)] - float(val)) < 1e-12
+    assert np.array_equal(Rm[mask == 0], I[mask == 0]) and np.array_equal(Sm[mask == 0], 0 * I[mask == 0])
+
+
+@pytest.mark.parametrize("rd,rb", [(0, 1), (1, 3), (2, 5)])
+def test_mask_fill_vs_scipy_filters_and_invariants(rd, rb):
+    """mask = wrap-around maximum filter of the thresholded seed (library routine); fill = ratio of two wrap-around
+    box filters (library routine); mask contains the thresholded set; filled values lie inside the range of the
+    unmasked neighbourhood; an unsaturated pair comes back untouched (idempotence)."""
+    H, W = 24, 20
+    R, S, sat = _saturated_pair(H, W, 31)
+    Rm, Sm, mask = oracle.mask_fill(R, S, sat, sat, rd, rb)
+    seed = ((R >= sat) | (S >= sat)).astype(np.uint8)
+    ref_mask = scipy.ndimage.maximum_filter(seed, size=2 * rd + 1, mode="wrap")
+    assert np.array_equal(mask, ref_mask) and np.all(mask[seed == 1] == 1)
+    keep = 1.0 - mask
+    for I, Im in ((R, Rm), (S, Sm)):
+        num = scipy.ndimage.uniform_filter(I * keep, size=2 * rb + 1, mode="wrap")
+        den = scipy.ndimage.uniform_filter(keep, size=2 * rb + 1, mode="wrap")
+        assert den[mask == 1].min() > 0
+        np.testing.assert_allclose(Im[mask == 1], (num / den)[mask == 1], rtol=1e-12)
+        assert np.array_equal(Im[mask == 0], I[mask == 0])
+        lo = scipy.ndimage.minimum_filter(np.where(mask == 1, np.inf, I), size=2 * rb + 1, mode="wrap")
+        hi = scipy.ndimage.maximum_filter(np.where(mask == 1, -np.inf, I), size=2 * rb + 1, mode="wrap")
+        assert np.all(Im[mask == 1] >= lo[mask == 1] - 1e-12) and np.all(Im[mask == 1] <= hi[mask == 1] + 1e-12)
+    R2, S2, m2 = oracle.mask_fill(Rm, Sm, sat, sat, rd, rb)          # nothing saturated any more
+    assert m2.sum() == 0 and np.array_equal(R2, Rm) and np.array_equal(S2, Sm)
+
+
+def test_mask_fill_empty_window_falls_back_to_global_mean():
+    """A saturated blob larger than the fill window: pixels whose window holds no unmasked pixel take the mean of all
+    unmasked pixels of the image."""
+    H = W = 16
+    R = 50.0 + np.arange(H * W, dtype=np.float64).reshape(H, W) % 7
+    S = R + 1.0
+    R[4:12, 4:12] = 1e4
+    Rm, Sm, mask = oracle.mask_fill(R, S, 1e3, 1e3, 0, 1)
+    assert mask.sum() == 64
+    np.testing.assert_allclose(Rm[7, 7], R[mask == 0].mean(), rtol=1e-13)
+    np.testing.assert_allclose(Sm[8, 8], S[mask == 0].mean(), rtol=1e-13)
