@@ -141,6 +141,17 @@ int sfft_subtract(sfft_plan *plan, const double *d_coef, const double *d_R, cons
  * The host-buffer entry points below fit and apply on the same staged pair and always reuse. */
 int sfft_plan_set_reuse_spectra(sfft_plan *plan, int on);
 
+/* NEXT-2, crowded-flavor preprocessing (reading DESIGN g21): build the masked pair the fit runs on.
+ *   seed = d_R >= sat_R or d_S >= sat_S (one joint mask for the pair), mask = seed grown by rd pixels (square
+ *   (2 rd + 1)^2 window), every masked pixel of an image replaced by the mean of that image's unmasked pixels in the
+ *   (2 rb + 1)^2 window around it (by the mean of all its unmasked pixels if that window holds none), unmasked pixels
+ *   copied; indices wrap around.  d_Rm, d_Sm: [nbatch][H][W] double, may alias d_R, d_S (in place); d_mask:
+ *   [nbatch][H][W] unsigned char, 1 = masked.  0 <= rd <= 64, 1 <= rb <= 128.  Needs the workspace (its spectrum
+ *   area is used as scratch, so call it before sfft_build_system, not between build and subtract).
+ * The paper's flow is then sfft_build_system(d_Rm, d_Sm) -> sfft_solve -> sfft_subtract(d_R, d_S). */
+int sfft_mask_fill(sfft_plan *plan, const double *d_R, const double *d_S, double sat_R, double sat_S, int rd, int rb,
+                   double *d_Rm, double *d_Sm, unsigned char *d_mask);
+
 /* Synchronise the plan's stream and report numerical status.  On SFFT_ERR_NOT_SPD, *info =
  * batch*ns + index of the first failing pivot in the order of the solved system (ns =
  * sfft_plan_num_solved(): the reduced layout under the constant photometric ratio); otherwise
@@ -166,6 +177,14 @@ int sfft_run_host(sfft_plan *plan, const double *h_R, const double *h_S, double 
  * sfft_run_host_wait returns.  sfft_run_host_wait drains everything submitted and reports like sfft_plan_status. */
 int sfft_run_host_async(sfft_plan *plan, const double *h_R, const double *h_S, double *h_D, double *h_coef);
 int sfft_run_host_wait(sfft_plan *plan);
+
+/* NEXT-4, FP32 storage / FP64 arithmetic: the same end-to-end calls with images stored as float on the host
+ * (h_R, h_S in, h_D out: [nbatch][H][W] float; h_coef stays double).  The images are widened to double on the
+ * device (exact), every step of the path computes in FP64 as before, and D is rounded to float once, on the way
+ * out.  Halves the bytes crossing PCIe per pair.  Same staging buffer, ordering and waiting rules as the double
+ * versions (sfft_run_host_wait drains both kinds). */
+int sfft_run_host_f32(sfft_plan *plan, const float *h_R, const float *h_S, float *h_D, double *h_coef);
+int sfft_run_host_async_f32(sfft_plan *plan, const float *h_R, const float *h_S, float *h_D, double *h_coef);
 
 /* Per-stage device timing.  sfft_plan_profile(plan, nsteps) with nsteps > 0 makes the next nsteps
  * build/solve/subtract rounds record CUDA events on the plan's stream around each stage (no host

@@ -20,8 +20,8 @@ EXPORTS = [
     "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_set_corr_route", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
     "sfft_plan_num_kernel_terms", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
-    "sfft_subtract", "sfft_plan_set_reuse_spectra", "sfft_plan_status", "sfft_plan_host_staging_bytes", "sfft_plan_set_host_staging",
-    "sfft_run_host", "sfft_run_host_async", "sfft_run_host_wait", "sfft_plan_launch_count", "sfft_plan_destroy",
+    "sfft_subtract", "sfft_mask_fill", "sfft_plan_set_reuse_spectra", "sfft_plan_status", "sfft_plan_host_staging_bytes", "sfft_plan_set_host_staging",
+    "sfft_run_host", "sfft_run_host_async", "sfft_run_host_wait", "sfft_run_host_f32", "sfft_run_host_async_f32", "sfft_plan_launch_count", "sfft_plan_destroy",
     "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
 ]
 SFFT_NUM_STAGES = 8
@@ -70,6 +70,7 @@ def load_library(build_if_missing=True):
         "sfft_get_lag_table": (ci, [vp, ci, pvp, ctypes.POINTER(cs), ctypes.POINTER(cs)]),
         "sfft_solve": (ci, [vp, vp]),
         "sfft_subtract": (ci, [vp, vp, vp, vp, vp]),
+        "sfft_mask_fill": (ci, [vp, vp, vp, ctypes.c_double, ctypes.c_double, ci, ci, vp, vp, vp]),
         "sfft_plan_set_reuse_spectra": (ci, [vp, ci]),
         "sfft_plan_status": (ci, [vp, pci]),
         "sfft_plan_host_staging_bytes": (cs, [vp]),
@@ -77,6 +78,8 @@ def load_library(build_if_missing=True):
         "sfft_run_host": (ci, [vp, vp, vp, vp, vp]),
         "sfft_run_host_async": (ci, [vp, vp, vp, vp, vp]),
         "sfft_run_host_wait": (ci, [vp]),
+        "sfft_run_host_f32": (ci, [vp, vp, vp, vp, vp]),
+        "sfft_run_host_async_f32": (ci, [vp, vp, vp, vp, vp]),
         "sfft_plan_launch_count": (ctypes.c_long, [vp]),
         "sfft_plan_destroy": (None, [vp]),
         "sfft_strerror": (ctypes.c_char_p, [ci]),
@@ -165,6 +168,12 @@ def sfft_subtract(plan, d_coef, d_R, d_S, d_D):
                                         ctypes.c_void_p(d_D))
 
 
+def sfft_mask_fill(plan, d_R, d_S, sat_R, sat_S, rd, rb, d_Rm, d_Sm, d_mask):
+    return load_library().sfft_mask_fill(plan, ctypes.c_void_p(d_R), ctypes.c_void_p(d_S), float(sat_R), float(sat_S),
+                                         int(rd), int(rb), ctypes.c_void_p(d_Rm), ctypes.c_void_p(d_Sm),
+                                         ctypes.c_void_p(d_mask))
+
+
 def sfft_plan_set_reuse_spectra(plan, on):
     return load_library().sfft_plan_set_reuse_spectra(plan, int(on))
 
@@ -191,6 +200,16 @@ def sfft_run_host(plan, h_R, h_S, h_D, h_coef):
 def sfft_run_host_async(plan, h_R, h_S, h_D, h_coef):
     return load_library().sfft_run_host_async(plan, ctypes.c_void_p(h_R), ctypes.c_void_p(h_S), ctypes.c_void_p(h_D),
                                               ctypes.c_void_p(h_coef))
+
+
+def sfft_run_host_f32(plan, h_R, h_S, h_D, h_coef):
+    return load_library().sfft_run_host_f32(plan, ctypes.c_void_p(h_R), ctypes.c_void_p(h_S), ctypes.c_void_p(h_D),
+                                            ctypes.c_void_p(h_coef))
+
+
+def sfft_run_host_async_f32(plan, h_R, h_S, h_D, h_coef):
+    return load_library().sfft_run_host_async_f32(plan, ctypes.c_void_p(h_R), ctypes.c_void_p(h_S), ctypes.c_void_p(h_D),
+                                                  ctypes.c_void_p(h_coef))
 
 
 def sfft_run_host_wait(plan):
@@ -299,6 +318,15 @@ class Plan:
         self._check(sfft_subtract(self.h, coef.data_ptr(), self._img(R), self._img(S), self._img(D)), "sfft_subtract")
         return D
 
+    def mask_fill(self, R, S, sat_R, sat_S, rd, rb, inplace=False):
+        """NEXT-2: masked pair (Rm, Sm) and the uint8 mask."""
+        torch = self.torch
+        Rm, Sm = (R, S) if inplace else (torch.empty_like(R), torch.empty_like(S))
+        mask = torch.empty(R.shape, dtype=torch.uint8, device=self.device)
+        self._check(sfft_mask_fill(self.h, self._img(R), self._img(S), sat_R, sat_S, rd, rb, Rm.data_ptr(), Sm.data_ptr(),
+                                   mask.data_ptr()), "sfft_mask_fill")
+        return Rm, Sm, mask
+
     def status(self, check=True):
         st, info = sfft_plan_status(self.h)
         if check and st != SFFT_OK:
@@ -326,6 +354,11 @@ class Plan:
         self.ensure_host_staging()
         D = np.empty_like(R_host)
         coef = np.empty((self.nbatch, self.n))
+        if R_host.dtype == np.float32:        # FP32 storage, FP64 arithmetic
+            assert S_host.dtype == np.float32
+            st = sfft_run_host_f32(self.h, R_host.ctypes.data, S_host.ctypes.data, D.ctypes.data, coef.ctypes.data)
+            self._check(st, "sfft_run_host_f32")
+            return D, coef
         st = sfft_run_host(self.h, R_host.ctypes.data, S_host.ctypes.data, D.ctypes.data, coef.ctypes.data)
         self._check(st, "sfft_run_host")
         return D, coef

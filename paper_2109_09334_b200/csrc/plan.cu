@@ -240,7 +240,7 @@ void free_tables(sfft_plan *p) {
 struct WsLayout {
     size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, coefr, kfold, ctab, khat, flag, total;
 };
-struct StagingLayout { size_t stR[2], stS[2], stD[2], stC[2], total; };
+struct StagingLayout { size_t stR[2], stS[2], stD[2], stC[2], stR32[2], stS32[2], stD32[2], total; };
 
 WsLayout ws_layout(const sfft_plan *p) {
     WsLayout l{};
@@ -279,6 +279,9 @@ StagingLayout staging_layout(const sfft_plan *p) {
         l.stS[q] = take(nb * P * sizeof(double));
         l.stD[q] = take(nb * P * sizeof(double));
         l.stC[q] = take(nb * (size_t)p->n * sizeof(double));
+        l.stR32[q] = take(nb * P * sizeof(float));          // FP32-storage entry points
+        l.stS32[q] = take(nb * P * sizeof(float));
+        l.stD32[q] = take(nb * P * sizeof(float));
     }
     l.total = off;
     return l;
@@ -492,6 +495,8 @@ int sfft_plan_set_host_staging(sfft_plan *p, void *d_buf, size_t bytes) {
     for (int q = 0; q < 2; ++q) {
         p->stageR[q] = (double *)(b + l.stR[q]); p->stageS[q] = (double *)(b + l.stS[q]);
         p->stageD[q] = (double *)(b + l.stD[q]); p->stageC[q] = (double *)(b + l.stC[q]);
+        p->stageR32[q] = (float *)(b + l.stR32[q]); p->stageS32[q] = (float *)(b + l.stS32[q]);
+        p->stageD32[q] = (float *)(b + l.stD32[q]);
     }
     p->host_slot = 0;
     return SFFT_OK;
@@ -616,6 +621,18 @@ int sfft_subtract(sfft_plan *p, const double *d_coef, const double *d_R, const d
     return SFFT_OK;
 }
 
+int sfft_mask_fill(sfft_plan *p, const double *d_R, const double *d_S, double sat_R, double sat_S, int rd, int rb,
+                   double *d_Rm, double *d_Sm, unsigned char *d_mask) {
+    if (!p || !d_R || !d_S || !d_Rm || !d_Sm || !d_mask) return SFFT_ERR_INVALID_ARG;
+    if (rd < 0 || rd > 64 || rb < 1 || rb > 128 || !(sat_R == sat_R) || !(sat_S == sat_S)) return SFFT_ERR_INVALID_ARG;
+    if (!p->ws) return SFFT_ERR_WORKSPACE;
+    if (wrong_device(p)) return SFFT_ERR_STATE;
+    p->rhat_from_build = false;                 // the spectrum area is used as scratch
+    cudaError_t e = launch_mask_fill(p, d_R, d_S, sat_R, sat_S, rd, rb, d_Rm, d_Sm, d_mask);
+    if (e != cudaSuccess) return fail_cuda(p, e);
+    return SFFT_OK;
+}
+
 int sfft_plan_status(sfft_plan *p, int *info) {
     if (info) *info = -1;
     if (!p) return SFFT_ERR_INVALID_ARG;
@@ -633,21 +650,25 @@ int sfft_plan_status(sfft_plan *p, int *info) {
     return SFFT_OK;
 }
 
-int sfft_run_host_async(sfft_plan *p, const double *h_R, const double *h_S, double *h_D, double *h_coef) {
+// Common body of the host-buffer entry points; f32 = images stored as float on the host.
+static int run_host_async_any(sfft_plan *p, const void *h_R, const void *h_S, void *h_D, double *h_coef, bool f32) {
     if (!p || !h_R || !h_S) return SFFT_ERR_INVALID_ARG;
     if (!p->ws || !p->staging) return SFFT_ERR_WORKSPACE;
     if (wrong_device(p)) return SFFT_ERR_STATE;
     const int q = p->host_slot;
     p->host_slot ^= 1;
-    const size_t img = (size_t)p->nbatch * p->H * p->W * sizeof(double);
+    const size_t npix = (size_t)p->nbatch * p->H * p->W;
+    const size_t img = npix * (f32 ? sizeof(float) : sizeof(double));
     // H2D on the copy stream, after the previous user of this slot (two calls ago) has finished computing
     cudaError_t e = cudaStreamWaitEvent(p->s_h2d, p->ev_done[q], 0);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(p->stageR[q], h_R, img, cudaMemcpyHostToDevice, p->s_h2d);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(p->stageS[q], h_S, img, cudaMemcpyHostToDevice, p->s_h2d);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(f32 ? (void *)p->stageR32[q] : (void *)p->stageR[q], h_R, img, cudaMemcpyHostToDevice, p->s_h2d);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(f32 ? (void *)p->stageS32[q] : (void *)p->stageS[q], h_S, img, cudaMemcpyHostToDevice, p->s_h2d);
     if (e == cudaSuccess) e = cudaEventRecord(p->ev_in[q], p->s_h2d);
     // compute on the plan's stream once the inputs are in and the slot's previous result has left
     if (e == cudaSuccess) e = cudaStreamWaitEvent(p->stream, p->ev_in[q], 0);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(p->stream, p->ev_out[q], 0);
+    if (f32 && e == cudaSuccess) e = launch_widen(p, p->stageR32[q], p->stageR[q], npix);
+    if (f32 && e == cudaSuccess) e = launch_widen(p, p->stageS32[q], p->stageS[q], npix);
     if (e != cudaSuccess) return fail_cuda(p, e);
     int st = sfft_build_system(p, p->stageR[q], p->stageS[q]);
     if (st == SFFT_OK) st = sfft_solve(p, p->stageC[q]);
@@ -655,15 +676,29 @@ int sfft_run_host_async(sfft_plan *p, const double *h_R, const double *h_S, doub
     if (st == SFFT_OK) st = sfft_subtract(p, p->stageC[q], p->stageR[q], p->stageS[q], p->stageD[q]);
     p->host_call = false;
     if (st != SFFT_OK) return st;
-    e = cudaEventRecord(p->ev_done[q], p->stream);
+    e = (f32 && h_D) ? launch_narrow(p, p->stageD[q], p->stageD32[q], npix) : cudaSuccess;
+    if (e == cudaSuccess) e = cudaEventRecord(p->ev_done[q], p->stream);
     // D2H on the other copy stream
     if (e == cudaSuccess) e = cudaStreamWaitEvent(p->s_d2h, p->ev_done[q], 0);
-    if (e == cudaSuccess && h_D) e = cudaMemcpyAsync(h_D, p->stageD[q], img, cudaMemcpyDeviceToHost, p->s_d2h);
+    if (e == cudaSuccess && h_D) e = cudaMemcpyAsync(h_D, f32 ? (void *)p->stageD32[q] : (void *)p->stageD[q], img, cudaMemcpyDeviceToHost, p->s_d2h);
     if (e == cudaSuccess && h_coef)
         e = cudaMemcpyAsync(h_coef, p->stageC[q], (size_t)p->nbatch * p->n * sizeof(double), cudaMemcpyDeviceToHost, p->s_d2h);
     if (e == cudaSuccess) e = cudaEventRecord(p->ev_out[q], p->s_d2h);
     if (e != cudaSuccess) return fail_cuda(p, e);
     return SFFT_OK;
+}
+
+int sfft_run_host_async(sfft_plan *p, const double *h_R, const double *h_S, double *h_D, double *h_coef) {
+    return run_host_async_any(p, h_R, h_S, h_D, h_coef, false);
+}
+
+int sfft_run_host_async_f32(sfft_plan *p, const float *h_R, const float *h_S, float *h_D, double *h_coef) {
+    return run_host_async_any(p, h_R, h_S, h_D, h_coef, true);
+}
+
+int sfft_run_host_f32(sfft_plan *p, const float *h_R, const float *h_S, float *h_D, double *h_coef) {
+    int st = sfft_run_host_async_f32(p, h_R, h_S, h_D, h_coef);
+    return st == SFFT_OK ? sfft_run_host_wait(p) : st;
 }
 
 int sfft_run_host_wait(sfft_plan *p) {

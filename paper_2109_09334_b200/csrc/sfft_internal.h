@@ -118,6 +118,7 @@ struct sfft_plan {
     // host-call staging: two slots so that the copies of one pair overlap the compute of another (sfft_run_host_async)
     double *stageR[2] = {nullptr, nullptr}, *stageS[2] = {nullptr, nullptr}, *stageD[2] = {nullptr, nullptr},
            *stageC[2] = {nullptr, nullptr};
+    float *stageR32[2] = {nullptr, nullptr}, *stageS32[2] = {nullptr, nullptr}, *stageD32[2] = {nullptr, nullptr};
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;           // plan-owned copy streams
     cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
     int host_slot = 0;                                       // next staging slot (round robin)
@@ -144,6 +145,10 @@ cudaError_t launch_corr_os(sfft_plan *p);
 cudaError_t launch_lagsum(sfft_plan *p);
 cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS);
 cudaError_t launch_gather(sfft_plan *p);
+cudaError_t launch_widen(sfft_plan *p, const float *src, double *dst, size_t count);     // float -> double (exact)
+cudaError_t launch_narrow(sfft_plan *p, const double *src, float *dst, size_t count);    // double -> float (round to nearest)
+cudaError_t launch_mask_fill(sfft_plan *p, const double *dR, const double *dS, double satR, double satS, int rd, int rb,
+                             double *dRm, double *dSm, unsigned char *dmask);
 cudaError_t launch_expand_coef(sfft_plan *p, const double *d_cr, double *d_coef);   // c = C c' (cpr)
 cudaError_t launch_solve(sfft_plan *p, double *d_coef);
 int solve_num_blocks(int n);     // 64-column panels of the Cholesky factorisation

@@ -414,6 +414,68 @@ def test_subtract_after_address_reuse_and_inplace_edit(cuda_device):
     plan.close(); plan2.close()
 
 
+def _saturate(p, sat, nsat=12, seed=5):
+    """Clip the brightest stars of a pair at `sat` plus a few bleed columns, as saturated sources look on a CCD."""
+    rng = np.random.default_rng(seed)
+    R, S = p.R.copy(), p.S.copy()
+    idx = np.argsort(R.ravel())[-nsat:]
+    for q in idx:
+        x, y = divmod(int(q), p.W)
+        h = int(rng.integers(2, 6))
+        for dx in range(-h, h + 1):
+            R[(x + dx) % p.H, y] = sat * 1.2
+            S[(x + dx) % p.H, y] = sat * 1.1
+    R[0, 0] = sat * 2; S[p.H - 1, p.W - 1] = sat * 3          # corners: the window wraps around the frame
+    return np.minimum(R, sat * 4), np.minimum(S, sat * 4)
+
+
+@pytest.mark.parametrize("cfg,H,W,L,rd,rb,nb", [(1, None, None, None, 2, 6, 1), (2, 64, 1024, 9, 1, 4, 1), (5, 128, 128, 5, 3, 8, 3)])
+def test_mask_fill_and_masked_fit_flow(cuda_device, cfg, H, W, L, rd, rb, nb):
+    """NEXT-2 (DESIGN g21): the CUDA mask/fill against the oracle (mask bit-exact, filled pixels to
+    rounding), then the paper's two-step flow end to end: fit on the masked pair, apply to the original pair."""
+    import torch
+    sat = 3000.0
+    if nb == 1:
+        p = synth.make_pair(cfg, H=H, W=W)
+        Rs, Ss = _saturate(p, sat)
+        Rl, Sl = [Rs], [Ss]
+    else:
+        p = synth.make_batch(cfg, nbatch=nb, H=H, W=W)
+        pp = [synth.Pair(R=p.R[e], S=p.S[e], H=p.H, W=p.W, L=p.L, DK=1, DB=1, basis="poly", sigma=p.sigma, config=cfg) for e in range(nb)]
+        Rl, Sl = zip(*[_saturate(q, sat, seed=e) for e, q in enumerate(pp)])
+        Rs, Ss = np.stack(Rl), np.stack(Sl)
+    L = p.L if L is None else L
+    DK, DB, basis = (p.DK, p.DB, p.basis) if nb == 1 else (1, 1, "poly")
+    plan = B.Plan(p.H, p.W, L, DK, DB, basis, nbatch=nb)
+    dR, dS = torch.from_numpy(np.ascontiguousarray(Rs)).cuda(), torch.from_numpy(np.ascontiguousarray(Ss)).cuda()
+    dRm, dSm, dmask = plan.mask_fill(dR, dS, sat, sat, rd, rb)
+    plan.build_system(dRm, dSm)
+    coef = plan.solve()
+    D = plan.subtract(coef, dR, dS)
+    plan.status()
+    Rm, Sm, mask = dRm.cpu().numpy().reshape(nb, p.H, p.W), dSm.cpu().numpy().reshape(nb, p.H, p.W), dmask.cpu().numpy().reshape(nb, p.H, p.W)
+    c, D = coef.cpu().numpy(), D.cpu().numpy().reshape(nb, p.H, p.W)
+    bid = _bid(basis)
+    for e in range(nb):
+        Rmo, Smo, mo = oracle.mask_fill(Rl[e], Sl[e], sat, sat, rd, rb)
+        assert mo.sum() > 0 and np.array_equal(mask[e], mo)
+        assert np.max(np.abs(Rm[e] - Rmo)) <= 1e-12 * sat and np.max(np.abs(Sm[e] - Smo)) <= 1e-12 * sat
+        assert np.array_equal(Rm[e][mo == 0], Rl[e][mo == 0])
+        Mo, ro = oracle.normal_from_lags(Rmo, Smo, L, bid, DK, DB)
+        co = oracle.solve(Mo, ro)
+        Do = oracle.difference(Rl[e], Sl[e], co, L, bid, DK, DB)
+        _check_coef(c[e], co, Mo.shape[0] - oracle.num_terms(bid, DB))
+        assert np.max(np.abs(D[e] - Do)) <= TOL_D * p.sigma
+    # in place, and argument errors
+    dR2, dS2 = dR.clone(), dS.clone()
+    a, b_, m2 = plan.mask_fill(dR2, dS2, sat, sat, rd, rb, inplace=True)
+    assert a.data_ptr() == dR2.data_ptr() and torch.equal(dR2, dRm) and torch.equal(dS2, dSm) and torch.equal(m2, dmask)
+    assert B.sfft_mask_fill(plan.h, dR.data_ptr(), dS.data_ptr(), sat, sat, -1, rb, dRm.data_ptr(), dSm.data_ptr(), dmask.data_ptr()) == B.SFFT_ERR_INVALID_ARG
+    assert B.sfft_mask_fill(plan.h, dR.data_ptr(), dS.data_ptr(), sat, sat, rd, 0, dRm.data_ptr(), dSm.data_ptr(), dmask.data_ptr()) == B.SFFT_ERR_INVALID_ARG
+    assert B.sfft_mask_fill(plan.h, dR.data_ptr(), 0, sat, sat, rd, rb, dRm.data_ptr(), dSm.data_ptr(), dmask.data_ptr()) == B.SFFT_ERR_INVALID_ARG
+    plan.close()
+
+
 def test_run_host_end_to_end(cuda_device):
     p = synth.make_pair(1)
     _, _, co, Do = _oracle_all(p.R, p.S, p.L, p.basis, p.DK, p.DB)
@@ -422,6 +484,36 @@ def test_run_host_end_to_end(cuda_device):
     _check_coef(c[0], co, 3 * p.L * p.L)
     assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
     assert plan.launch_count() > 0
+    plan.close()
+
+
+def test_run_host_f32_storage(cuda_device):
+    """NEXT-4: images stored as float on the host, arithmetic in FP64.  The oracle gets the same float-rounded
+    images (exactly representable in double); coefficients at the usual tolerance; D equals the oracle's D up to the
+    one rounding to float on the way out (half an ulp of float at |D|) plus the usual 1e-6 sigma."""
+    import torch
+    p = synth.make_pair(2, H=64, W=1024)
+    L = 9
+    R32, S32 = p.R.astype(np.float32), p.S.astype(np.float32)
+    _, _, co, Do = _oracle_all(R32.astype(np.float64), S32.astype(np.float64), L, "poly", p.DK, p.DB)
+    plan = B.Plan(p.H, p.W, L, p.DK, p.DB, "poly")
+    D, c = plan.run_host(R32, S32)
+    assert D.dtype == np.float32
+    _check_coef(c[0], co, 6 * L * L)
+    tol = TOL_D * p.sigma + np.abs(Do) * 2.0 ** -24 * 1.0001
+    assert np.all(np.abs(D.astype(np.float64) - Do) <= tol)
+    # mixed traffic through the two staging slots: f32, f64, f32 back to back, one wait
+    hR, hS = torch.from_numpy(R32).pin_memory(), torch.from_numpy(S32).pin_memory()
+    hR64, hS64 = torch.from_numpy(p.R).pin_memory(), torch.from_numpy(p.S).pin_memory()
+    hD = [torch.empty_like(hR).pin_memory(), torch.empty_like(hR64).pin_memory(), torch.empty_like(hR).pin_memory()]
+    hC = [torch.empty((1, plan.n), dtype=torch.float64).pin_memory() for _ in range(3)]
+    assert B.sfft_run_host_async_f32(plan.h, hR.data_ptr(), hS.data_ptr(), hD[0].data_ptr(), hC[0].data_ptr()) == B.SFFT_OK
+    assert B.sfft_run_host_async(plan.h, hR64.data_ptr(), hS64.data_ptr(), hD[1].data_ptr(), hC[1].data_ptr()) == B.SFFT_OK
+    assert B.sfft_run_host_async_f32(plan.h, hR.data_ptr(), hS.data_ptr(), hD[2].data_ptr(), hC[2].data_ptr()) == B.SFFT_OK
+    assert B.sfft_run_host_wait(plan.h) == B.SFFT_OK
+    assert np.array_equal(hD[0].numpy(), D) and np.array_equal(hD[2].numpy(), D) and np.array_equal(hC[2].numpy(), c)
+    _, _, co64, Do64 = _oracle_all(p.R, p.S, L, "poly", p.DK, p.DB)
+    assert np.max(np.abs(hD[1].numpy() - Do64)) <= TOL_D * p.sigma
     plan.close()
 
 
