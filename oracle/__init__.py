@@ -13,3 +13,4 @@ from .binding import (  # noqa: F401
     normal_from_lags, solve, difference, difference_at, corr_diff_one, weighted_ref,
     cpr_num_unknowns, cpr_constrain, cpr_expand, mask_fill,
 )
+from . import decorr  # noqa: F401,E402   (NEXT-3, App. C; numpy)

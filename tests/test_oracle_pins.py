@@ -517,3 +517,100 @@ def test_mask_fill_empty_window_falls_back_to_global_mean():
     assert mask.sum() == 64
     np.testing.assert_allclose(Rm[7, 7], R[mask == 0].mean(), rtol=1e-13)
     np.testing.assert_allclose(Sm[8, 8], S[mask == 0].mean(), rtol=1e-13)
+
+
+# --------------------------------------------------------------------------- NEXT-3: noise decorrelation (App. C)
+
+def _gauss_kernel(L, sig, shift=(0.0, 0.0)):
+    w = (L - 1) // 2
+    a = np.arange(-w, w + 1)
+    k = np.exp(-0.5 * ((a[:, None] - shift[0]) ** 2 + (a[None, :] - shift[1]) ** 2) / sig ** 2)
+    return k / k.sum()
+
+
+def _coef_from_pixel_kernels(ks, FB=1):
+    """Delta-basis coefficients whose pixel kernels (Eqs. 3-4) are ks[t]: centre coefficient = kernel sum."""
+    out = []
+    for k in ks:
+        a = k.ravel().copy()
+        a[a.size // 2] = k.sum()
+        out.append(a)
+    return np.concatenate(out + [np.zeros(FB)])
+
+
+def test_decorrelation_delta_kernel_is_identity_and_c20_values():
+    """K = c * delta, G = H = delta  =>  the C20 denominator is flat, Q0^ = 1, the image comes back unchanged.
+    And C20 itself at a few frequencies with K^ summed straight from its definition (no FFT): catches a wrong
+    sign/normalisation of the kernel transform, a missing square, or swapped variances."""
+    from oracle import decorr
+    rng = np.random.default_rng(41)
+    D = rng.standard_normal((64, 64))
+    L = 5
+    kd = np.zeros((L, L)); kd[2, 2] = 1.7
+    coef = _coef_from_pixel_kernels([kd])
+    out = decorr.decorrelate(D, coef, L, POLY, 0, 32, [2.0], [[[1.0]]], [3.0], [[[1.0]]])
+    np.testing.assert_allclose(out, D, rtol=0, atol=1e-13)
+    K = _gauss_kernel(L, 1.1, (0.3, -0.2)) * 0.9
+    Hk = _gauss_kernel(3, 0.8) / 2.0
+    T = 16
+    Q0, den = decorr.q0_hat(K, T, [2.0, 1.5], [[[0.5]], [[0.5]]], [3.0, 2.5], [Hk, Hk])
+    a = np.arange(-2, 3)
+    for (l, m) in [(0, 0), (1, 0), (3, 5), (8, 8), (15, 2)]:
+        Kh = np.sum(K * np.exp(-2j * np.pi * (l * a[:, None] + m * a[None, :]) / T))
+        ah = np.arange(-1, 2)
+        Hh = np.sum(Hk * np.exp(-2j * np.pi * (l * ah[:, None] + m * ah[None, :]) / T))
+        d = (2.0 + 1.5) * 0.25 + abs(Kh) ** 2 * (3.0 + 2.5) * abs(Hh) ** 2
+        assert abs(den[l, m] - d) < 1e-13 * d
+    d0 = (2.0 + 1.5) * 0.25 + K.sum() ** 2 * (3.0 + 2.5) * Hk.sum() ** 2
+    assert abs(Q0[3, 5] - np.sqrt(d0 / den[3, 5])) < 1e-14 and abs(Q0[0, 0] - 1.0) < 1e-15
+
+
+def test_decorrelation_kernel_has_unit_sum_and_is_a_wrap_convolution():
+    """Q has unit sum.  The response to a delta image IS Q; convolving with that Q through an
+    independent routine (scipy wrap convolution) must reproduce the tile-wise output: checks linearity, shift
+    invariance inside a tile, tile independence and the frozen-at-tile-centre kernel (spatially varying fit)."""
+    from oracle import decorr
+    H = W = 64; T = 32; L = 5
+    k0, k1 = _gauss_kernel(L, 1.0), _gauss_kernel(L, 1.6, (0.4, 0.0)) - _gauss_kernel(L, 1.0)
+    coef = np.concatenate([_coef_from_pixel_kernels([k0, 0.3 * k1, -0.2 * k1], FB=0), np.zeros(3)])   # DK = 1: 3 terms
+    args = (coef, L, POLY, 1, T, [1.0], [[[1.0]]], [1.3], [[[1.0]]])
+    rng = np.random.default_rng(42)
+    D = rng.standard_normal((H, W))
+    out = decorr.decorrelate(D, *args)
+    for a in range(2):
+        for b in range(2):
+            imp = np.zeros((H, W)); imp[a * T + T // 2, b * T + T // 2] = 1.0
+            Q = decorr.decorrelate(imp, *args)[a * T:(a + 1) * T, b * T:(b + 1) * T]     # centred at (T/2, T/2)
+            assert abs(Q.sum() - 1.0) < 1e-13
+            np.testing.assert_allclose(Q[1:, 1:], Q[1:, 1:][::-1, ::-1], atol=1e-14)    # Q(-u) = Q(u): Q0^ is real
+            ref = scipy.ndimage.convolve(D[a * T:(a + 1) * T, b * T:(b + 1) * T], Q, mode="wrap", origin=0)
+            np.testing.assert_allclose(out[a * T:(a + 1) * T, b * T:(b + 1) * T], ref, rtol=0, atol=1e-12)
+    # the kernel differs between tiles (spatial variation of the fit)
+    assert np.abs(decorr.kernel_at(coef, L, POLY, 1, H, W, 16, 16) - decorr.kernel_at(coef, L, POLY, 1, H, W, 48, 48)).max() > 1e-3
+    # kernel_at against the model of the difference image: -D of a delta reference at (xc,yc) read around (xc,yc)
+    R = np.zeros((H, W)); R[16, 16] = 1.0
+    model = -oracle.difference(R, np.zeros((H, W)), coef, L, POLY, 1, 1)
+    np.testing.assert_allclose(model[14:19, 14:19], decorr.kernel_at(coef, L, POLY, 1, H, W, 16, 16), atol=1e-14)
+
+
+def test_decorrelation_whitens_the_noise():
+    """Statistical pin (App. C's purpose): D = n_S - n_R (*) K with white n_S, n_R has correlated noise; after
+    decorrelation the sample autocorrelation at small lags vanishes to sampling error and the variance is the
+    C20 denominator at zero frequency, sigma_S^2 + sigma_R^2 (sum K)^2."""
+    from oracle import decorr
+    T = 128; L = 7
+    rng = np.random.default_rng(43)
+    K = _gauss_kernel(L, 1.4) * 1.1
+    vS, vR = 4.0, 9.0
+    nS, nR = rng.normal(0, np.sqrt(vS), (T, T)), rng.normal(0, np.sqrt(vR), (T, T))
+    D = nS - scipy.ndimage.convolve(nR, K, mode="wrap")
+    coef = _coef_from_pixel_kernels([K])
+    out = decorr.decorrelate(D, coef, L, POLY, 0, T, [vS], [[[1.0]]], [vR], [[[1.0]]])
+
+    def acorr(img, dx, dy):
+        z = img - img.mean()
+        return float(np.mean(z * np.roll(z, (dx, dy), axis=(0, 1))) / np.mean(z * z))
+    assert abs(acorr(D, 0, 1)) > 0.05 and abs(acorr(D, 1, 1)) > 0.03           # correlated before (sampling error 1/T = 0.008)
+    for lag in [(0, 1), (1, 0), (1, 1), (2, 0), (0, 3)]:
+        assert abs(acorr(out, *lag)) < 5.0 / T                                     # white after (sampling error 1/T)
+    assert abs(out.var() / (vS + vR * K.sum() ** 2) - 1.0) < 0.05
