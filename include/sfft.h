@@ -152,6 +152,22 @@ int sfft_plan_set_reuse_spectra(sfft_plan *plan, int on);
 int sfft_mask_fill(sfft_plan *plan, const double *d_R, const double *d_S, double sat_R, double sat_S, int rd, int rb,
                    double *d_Rm, double *d_Sm, unsigned char *d_mask);
 
+/* NEXT-3, noise decorrelation of a difference image (App. C; readings DESIGN g22).  With
+ *   D = sum_j S_j (*) G_j - [sum_i R_i (*) H_i] (*) K                                            (C17)
+ *   Q0^ = sqrt( sigma_D^2 / { sum_j varS_j |G_j^|^2 + sum_i varR_i |K^|^2 |H_i^|^2 } )           (C20)
+ * and Q normalised to unit kernel sum, d_Ddc = D (*) Q, segment by segment: the frame
+ * is cut in square tiles of `tile` pixels (a power of two in [32, 512] dividing H and W, >= L), K is the fitted
+ * kernel of d_coef frozen at each tile's centre pixel (tile/2, tile/2 of the tile), and every tile is convolved
+ * circularly with its own Q.  G_j (nS kernels, LG x LG, row-major, centred, LG odd <= tile) and H_i (nR kernels,
+ * LH x LH) are the PSF-homogenisation kernels of the co-added science / reference images, already divided by the
+ * number of images as in the paper; varS / varR their background noise variances.  For a plain pair pass
+ * nS = nR = 1, LG = LH = 1, G = H = {1.0}.  h_* are HOST arrays (read before the call returns).  d_D, d_Ddc:
+ * [nbatch][H][W] double, may alias.  Uses the spectrum area of the workspace as scratch (SFFT_ERR_WORKSPACE if it is
+ * too small for the tile size), so a following Fourier-route sfft_subtract transforms its reference again. */
+int sfft_decorrelate(sfft_plan *plan, const double *d_coef, const double *d_D, double *d_Ddc, int tile,
+                     int nS, const double *h_varS, int LG, const double *h_G,
+                     int nR, const double *h_varR, int LH, const double *h_H);
+
 /* Synchronise the plan's stream and report numerical status.  On SFFT_ERR_NOT_SPD, *info =
  * batch*ns + index of the first failing pivot in the order of the solved system (ns =
  * sfft_plan_num_solved(): the reduced layout under the constant photometric ratio); otherwise

@@ -20,7 +20,7 @@ EXPORTS = [
     "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_set_corr_route", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
     "sfft_plan_num_kernel_terms", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
-    "sfft_subtract", "sfft_mask_fill", "sfft_plan_set_reuse_spectra", "sfft_plan_status", "sfft_plan_host_staging_bytes", "sfft_plan_set_host_staging",
+    "sfft_subtract", "sfft_mask_fill", "sfft_decorrelate", "sfft_plan_set_reuse_spectra", "sfft_plan_status", "sfft_plan_host_staging_bytes", "sfft_plan_set_host_staging",
     "sfft_run_host", "sfft_run_host_async", "sfft_run_host_wait", "sfft_run_host_f32", "sfft_run_host_async_f32", "sfft_plan_launch_count", "sfft_plan_destroy",
     "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
 ]
@@ -71,6 +71,7 @@ def load_library(build_if_missing=True):
         "sfft_solve": (ci, [vp, vp]),
         "sfft_subtract": (ci, [vp, vp, vp, vp, vp]),
         "sfft_mask_fill": (ci, [vp, vp, vp, ctypes.c_double, ctypes.c_double, ci, ci, vp, vp, vp]),
+        "sfft_decorrelate": (ci, [vp, vp, vp, vp, ci, ci, vp, ci, vp, ci, vp, ci, vp]),
         "sfft_plan_set_reuse_spectra": (ci, [vp, ci]),
         "sfft_plan_status": (ci, [vp, pci]),
         "sfft_plan_host_staging_bytes": (cs, [vp]),
@@ -172,6 +173,16 @@ def sfft_mask_fill(plan, d_R, d_S, sat_R, sat_S, rd, rb, d_Rm, d_Sm, d_mask):
     return load_library().sfft_mask_fill(plan, ctypes.c_void_p(d_R), ctypes.c_void_p(d_S), float(sat_R), float(sat_S),
                                          int(rd), int(rb), ctypes.c_void_p(d_Rm), ctypes.c_void_p(d_Sm),
                                          ctypes.c_void_p(d_mask))
+
+
+def sfft_decorrelate(plan, d_coef, d_D, d_Ddc, tile, var_S, G, var_R, H):
+    """var_S [nS], G [nS][LG][LG], var_R [nR], H [nR][LH][LH]: numpy (host) arrays."""
+    vS, vR = np.ascontiguousarray(var_S, dtype=np.float64), np.ascontiguousarray(var_R, dtype=np.float64)
+    Gk, Hk = np.ascontiguousarray(G, dtype=np.float64), np.ascontiguousarray(H, dtype=np.float64)
+    assert Gk.ndim == 3 and Hk.ndim == 3 and Gk.shape[0] == vS.size and Hk.shape[0] == vR.size
+    return load_library().sfft_decorrelate(plan, ctypes.c_void_p(d_coef), ctypes.c_void_p(d_D), ctypes.c_void_p(d_Ddc),
+                                           int(tile), int(vS.size), vS.ctypes.data, int(Gk.shape[1]), Gk.ctypes.data,
+                                           int(vR.size), vR.ctypes.data, int(Hk.shape[1]), Hk.ctypes.data)
 
 
 def sfft_plan_set_reuse_spectra(plan, on):
@@ -326,6 +337,13 @@ class Plan:
         self._check(sfft_mask_fill(self.h, self._img(R), self._img(S), sat_R, sat_S, rd, rb, Rm.data_ptr(), Sm.data_ptr(),
                                    mask.data_ptr()), "sfft_mask_fill")
         return Rm, Sm, mask
+
+    def decorrelate(self, coef, D, tile, var_S, G, var_R, H, out=None):
+        """NEXT-3 (App. C): D convolved tile by tile with the unit-sum decorrelation kernel of Eq. C20."""
+        out = self.torch.empty_like(D) if out is None else out
+        self._check(sfft_decorrelate(self.h, coef.data_ptr(), self._img(D), self._img(out), tile, var_S, G, var_R, H),
+                    "sfft_decorrelate")
+        return out
 
     def status(self, check=True):
         st, info = sfft_plan_status(self.h)

@@ -633,6 +633,27 @@ int sfft_mask_fill(sfft_plan *p, const double *d_R, const double *d_S, double sa
     return SFFT_OK;
 }
 
+int sfft_decorrelate(sfft_plan *p, const double *d_coef, const double *d_D, double *d_Ddc, int tile, int nS,
+                     const double *h_varS, int LG, const double *h_G, int nR, const double *h_varR, int LH,
+                     const double *h_H) {
+    if (!p || !d_coef || !d_D || !d_Ddc || !h_varS || !h_G || !h_varR || !h_H) return SFFT_ERR_INVALID_ARG;
+    if (!is_pow2(tile) || tile < 32 || tile > 512 || p->H % tile || p->W % tile || p->L > tile) return SFFT_ERR_INVALID_ARG;
+    if (nS < 1 || nR < 1 || nS > 64 || nR > 64 || LG < 1 || LH < 1 || !(LG & 1) || !(LH & 1) || LG > tile || LH > tile ||
+        LG > 65 || LH > 65)
+        return SFFT_ERR_INVALID_ARG;
+    if (!p->ws) return SFFT_ERR_WORKSPACE;
+    if (wrong_device(p)) return SFFT_ERR_STATE;
+    const size_t P = (size_t)p->H * p->W, area = (size_t)p->nbatch * p->nimg * P * sizeof(double);
+    const size_t need = (size_t)p->nbatch * P * sizeof(double) + (size_t)tile * sizeof(double2) +
+                        2 * (size_t)tile * (tile / 2 + 1) * sizeof(double) +
+                        ((size_t)nS * LG * LG + nS + (size_t)nR * LH * LH + nR) * sizeof(double);
+    if (need > area) return SFFT_ERR_WORKSPACE;
+    p->rhat_from_build = false;                 // the spectrum area is used as scratch
+    cudaError_t e = launch_decorrelate(p, d_coef, d_D, d_Ddc, tile, nS, h_varS, LG, h_G, nR, h_varR, LH, h_H);
+    if (e != cudaSuccess) return fail_cuda(p, e);
+    return SFFT_OK;
+}
+
 int sfft_plan_status(sfft_plan *p, int *info) {
     if (info) *info = -1;
     if (!p) return SFFT_ERR_INVALID_ARG;

@@ -145,6 +145,9 @@ cudaError_t launch_corr_os(sfft_plan *p);
 cudaError_t launch_lagsum(sfft_plan *p);
 cudaError_t launch_moments(sfft_plan *p, const double *dR, const double *dS);
 cudaError_t launch_gather(sfft_plan *p);
+cudaError_t launch_decorrelate(sfft_plan *p, const double *d_coef, const double *dD, double *dOut, int T, int nS,
+                               const double *h_varS, int LG, const double *h_G, int nR, const double *h_varR, int LH,
+                               const double *h_H);
 cudaError_t launch_widen(sfft_plan *p, const float *src, double *dst, size_t count);     // float -> double (exact)
 cudaError_t launch_narrow(sfft_plan *p, const double *src, float *dst, size_t count);    // double -> float (round to nearest)
 cudaError_t launch_mask_fill(sfft_plan *p, const double *dR, const double *dS, double satR, double satS, int rd, int rb,

@@ -476,6 +476,46 @@ def test_mask_fill_and_masked_fit_flow(cuda_device, cfg, H, W, L, rd, rb, nb):
     plan.close()
 
 
+@pytest.mark.parametrize("cfg,H,W,L,DK,tile,coadd", [(1, 128, 128, 7, 1, 32, False), (2, 256, 512, 11, 2, 128, True),
+                                                        (2, 512, 512, 9, 2, 512, False), (2, 64, 1024, 5, 0, 64, True)])
+def test_decorrelation_parity(cuda_device, cfg, H, W, L, DK, tile, coadd):
+    """NEXT-3 (App. C, Eq. C20; DESIGN g22): fit, subtract, then decorrelate on the GPU; the oracle decorrelates the
+    GPU's difference image with the GPU's coefficients (both already checked against the oracle elsewhere), so this
+    compares the decorrelation step alone, tile by tile, including the spatially varying kernel frozen at the tile
+    centres and co-addition kernels G_j, H_i."""
+    import torch
+    from oracle import decorr
+    p = synth.make_pair(cfg, H=H, W=W)
+    DB = 1
+    plan = B.Plan(H, W, L, DK, DB, "poly")
+    dR, dS = torch.from_numpy(p.R).cuda(), torch.from_numpy(p.S).cuda()
+    plan.build_system(dR, dS)
+    coef = plan.solve()
+    D = plan.subtract(coef, dR, dS)
+    if coadd:
+        g = np.array([[0.0, 0.1, 0.0], [0.1, 0.6, 0.1], [0.0, 0.1, 0.0]])
+        var_S, G = [120.0, 130.0], np.stack([g / 2, np.roll(g, 1, axis=1) / 2])
+        hk = np.zeros((5, 5)); hk[2, 2] = 0.5; hk[1, 2] = hk[3, 2] = 0.2; hk[2, 0] = 0.1
+        var_R, Hk = [125.0, 110.0, 140.0], np.stack([hk / 3, hk.T / 3, hk[::-1] / 3])
+    else:
+        var_S, G, var_R, Hk = [125.0], np.ones((1, 1, 1)), [125.0], np.ones((1, 1, 1))
+    Ddc = plan.decorrelate(coef, D, tile, var_S, G, var_R, Hk)
+    plan.status()
+    Dn, cn = D.cpu().numpy(), coef.cpu().numpy()[0]
+    ref = decorr.decorrelate(Dn, cn, L, oracle.POLY, DK, tile, var_S, G, var_R, Hk)
+    assert np.max(np.abs(ref - Dn)) > 1e-3 * p.sigma                       # the step does something
+    assert np.max(np.abs(Ddc.cpu().numpy() - ref)) <= TOL_D * p.sigma
+    # in place, and the documented argument errors
+    D2 = D.clone()
+    plan.decorrelate(coef, D2, tile, var_S, G, var_R, Hk, out=D2)
+    plan.status()
+    assert torch.equal(D2, Ddc)
+    for bad_tile in (48, 16, 1024):
+        assert B.sfft_decorrelate(plan.h, coef.data_ptr(), D.data_ptr(), D2.data_ptr(), bad_tile, var_S, G, var_R, Hk) == B.SFFT_ERR_INVALID_ARG
+    assert B.sfft_decorrelate(plan.h, coef.data_ptr(), D.data_ptr(), D2.data_ptr(), tile, var_S, np.ones((len(var_S), 2, 2)), var_R, Hk) == B.SFFT_ERR_INVALID_ARG
+    plan.close()
+
+
 def test_run_host_end_to_end(cuda_device):
     p = synth.make_pair(1)
     _, _, co, Do = _oracle_all(p.R, p.S, p.L, p.basis, p.DK, p.DB)
