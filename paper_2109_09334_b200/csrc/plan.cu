@@ -238,7 +238,7 @@ void free_tables(sfft_plan *p) {
 }
 
 struct WsLayout {
-    size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, coefr, kfold, ctab, khat, flag, total;
+    size_t rhat, G, lagpart, tab, Q, QS, LamC, mu, M, rhs, Lf, Winv, dscale, coefr, ybuf, kfold, ctab, khat, flag, total;
 };
 struct StagingLayout { size_t stR[2], stS[2], stD[2], stC[2], stR32[2], stS32[2], stD32[2], total; };
 
@@ -260,6 +260,7 @@ WsLayout ws_layout(const sfft_plan *p) {
     l.Winv = take(nb * (size_t)solve_num_blocks(p->n) * 64 * 64 * sizeof(double));
     l.dscale = take(nb * n * sizeof(double));
     l.coefr = take(nb * n * sizeof(double));
+    l.ybuf = take(nb * (size_t)solve_num_blocks(p->n) * 64 * sizeof(double));
     l.kfold = take(nb * (size_t)p->FK * p->L * p->L * sizeof(double));
     // only the subtract route the plan takes gets its table
     l.ctab = take(subtract_use_fourier(p) ? 0 : nb * (size_t)p->H * p->L * p->LT * sizeof(double));
@@ -478,7 +479,7 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     p->rhat = (double2 *)(b + l.rhat); p->G = (double2 *)(b + l.G); p->lagpart = (double *)(b + l.lagpart); p->tab = (double *)(b + l.tab);
     p->Q = (double *)(b + l.Q); p->QS = (double *)(b + l.QS); p->LamC = (double *)(b + l.LamC); p->mu = (double *)(b + l.mu);
     p->M = (double *)(b + l.M); p->rhs = (double *)(b + l.rhs); p->Lf = (double *)(b + l.Lf); p->Winv = (double *)(b + l.Winv);
-    p->dscale = (double *)(b + l.dscale); p->coefr = (double *)(b + l.coefr); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
+    p->dscale = (double *)(b + l.dscale); p->coefr = (double *)(b + l.coefr); p->ybuf = (double *)(b + l.ybuf); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
     p->built = p->solved = false;
     p->rhat_from_build = false;
     return SFFT_OK;

@@ -115,6 +115,7 @@ struct sfft_plan {
     bool host_call = false;                     // inside sfft_run_host*: build and subtract see the same staged pair
     int device = 0;                             // CUDA device the plan was created on
     double *coefr = nullptr;                    // [b][ns] reduced solution (cpr) before expansion to the full layout
+    double *ybuf = nullptr;                     // [b][nblk*64] published blocks of the back substitution (solve.cu)
     // host-call staging: two slots so that the copies of one pair overlap the compute of another (sfft_run_host_async)
     double *stageR[2] = {nullptr, nullptr}, *stageS[2] = {nullptr, nullptr}, *stageD[2] = {nullptr, nullptr},
            *stageC[2] = {nullptr, nullptr};

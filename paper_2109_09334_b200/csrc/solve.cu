@@ -18,19 +18,16 @@
 //      instead - one factoring CTA per system (k_chol_step with a single slab), lean slab CTAs that read
 //      W from global memory (k_chol_slab), and the trailing update by segments of tile rows with a
 //      cp.async double buffer and register-prefetched C tiles (k_chol_update_row).
-//   3. Backward substitution L^T y = z by a thread-block cluster of 8 CTAs per system: the owner
-//      of diagonal block b forms y_b = W_b^T z_b (W_b = L_bb^-1 from the factorisation), broadcasts it
-//      through distributed shared memory, and every CTA updates the columns it owns.  c = D y.
+//   3. Backward substitution L^T y = z with one CTA per 64-column block: CTA b prefetches its tiles of the factor,
+//      consumes the blocks y_j (j > b) as their owners publish them in global memory (the values are their own
+//      flags: a sentinel pattern marks "not yet written"), then forms y_b = W_b^T z_b with W_b = L_bb^-1 from the
+//      factorisation.  c = D y.
 // A diagonal entry that is not positive and finite, or a pivot of the scaled matrix (unit diagonal) that is not
 // finite or lies below kPivotFloor * n (rounding-noise level of the assembled entries: the system is numerically
 // rank-deficient even where the noise happens to be positive), writes its index to flag[2*b] (SFFT_ERR_NOT_SPD).
-#include <cooperative_groups.h>
-
 #include <algorithm>
 
 #include "sfft_internal.h"
-
-namespace cg = cooperative_groups;
 
 namespace sfft {
 namespace {
@@ -38,27 +35,51 @@ namespace {
 constexpr int NB = 64;        // panel width = tile size
 constexpr int LDT = NB + 4;   // smem stride of MMA operand tiles (= 4 mod 16: conflict-free fragments)
 constexpr int LDX = NB + 1;   // smem stride of the factor / solve views (conflict-free row-per-thread access)
-constexpr int CS = 8;         // cluster size of the back substitution
 constexpr double kPivotFloor = 64.0 * 2.220446049250313e-16;   // x n: smallest pivot of the scaled matrix taken as non-zero
 
 __device__ __forceinline__ bool pivot_ok(double p, double pmin) { return p > pmin && p < 1e300; }
 
-__global__ void k_scale_diag(const double *__restrict__ M, double *__restrict__ dscale, int *flag, int n) {
+__global__ void k_scale_diag(const double *__restrict__ M, double *__restrict__ dscale, int *flag, int n,
+                             unsigned long long *__restrict__ ybuf, int ny, unsigned long long sentinel) {
     int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (i < ny) ybuf[(size_t)b * ny + i] = sentinel;       // "not yet published" marks of the look-back back substitution
     if (i >= n) return;
     double d = M[((size_t)b * n + i) * n + i];
     if (!(d > 0.0 && d < 1e300)) { atomicCAS(&flag[2 * b], -1, i); d = 1.0; }
     dscale[(size_t)b * n + i] = rsqrt(d);
 }
 
-// Lf[i][j] = M[i][j] d_i d_j (j <= i), row n = rhs_j d_j
-__global__ void k_scale_copy(const double *__restrict__ M, const double *__restrict__ rhs,
-                             const double *__restrict__ dscale, double *__restrict__ Lf, int n, int ldl) {
-    int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y, b = blockIdx.z;
-    if (j >= n || j > i) return;
+// Lf[i][j] = M[i][j] d_i d_j (j <= i), row n = rhs_j d_j.  CTA = 16 rows x 128 columns, thread = 4 rows x 2 columns
+// (eight independent loads in flight); tiles above the diagonal exit at once.
+__global__ void __launch_bounds__(256) k_scale_copy(const double *__restrict__ M, const double *__restrict__ rhs,
+                                                    const double *__restrict__ dscale, double *__restrict__ Lf, int n, int ldl) {
+    const int j = blockIdx.x * 128 + 2 * (threadIdx.x & 63), i0 = blockIdx.y * 16 + (threadIdx.x >> 6), b = blockIdx.z;
+    if (blockIdx.x * 128 > blockIdx.y * 16 + 15 || j >= n) return;
     const double *d = dscale + (size_t)b * n;
-    double v = (i < n) ? M[((size_t)b * n + i) * n + j] * d[i] * d[j] : rhs[(size_t)b * n + j] * d[j];
-    Lf[((size_t)b * (n + 1) + i) * ldl + j] = v;
+    const double dj0 = d[j], dj1 = (j + 1 < n) ? d[j + 1] : 0.0;
+    double v0[4], v1[4], di[4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int i = i0 + 4 * r;
+        v0[r] = v1[r] = 0.0; di[r] = 1.0;
+        if (i < n) {
+            const double *src = M + ((size_t)b * n + i) * n + j;
+            di[r] = d[i];
+            if (j <= i) v0[r] = src[0];
+            if (j + 1 <= i) v1[r] = src[1];
+        } else if (i == n) {
+            v0[r] = rhs[(size_t)b * n + j];
+            if (j + 1 < n) v1[r] = rhs[(size_t)b * n + j + 1];
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int i = i0 + 4 * r;
+        if (i > n || j > i) continue;
+        double *dst = Lf + ((size_t)b * (n + 1) + i) * ldl + j;
+        if (j + 1 <= i && j + 1 < n) *reinterpret_cast<double2 *>(dst) = make_double2(v0[r] * di[r] * dj0, v1[r] * di[r] * dj1);
+        else dst[0] = v0[r] * di[r] * dj0;
+    }
 }
 
 // T[r][c] = L[row0 + r][col0 + c] for r < nr (else 0), 64 columns, into an MMA operand tile (stride LDT).
@@ -553,73 +574,109 @@ __global__ void __launch_bounds__(256, 2) k_chol_slab(double *__restrict__ Lf, c
         }
 }
 
-// Backward substitution L^T y = z (z = row n of Lf), c = D y.  One cluster of CS CTAs per system; CTA `rank`
-// owns the 64-column blocks with block % CS == rank and keeps their part of z in shared memory.  Per diagonal
-// block (from the last): the owner forms y_b = W_b^T z_b, broadcasts it through distributed shared memory, and
-// after one cluster barrier every CTA subtracts L[b-rows][own columns]^T y_b from its part of z.  All global
-// loads of a step are issued as independent batches of 16 per thread (the step is L2-latency bound).
-__global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(256)
-k_chol_backsolve(const double *__restrict__ Lf, const double *__restrict__ Winv, const double *__restrict__ dscale,
-                 double *__restrict__ coef, int n, int ldl, int nblk, int nown_max) {
-    extern __shared__ double zs[];                 // [nblk * 64] (own blocks valid), then part[4][nown_max * 64]
-    __shared__ double ybuf[2][NB];
-    __shared__ double red[4][NB];
-    double *part = zs + (size_t)nblk * NB;
-    cg::cluster_group cluster = cg::this_cluster();
-    const int rank = (int)cluster.block_rank(), b = blockIdx.y, tid = threadIdx.x;
-    const int col = tid & 63, q = tid >> 6;
-    const double *L = Lf + (size_t)b * (n + 1) * ldl;
-    for (int i = tid; i < nblk * NB; i += 256) zs[i] = (i < n) ? L[(size_t)n * ldl + i] : 0.0;
-    cluster.sync();
-    for (int blk = nblk - 1; blk >= 0; --blk) {
-        const int i0 = blk * NB, nbk = min(NB, n - i0);
-        if (rank == blk % CS) {
-            // y_i = sum_k W[k][i] z_k  (W lower triangular, stored with its zeros): quarter q of the k range per thread
-            const double *W = Winv + ((size_t)b * nblk + blk) * NB * NB + (size_t)(16 * q) * NB + col;
-            double w[16];
+// Backward substitution L^T y = z (z = row n of Lf), c = D y, look-back form.  One CTA per 64-column block b of one
+// system; CTA b keeps z_b, prefetches the tiles L[j-rows][b-columns] of the blocks j > b through a ring of
+// cp.async stages (the factor is complete when the kernel starts, so the tiles never wait), and consumes
+// y_j = (L^T)^-1 part of block j as soon as its owner publishes it:  z_b -= L_jb^T y_j (partial sums stay in
+// registers over all j), then y_b = W_b^T z_b, c_b = D y_b.  The y values themselves are the flags: the buffer is
+// filled with a sentinel NaN pattern (k_scale_diag) and every consumer thread polls the 16 values it needs with
+// volatile loads, so a step of the dependent chain costs one L2 round trip, two 64 x 64 matrix-vector products
+// and three barriers instead of a cluster barrier and a round of global loads.  CTAs are ordered so that a CTA only
+// waits for CTAs with a smaller linear index (in-order dispatch): no co-residency requirement beyond one CTA.
+constexpr int kBsStages = 4;
+constexpr unsigned long long kBsSentinel = 0xFFF8DEADBEEF5AFEull;
+constexpr size_t kBsSmem = (size_t)(1 + kBsStages) * NB * NB * sizeof(double);
+
+__device__ __forceinline__ double ld_volatile_f64(const double *p) {
+    double v;
+    asm volatile("ld.volatile.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void ld_volatile_f64x2(const double *p, double &a, double &b) {
+    asm volatile("ld.volatile.global.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void st_volatile_f64(double *p, double v) {
+    asm volatile("st.volatile.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
+
+__global__ void __launch_bounds__(256)
+k_chol_backsolve_lb(const double *__restrict__ Lf, const double *__restrict__ Winv, const double *__restrict__ dscale,
+                    double *__restrict__ coef, double *ybuf, int n, int ldl, int nblk, int nbat) {
+    extern __shared__ double sm[];
+    double *Ws = sm, *T = sm + NB * NB;                 // W_b [k][i]; tile ring [stage][k][col]
+    __shared__ double zs[NB], red[4][NB], ysh[2][NB];
+    const int id = blockIdx.x, bz = id % nbat, x = id / nbat, blk = nblk - 1 - x;
+    const int tid = threadIdx.x, col = tid & 63, q = tid >> 6;
+    const double *L = Lf + (size_t)bz * (n + 1) * ldl;
+    double *yb = ybuf + (size_t)bz * nblk * NB;
+    const int i0 = blk * NB, nbk = min(NB, n - i0);
+    {
+        const double *W = Winv + ((size_t)bz * nblk + blk) * NB * NB;
+        for (int i = tid; i < NB * NB / 2; i += 256) cp_async16(&Ws[2 * i], &W[2 * i]);
+        asm volatile("cp.async.commit_group;");
+    }
+    auto fetch = [&](int t) {                              // tile of block j = nblk-1-t into stage t % kBsStages
+        if (t < x) {
+            const int j0 = (nblk - 1 - t) * NB;
+            double *dst = T + (size_t)(t % kBsStages) * NB * NB;
 #pragma unroll
-            for (int k = 0; k < 16; ++k) w[k] = W[k * NB];
-            double y0 = 0.0, y1 = 0.0;
-#pragma unroll
-            for (int k = 0; k < 16; k += 2) {
-                y0 = fma(w[k], zs[i0 + 16 * q + k], y0);
-                y1 = fma(w[k + 1], zs[i0 + 16 * q + k + 1], y1);
-            }
-            red[q][col] = y0 + y1;
-            __syncthreads();
-            if (tid < NB) {
-                const double y = (red[0][tid] + red[1][tid]) + (red[2][tid] + red[3][tid]);
-                if (tid < nbk) coef[(size_t)b * n + i0 + tid] = y * dscale[(size_t)b * n + i0 + tid];
-#pragma unroll
-                for (int c = 0; c < CS; ++c) cluster.map_shared_rank(&ybuf[blk & 1][0], c)[tid] = (tid < nbk) ? y : 0.0;
+            for (int r = 0; r < NB * NB / 2 / 256; ++r) {
+                const int i = tid + 256 * r, k = i >> 5, c = (i & 31) * 2;
+                if (j0 + k < n) cp_async16(&dst[k * NB + c], &L[(size_t)(j0 + k) * ldl + i0 + c]);
+                else { dst[k * NB + c] = 0.0; dst[k * NB + c + 1] = 0.0; }
             }
         }
-        cluster.sync();
-        // z_j -= sum_k L[i0 + k][j] y_k for the columns of the blocks this CTA owns below blk (nearest first)
-        const double *yb = ybuf[blk & 1];
-        const int first = blk - 1 - ((blk - 1 - rank) % CS + CS) % CS;      // largest owned block < blk
-        const int nown = first >= 0 ? first / CS + 1 : 0;
-        for (int o = 0; o < nown; ++o) {
-            const int ob = first - o * CS;
-            const double *src = L + (size_t)(i0 + 16 * q) * ldl + ob * NB + col;
-            double v[16];
+        asm volatile("cp.async.commit_group;");
+    };
 #pragma unroll
-            for (int k = 0; k < 16; ++k) v[k] = (16 * q + k < nbk) ? src[(size_t)k * ldl] : 0.0;
-            double s0 = 0.0, s1 = 0.0;
+    for (int t = 0; t < kBsStages - 1; ++t) fetch(t);
+    if (tid < NB) zs[tid] = (tid < nbk) ? L[(size_t)n * ldl + i0 + tid] : 0.0;
+    double a0 = 0.0, a1 = 0.0;
+    for (int t = 0; t < x; ++t) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(kBsStages - 2) : "memory");     // tile t (and W) landed
+        if (tid < 32) {
+            // one warp polls the 64 values of block j (a hot line for every CTA below j: keep the request count low)
+            const double *yj = yb + (size_t)(nblk - 1 - t) * NB + 2 * tid;
+            double v0, v1;
+            do {
+                ld_volatile_f64x2(yj, v0, v1);
+            } while ((unsigned long long)__double_as_longlong(v0) == kBsSentinel ||
+                     (unsigned long long)__double_as_longlong(v1) == kBsSentinel);
+            ysh[t & 1][2 * tid] = v0;
+            ysh[t & 1][2 * tid + 1] = v1;
+        }
+        __syncthreads();        // tile t and y_j visible to every thread; stage (t-1) % S and ysh[(t-1) & 1] are free again
+        fetch(t + kBsStages - 1);
+        const double *yv = &ysh[t & 1][16 * q];
+        const double *tp = T + (size_t)(t % kBsStages) * NB * NB + (16 * q) * NB + col;
 #pragma unroll
-            for (int k = 0; k < 16; k += 2) {
-                s0 = fma(v[k], yb[16 * q + k], s0);
-                s1 = fma(v[k + 1], yb[16 * q + k + 1], s1);
-            }
-            part[((size_t)q * nown_max + o) * NB + col] = s0 + s1;
+        for (int k = 0; k < 16; k += 2) {
+            a0 = fma(tp[k * NB], yv[k], a0);
+            a1 = fma(tp[(k + 1) * NB], yv[k + 1], a1);
         }
-        __syncthreads();
-        for (int o = q; o < nown; o += 4) {
-            const int ob = first - o * CS;
-            const size_t po = (size_t)o * NB + col, ps = (size_t)nown_max * NB;
-            zs[ob * NB + col] -= (part[po] + part[ps + po]) + (part[2 * ps + po] + part[3 * ps + po]);
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    red[q][col] = a0 + a1;
+    __syncthreads();
+    if (tid < NB) zs[tid] -= (red[0][tid] + red[1][tid]) + (red[2][tid] + red[3][tid]);
+    __syncthreads();
+    {
+        // y_i = sum_k W[k][i] z_k  (W lower triangular, stored with its zeros)
+        const double *wp = Ws + (16 * q) * NB + col;
+        double y0 = 0.0, y1 = 0.0;
+#pragma unroll
+        for (int k = 0; k < 16; k += 2) {
+            y0 = fma(wp[k * NB], zs[16 * q + k], y0);
+            y1 = fma(wp[(k + 1) * NB], zs[16 * q + k + 1], y1);
         }
-        __syncthreads();
+        __syncthreads();                                   // red (read above by tid < 64) may be rewritten
+        red[q][col] = y0 + y1;
+    }
+    __syncthreads();
+    if (tid < NB) {
+        const double y = (tid < nbk) ? (red[0][tid] + red[1][tid]) + (red[2][tid] + red[3][tid]) : 0.0;
+        st_volatile_f64(&yb[(size_t)blk * NB + tid], y);
+        if (tid < nbk) coef[(size_t)bz * n + i0 + tid] = y * dscale[(size_t)bz * n + i0 + tid];
     }
 }
 
@@ -630,8 +687,9 @@ int solve_num_blocks(int n) { return (n + NB - 1) / NB; }
 cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     const int n = p->ns, ldl = p->ldl, nbat = p->nbatch, nblk = solve_num_blocks(n);
     double *d_out = p->cpr ? p->coefr : d_coef;      // reduced solution first when the photometric ratio is constrained
-    k_scale_diag<<<dim3((n + 255) / 256, nbat), 256, 0, p->stream>>>(p->M, p->dscale, p->flag, n);
-    k_scale_copy<<<dim3((n + 127) / 128, n + 1, nbat), 128, 0, p->stream>>>(p->M, p->rhs, p->dscale, p->Lf, n, ldl);
+    k_scale_diag<<<dim3((n + 255) / 256, nbat), 256, 0, p->stream>>>(p->M, p->dscale, p->flag, n,
+                                                                    (unsigned long long *)p->ybuf, nblk * NB, kBsSentinel);
+    k_scale_copy<<<dim3((n + 127) / 128, (n + 1 + 15) / 16, nbat), 256, 0, p->stream>>>(p->M, p->rhs, p->dscale, p->Lf, n, ldl);
     p->launches += 2;
     cudaError_t e = cudaFuncSetAttribute(k_chol_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStepSmem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chol_update_row, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
@@ -665,11 +723,10 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
             p->launches++;
         }
     }
-    const int nown_max = (nblk + CS - 1) / CS;
-    const size_t smem = ((size_t)nblk * NB + 4 * (size_t)nown_max * NB) * sizeof(double);
-    e = cudaFuncSetAttribute(k_chol_backsolve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    e = cudaFuncSetAttribute(k_chol_backsolve_lb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBsSmem);
     if (e != cudaSuccess) return e;
-    k_chol_backsolve<<<dim3(CS, nbat), 256, smem, p->stream>>>(p->Lf, p->Winv, p->dscale, d_out, n, ldl, nblk, nown_max);
+    k_chol_backsolve_lb<<<dim3(nblk * nbat), 256, kBsSmem, p->stream>>>(p->Lf, p->Winv, p->dscale, d_out, p->ybuf, n, ldl, nblk,
+                                                                       nbat);
     p->launches++;
     e = cudaGetLastError();
     if (e == cudaSuccess && p->cpr) e = launch_expand_coef(p, p->coefr, d_coef);
