@@ -60,6 +60,18 @@ enum {
  * Builds constant tables on the host and uploads them (synchronous). */
 int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int basis);
 
+/* NEXT-4, rectangular kernels (the delta basis spans L0 x L1 pixels, |alpha| <= (L0-1)/2 along x and
+ * |beta| <= (L1-1)/2 along y; L0, L1 odd, 1 <= L0, L1 <= 33, other restrictions as above with L = max(L0, L1)).
+ * Every layout of this header keeps the enclosing SQUARE L = max(L0, L1): n = F_K*L*L + F_B, lag index
+ * a = (alpha+w)*L + (beta+w) with w = (L-1)/2, and the coefficients outside the rectangle are fixed at zero
+ * (sfft_solve writes them as 0; vectors given to sfft_subtract are used as they are).  The system that is
+ * assembled and solved holds only the free unknowns: sfft_plan_num_solved() = F_K*L0*L1 + F_B of them (fewer under
+ * the constant photometric ratio), in the order of the full layout with the fixed entries removed - for L0 != L1
+ * that is exactly the order t*L0*L1 + (alpha+w0)*L1 + (beta+w1) of the rectangular model.  The lag tables are
+ * formed for the enclosing square, so the cost is that of an L x L kernel.  sfft_plan_create(.., L, ..) is
+ * sfft_plan_create_rect(.., L, L, ..). */
+int sfft_plan_create_rect(sfft_plan **out, int H, int W, int L0, int L1, int DK, int DB, int basis);
+
 /* Number of independent pairs processed per call (default 1).  Must precede set_workspace. */
 int sfft_plan_set_batch(sfft_plan *plan, int nbatch);
 
@@ -68,8 +80,8 @@ int sfft_plan_set_stream(sfft_plan *plan, void *cuda_stream);
 
 /* NEXT-1, constant photometric ratio (PAPER.md:121, 264 -ConstPhotRatio): on = 1 constrains the kernel integral
  * sum_t a_{t,00} T_t(x,y) to a constant (POLY: a_{t,00} = 0 for t >= 1; BSPLINE: all a_{t,00} equal), leaving
- * sfft_plan_num_solved() = n - (F_K - 1) unknowns in the system returned by sfft_get_system (order of the full
- * layout with the centre entries of t >= 1 removed).  Coefficient vectors keep the full layout of n entries,
+ * sfft_plan_num_solved() = (free unknowns) - (F_K - 1) unknowns in the system returned by sfft_get_system (order of
+ * the full layout with the centre entries of t >= 1 removed).  Coefficient vectors keep the full layout of n entries,
  * the constrained ones filled in.  Default 0 (BASELINE.json's unknown counts).  Call before sfft_build_system. */
 int sfft_plan_set_const_phot_ratio(sfft_plan *plan, int on);
 int sfft_plan_num_solved(const sfft_plan *plan);

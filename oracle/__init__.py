@@ -11,6 +11,6 @@ from .binding import (  # noqa: F401
     POLY, BSPLINE, build_library, num_threads, num_terms, num_axis, terms, axis_table,
     num_unknowns, design_matrix, gram, normal_bruteforce, diag_and_rhs, lag_tables, gather,
     normal_from_lags, solve, difference, difference_at, corr_diff_one, weighted_ref,
-    cpr_num_unknowns, cpr_constrain, cpr_expand, mask_fill,
+    cpr_num_unknowns, cpr_constrain, cpr_expand, mask_fill, rect_select, rect_expand,
 )
 from . import decorr  # noqa: F401,E402   (NEXT-3, App. C; numpy)

@@ -226,6 +226,26 @@ def cpr_expand(cr, L, basis, DK, DB):
     return c
 
 
+def rect_select(L0, L1, basis, DK, DB):
+    """NEXT-4, rectangular kernels (the delta basis spans L0 x L1 pixels).  Indices, in the layout of the
+    enclosing square L = max(L0, L1), of the unknowns of the L0 x L1 model: kernel unknowns with |alpha| <= (L0-1)/2
+    and |beta| <= (L1-1)/2, then the background unknowns.  The rectangular model is the square one without the other
+    basis images, so its normal system is the sub-matrix M[sel][:, sel], rhs[sel] (no arithmetic involved)."""
+    L = max(L0, L1)
+    w, w0, w1 = (L - 1) // 2, (L0 - 1) // 2, (L1 - 1) // 2
+    FK, FB = num_terms(basis, DK), num_terms(basis, DB)
+    sel = [t * L * L + (al + w) * L + (be + w) for t in range(FK) for al in range(-w0, w0 + 1) for be in range(-w1, w1 + 1)]
+    sel += [FK * L * L + s for s in range(FB)]
+    return np.array(sel, dtype=np.int64)
+
+
+def rect_expand(cs, L0, L1, basis, DK, DB):
+    """Coefficients of the L0 x L1 model in the layout of the enclosing square (zeros outside the rectangle)."""
+    c = np.zeros(num_unknowns(max(L0, L1), basis, DK, DB))
+    c[rect_select(L0, L1, basis, DK, DB)] = cs
+    return c
+
+
 def mask_fill(R, S, sat_R, sat_S, rd, rb):
     """NEXT-2 (DESIGN g21): joint saturation mask grown by rd, masked pixels replaced by the mean of the
     unmasked pixels in the (2 rb + 1)^2 neighbourhood.  Returns (Rm, Sm, mask uint8)."""

@@ -17,7 +17,7 @@ SFFT_OK, SFFT_ERR_INVALID_ARG, SFFT_ERR_STATE, SFFT_ERR_WORKSPACE, SFFT_ERR_CUDA
 
 # every symbol include/sfft.h declares (checked against the built library by tests/test_abi_and_host.py)
 EXPORTS = [
-    "sfft_plan_create", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_set_corr_route", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
+    "sfft_plan_create", "sfft_plan_create_rect", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_set_corr_route", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
     "sfft_plan_num_kernel_terms", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
     "sfft_subtract", "sfft_mask_fill", "sfft_decorrelate", "sfft_plan_set_reuse_spectra", "sfft_plan_status", "sfft_plan_host_staging_bytes", "sfft_plan_set_host_staging",
@@ -55,6 +55,7 @@ def load_library(build_if_missing=True):
     pvp, pci = ctypes.POINTER(ctypes.c_void_p), ctypes.POINTER(ctypes.c_int)
     sig = {
         "sfft_plan_create": (ci, [pvp, ci, ci, ci, ci, ci, ci]),
+        "sfft_plan_create_rect": (ci, [pvp, ci, ci, ci, ci, ci, ci, ci]),
         "sfft_plan_set_batch": (ci, [vp, ci]),
         "sfft_plan_set_stream": (ci, [vp, vp]),
         "sfft_plan_set_const_phot_ratio": (ci, [vp, ci]),
@@ -109,6 +110,12 @@ def sfft_version():
 def sfft_plan_create(H, W, L, DK, DB, basis):
     h = ctypes.c_void_p()
     st = load_library().sfft_plan_create(ctypes.byref(h), H, W, L, DK, DB, basis)
+    return st, h
+
+
+def sfft_plan_create_rect(H, W, L0, L1, DK, DB, basis):
+    h = ctypes.c_void_p()
+    st = load_library().sfft_plan_create_rect(ctypes.byref(h), H, W, L0, L1, DK, DB, basis)
     return st, h
 
 
@@ -269,7 +276,11 @@ class Plan:
         self.torch = torch
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        st, self.h = sfft_plan_create(H, W, L, DK, DB, _basis_id(basis))
+        if isinstance(L, (tuple, list)):          # rectangular kernel (L0 along x, L1 along y); layouts keep max(L0, L1)
+            st, self.h = sfft_plan_create_rect(H, W, L[0], L[1], DK, DB, _basis_id(basis))
+            L = max(L)
+        else:
+            st, self.h = sfft_plan_create(H, W, L, DK, DB, _basis_id(basis))
         if st != SFFT_OK:
             raise SfftError(st, "sfft_plan_create")
         self.H, self.W, self.L, self.nbatch = H, W, L, nbatch

@@ -14,7 +14,7 @@
 namespace sfft {
 namespace {
 
-struct GatherDims { int FK, FB, L, w, n, nO, LL, ns, cpr, nshare; size_t off_om, off_th, off_la, off_de, tab_size; };
+struct GatherDims { int FK, FB, L, w, n, nO, LL, ns, cpr, nshare, rshare; size_t off_om, off_th, off_la, off_de, tab_size; };
 
 __device__ __forceinline__ double omega(const double *om, const GatherDims &d, int tb, int t, int rho, int eps) {
     if (tb > t) { int q = tb; tb = t; t = q; rho = -rho; eps = -eps; }
@@ -58,29 +58,20 @@ __device__ __forceinline__ double rhs_entry(const double *th, const double *de, 
     return (ab == d.w * d.L + d.w) ? c0 : t0[ab] - c0;
 }
 
-// Full index of reduced unknown r (constant photometric ratio: the centre coefficients of the
-// terms t >= 1 are not free).  The shared unknown sits at r = a0; it stands for `nshare` centre entries
-// t*LL + a0, t < nshare (1: POLY, the others are zero; F_K: BSPLINE, all equal).
-__device__ __forceinline__ int full_index(const GatherDims &d, int r) {
-    const int a0 = d.w * d.L + d.w;
-    if (!d.cpr || r < d.LL) return r;
-    const int na_r = d.FK * d.LL - (d.FK - 1);
-    if (r >= na_r) return r + (d.FK - 1);
-    const int q = r - d.LL, t = 1 + q / (d.LL - 1), a = q % (d.LL - 1);
-    return t * d.LL + (a < a0 ? a : a + 1);
-}
-
+// Reduced systems (constant photometric ratio; rectangular kernels): solved unknown r
+// stands for the full-layout unknown ridx[r] (plan table).  Under the constant photometric ratio the shared unknown
+// at r = rshare stands for `nshare` centre entries t*LL + a0, t < nshare (1: POLY, the others are zero; F_K:
+// BSPLINE, all equal).  M' = C^T M C is formed entry by entry.
 __global__ void k_gather(const double *__restrict__ tab, const double *__restrict__ phi0, const int *__restrict__ kdec,
-                         double *__restrict__ M, double *__restrict__ rhs, GatherDims d) {
+                         const int *__restrict__ ridx, double *__restrict__ M, double *__restrict__ rhs, GatherDims d) {
     const int col = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y, b = blockIdx.z;
     if (col >= d.ns) return;
     const double *tb_ = tab + (size_t)b * d.tab_size;
     const double *om = tb_ + d.off_om, *th = tb_ + d.off_th, *la = tb_ + d.off_la, *de = tb_ + d.off_de;
-    const int a0 = d.w * d.L + d.w;
     // ordered pair (lo <= hi) so that M[row][col] and M[col][row] run the same arithmetic
     const int lo = min(row, col), hi = max(row, col);
-    const int klo = full_index(d, lo), khi = full_index(d, hi);
-    const int nlo = (d.cpr && lo == a0) ? d.nshare : 1, nhi = (d.cpr && hi == a0) ? d.nshare : 1;
+    const int klo = __ldg(&ridx[lo]), khi = __ldg(&ridx[hi]);
+    const int nlo = (lo == d.rshare) ? d.nshare : 1, nhi = (hi == d.rshare) ? d.nshare : 1;
     double v = 0.0;
     for (int p = 0; p < nlo; ++p)
         for (int q = 0; q < nhi; ++q) {
@@ -89,7 +80,7 @@ __global__ void k_gather(const double *__restrict__ tab, const double *__restric
         }
     M[((size_t)b * d.ns + row) * d.ns + col] = v;
     if (row == 0) {   // the first row of CTAs also fills the right-hand side
-        const int kc = full_index(d, col), nc = (d.cpr && col == a0) ? d.nshare : 1;
+        const int kc = __ldg(&ridx[col]), nc = (col == d.rshare) ? d.nshare : 1;
         double r = 0.0;
         for (int q = 0; q < nc; ++q) r += rhs_entry(th, de, d, kc + q * d.LL);
         rhs[(size_t)b * d.ns + col] = r;
@@ -150,34 +141,25 @@ __global__ void __launch_bounds__(128) k_gather_bg(const double *__restrict__ ta
     if (s == 0) rhs[(size_t)b * d.ns + i] = rhs_entry(th, de, d, i);
 }
 
-// c = C c': reduced solution -> full coefficient layout (constrained centre entries filled in)
-__global__ void k_expand_coef(const double *__restrict__ cr, double *__restrict__ c, GatherDims d, int poly) {
+// c = C c': reduced solution -> full coefficient layout (fmap[k] = solved index of full unknown k, -1 = zero)
+__global__ void k_expand_coef(const double *__restrict__ cr, double *__restrict__ c, const int *__restrict__ fmap, int n,
+                              int ns) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
-    if (k >= d.n) return;
-    const int a0 = d.w * d.L + d.w, na = d.FK * d.LL;
-    double v;
-    if (k < na && k % d.LL == a0) {
-        v = (k / d.LL == 0 || !poly) ? cr[(size_t)b * d.ns + a0] : 0.0;
-    } else if (k < na) {
-        const int t = k / d.LL, a = k % d.LL;
-        const int r = t == 0 ? a : d.LL + (t - 1) * (d.LL - 1) + (a < a0 ? a : a - 1);
-        v = cr[(size_t)b * d.ns + r];
-    } else {
-        v = cr[(size_t)b * d.ns + (k - (d.FK - 1))];
-    }
-    c[(size_t)b * d.n + k] = v;
+    if (k >= n) return;
+    const int r = __ldg(&fmap[k]);
+    c[(size_t)b * n + k] = r >= 0 ? cr[(size_t)b * ns + r] : 0.0;
 }
 
 }  // namespace
 
 static GatherDims gather_dims(const sfft_plan *p) {
     return GatherDims{p->FK, p->FB, p->L, p->w, p->n, 2 * p->L - 1, p->L * p->L, p->ns, p->cpr,
-                      p->basis == SFFT_BASIS_POLY ? 1 : p->FK, p->off_om, p->off_th, p->off_la, p->off_de, p->tab_size};
+                      p->basis == SFFT_BASIS_POLY ? 1 : p->FK, p->cpr ? p->rshare : -1, p->off_om, p->off_th, p->off_la, p->off_de, p->tab_size};
 }
 
 cudaError_t launch_gather(sfft_plan *p) {
     GatherDims d = gather_dims(p);
-    if (!p->cpr) {
+    if (!p->reduced) {
         const int nchunk = (d.LL + kGatherRows - 1) / kGatherRows;
         const size_t smem = (size_t)d.nO * d.nO * sizeof(double) + (size_t)d.LL * sizeof(int);
         k_gather_kk<<<dim3(p->FK, p->FK, p->nbatch * nchunk), 256, smem, p->stream>>>(p->tab, p->M, d, nchunk);
@@ -187,14 +169,13 @@ cudaError_t launch_gather(sfft_plan *p) {
         return cudaGetLastError();
     }
     dim3 grid((p->ns + 127) / 128, p->ns, p->nbatch);
-    k_gather<<<grid, 128, 0, p->stream>>>(p->tab, p->dt.phi0, p->dt.kdec, p->M, p->rhs, d);
+    k_gather<<<grid, 128, 0, p->stream>>>(p->tab, p->dt.phi0, p->dt.kdec, p->dt.ridx, p->M, p->rhs, d);
     p->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_expand_coef(sfft_plan *p, const double *d_cr, double *d_coef) {
-    GatherDims d = gather_dims(p);
-    k_expand_coef<<<dim3((p->n + 255) / 256, p->nbatch), 256, 0, p->stream>>>(d_cr, d_coef, d, p->basis == SFFT_BASIS_POLY);
+    k_expand_coef<<<dim3((p->n + 255) / 256, p->nbatch), 256, 0, p->stream>>>(d_cr, d_coef, p->dt.fmap, p->n, p->ns);
     p->launches++;
     return cudaGetLastError();
 }

@@ -233,6 +233,7 @@ void free_tables(sfft_plan *p) {
     cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.lagtw); cudaFree(d.cy); cudaFree(d.fx); cudaFree(d.cq); cudaFree(d.cwr);
     cudaFree(d.phi0);
     cudaFree(d.seqs); cudaFree(d.jobs); cudaFree(d.units);
+    cudaFree(d.ridx); cudaFree(d.fmap);
     cudaFree(d.kdec); cudaFree(d.kti); cudaFree(d.ktj); cudaFree(d.bti); cudaFree(d.btj);
     d = DeviceTables();
 }
@@ -288,6 +289,36 @@ StagingLayout staging_layout(const sfft_plan *p) {
     return l;
 }
 
+// Solved unknowns of a reduced system, in the order of the full (square) layout:
+//   rectangular kernel: the entries with |alpha| > (Lx-1)/2 or |beta| > (Ly-1)/2 are fixed at zero;
+//   constant photometric ratio (DESIGN g20): the centre entries of the terms t >= 1 are not free
+//   (POLY: zero; BSPLINE: equal to the centre entry of t = 0, the shared unknown at solved index `rshare`).
+// ridx[r] = full index of solved unknown r;  fmap[k] = solved index of full unknown k, or -1 (zero).
+cudaError_t build_reduction(sfft_plan *p) {
+    const int L = p->L, w = p->w, LL = L * L, wx = (p->Lx - 1) / 2, wy = (p->Ly - 1) / 2, a0 = w * L + w;
+    std::vector<int> ridx, fmap(p->n, -1);
+    p->rshare = -1;
+    for (int k = 0; k < p->n; ++k) {
+        if (k < p->FK * LL) {
+            const int t = k / LL, a = k % LL, al = a / L - w, be = a % L - w;
+            if (al < -wx || al > wx || be < -wy || be > wy) continue;
+            if (p->cpr && a == a0 && t > 0) continue;
+            if (p->cpr && a == a0) p->rshare = (int)ridx.size();
+        }
+        fmap[k] = (int)ridx.size();
+        ridx.push_back(k);
+    }
+    if (p->cpr && p->basis != SFFT_BASIS_POLY)
+        for (int t = 1; t < p->FK; ++t) fmap[t * LL + a0] = p->rshare;
+    p->ns = (int)ridx.size();
+    p->reduced = p->ns != p->n;
+    cudaFree(p->dt.ridx); cudaFree(p->dt.fmap);
+    p->dt.ridx = p->dt.fmap = nullptr;
+    cudaError_t e = upload(&p->dt.ridx, ridx.data(), ridx.size());
+    if (e == cudaSuccess) e = upload(&p->dt.fmap, fmap.data(), fmap.size());
+    return e;
+}
+
 // a plan is tied to the device it was created on
 bool wrong_device(const sfft_plan *p) {
     int dev = -1;
@@ -300,10 +331,16 @@ bool wrong_device(const sfft_plan *p) {
 extern "C" {
 
 int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int basis) {
+    return sfft_plan_create_rect(out, H, W, L, L, DK, DB, basis);
+}
+
+int sfft_plan_create_rect(sfft_plan **out, int H, int W, int L0, int L1, int DK, int DB, int basis) {
     if (!out) return SFFT_ERR_INVALID_ARG;
     *out = nullptr;
     if (!is_pow2(H) || !is_pow2(W) || H < 32 || H > 8192 || W < 64 || W > 8192) return SFFT_ERR_INVALID_ARG;
-    if (L < 1 || L > 33 || (L % 2) == 0 || 2 * L - 1 > std::min(H, W)) return SFFT_ERR_INVALID_ARG;
+    if (L0 < 1 || L0 > 33 || (L0 % 2) == 0 || L1 < 1 || L1 > 33 || (L1 % 2) == 0) return SFFT_ERR_INVALID_ARG;
+    const int L = std::max(L0, L1);      // every table is built for the enclosing square; the gather keeps the rectangle
+    if (2 * L - 1 > std::min(H, W)) return SFFT_ERR_INVALID_ARG;
     if (DK < 0 || DB < 0 || DK > 8 || DB > 8) return SFFT_ERR_INVALID_ARG;
     if (basis != SFFT_BASIS_POLY && basis != SFFT_BASIS_BSPLINE) return SFFT_ERR_INVALID_ARG;
     int ndev = 0;
@@ -313,6 +350,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     if (!p) return SFFT_ERR_INVALID_ARG;
     if (cudaGetDevice(&p->device) != cudaSuccess) { cudaGetLastError(); delete p; return SFFT_ERR_CUDA; }
     p->H = H; p->W = W; p->L = L; p->w = (L - 1) / 2; p->DK = DK; p->DB = DB; p->basis = basis;
+    p->Lx = L0; p->Ly = L1;
     p->Nh = W / 2;
     p->nKa = num_axis(basis, DK); p->nBa = num_axis(basis, DB);
     term_list(basis, DK, p->kti, p->ktj);
@@ -413,6 +451,7 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
     for (int t = 0; t < p->FK; ++t)
         for (int a = 0; a < L * L; ++a) kdec[(size_t)t * L * L + a] = (t << 16) | ((a / L) << 8) | (a % L);
     UP(kdec, kdec);
+    if (e == cudaSuccess) e = build_reduction(p);
     UP(seqs, p->seqs); UP(jobs, p->jobs); UP(units, p->units);
     UP(kti, p->kti); UP(ktj, p->ktj); UP(bti, p->bti); UP(btj, p->btj);
 #undef UP
@@ -441,9 +480,11 @@ int sfft_plan_set_batch(sfft_plan *p, int nbatch) {
 
 int sfft_plan_set_const_phot_ratio(sfft_plan *p, int on) {
     if (!p || (on != 0 && on != 1)) return SFFT_ERR_INVALID_ARG;
+    if (wrong_device(p)) return SFFT_ERR_STATE;
     p->cpr = on;
-    p->ns = on ? p->n - (p->FK - 1) : p->n;
     p->built = p->solved = false;
+    cudaError_t e = build_reduction(p);
+    if (e != cudaSuccess) return fail_cuda(p, e);
     return SFFT_OK;
 }
 

@@ -72,6 +72,8 @@ struct DeviceTables {
     LagUnit *units = nullptr;
     int *kti = nullptr, *ktj = nullptr, *bti = nullptr, *btj = nullptr;
     int *kdec = nullptr;        // [FK*L*L]         t << 16 | (alpha+w) << 8 | (beta+w) of every kernel unknown (gather.cu)
+    int *ridx = nullptr;        // [ns]             full-layout index of every solved unknown (reduced systems: cpr, rectangular kernels)
+    int *fmap = nullptr;        // [n]              solved index of every full-layout unknown, -1 = fixed at zero
 };
 
 }  // namespace sfft
@@ -82,6 +84,9 @@ struct sfft_plan {
     bool corr_os = false; int os_hop = 0;   // the build takes the sectioned correlation (set by choose_split), its hop length
     int corr_route = 0;  // 0: chosen by the plan, 1: direct lag sums (corr.cu), 2: sectioned FFT64 correlation (corr_os.cu)
     int cpr = 0;         // constant photometric ratio: centre coefficients of the terms t >= 1 not free
+    int Lx = 0, Ly = 0;  // kernel extent along x / y (rectangular kernels); L = max(Lx, Ly) is the enclosing square
+    bool reduced = false;   // the solved system is a reduction of the full square layout (cpr and / or Lx != Ly)
+    int rshare = -1;     // solved index of the shared centre unknown under cpr
     int ns = 0;          // solved unknowns: n, or n - (FK - 1) under cpr
     int nimg = 0;        // spectrum stack depth per batch entry: nKa weighted-y images + S
     int nseq = 0;        // FK + 1 column sequences (kernel terms, then S)

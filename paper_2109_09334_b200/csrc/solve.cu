@@ -686,7 +686,7 @@ int solve_num_blocks(int n) { return (n + NB - 1) / NB; }
 
 cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     const int n = p->ns, ldl = p->ldl, nbat = p->nbatch, nblk = solve_num_blocks(n);
-    double *d_out = p->cpr ? p->coefr : d_coef;      // reduced solution first when the photometric ratio is constrained
+    double *d_out = p->reduced ? p->coefr : d_coef;      // reduced solution first when the photometric ratio is constrained
     k_scale_diag<<<dim3((n + 255) / 256, nbat), 256, 0, p->stream>>>(p->M, p->dscale, p->flag, n,
                                                                     (unsigned long long *)p->ybuf, nblk * NB, kBsSentinel);
     k_scale_copy<<<dim3((n + 127) / 128, (n + 1 + 15) / 16, nbat), 256, 0, p->stream>>>(p->M, p->rhs, p->dscale, p->Lf, n, ldl);
@@ -729,7 +729,7 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
                                                                        nbat);
     p->launches++;
     e = cudaGetLastError();
-    if (e == cudaSuccess && p->cpr) e = launch_expand_coef(p, p->coefr, d_coef);
+    if (e == cudaSuccess && p->reduced) e = launch_expand_coef(p, p->coefr, d_coef);
     return e;
 }
 

@@ -324,6 +324,49 @@ def test_parity_constant_photometric_ratio(cuda_device, cfg, H, W, L, basis, DK,
     plan.close()
 
 
+@pytest.mark.parametrize("cfg,H,W,L0,L1,basis,DK,DB,cpr", [
+    (2, 128, 256, 5, 9, "poly", 2, 1, False),       # wider along y; direct-route subtract
+    (2, 64, 1024, 13, 7, "poly", 1, 1, False),      # wider along x; Fourier-route subtract (W >= 1024, L = 13)
+    (5, 128, 128, 3, 5, "bspline", 1, 0, False),    # B-spline weights, direct lag sums
+    (2, 128, 128, 7, 3, "poly", 2, 2, True),        # together with the constant photometric ratio
+    (2, 64, 64, 1, 5, "poly", 1, 1, False),         # a single column of lags (L0 = 1)
+])
+def test_parity_rectangular_kernel(cuda_device, cfg, H, W, L0, L1, basis, DK, DB, cpr):
+    """NEXT-4 (the delta basis spans L0 x L1 pixels): system of the free unknowns, solution in the
+    layout of the enclosing square (zeros outside the rectangle) and difference image, against the oracle's
+    rectangular model (pinned to a direct L0 x L1 design matrix in tests/test_oracle_pins.py)."""
+    import torch
+    p = synth.make_pair(cfg, H=H, W=W)
+    bid, L = _bid(basis), max(L0, L1)
+    Mf, rf = oracle.normal_from_lags(p.R, p.S, L, bid, DK, DB)
+    sel = oracle.rect_select(L0, L1, bid, DK, DB)
+    FK, FB = oracle.num_terms(bid, DK), oracle.num_terms(bid, DB)
+    if cpr:
+        # constant kernel integral (POLY, PAPER.md:121): the centre coefficients of the terms t >= 1 are zero as well
+        a0 = ((L - 1) // 2) * L + (L - 1) // 2
+        sel = np.array([k for k in sel if not (k < FK * L * L and k % (L * L) == a0 and k // (L * L) > 0)])
+    Mo, ro = Mf[np.ix_(sel, sel)], rf[sel]
+    cs = oracle.solve(Mo, ro)
+    co = np.zeros(Mf.shape[0])
+    co[sel] = cs
+    Do = oracle.difference(p.R, p.S, co, L, bid, DK, DB)
+    plan = B.Plan(p.H, p.W, (L0, L1), DK, DB, basis, const_phot_ratio=cpr)
+    assert plan.n == Mf.shape[0] and plan.ns == len(sel) == FK * L0 * L1 + FB - (FK - 1 if cpr else 0)
+    dR, dS = torch.from_numpy(p.R).cuda(), torch.from_numpy(p.S).cuda()
+    plan.build_system(dR, dS)
+    coef = plan.solve()
+    D = plan.subtract(coef, dR, dS)
+    plan.status()
+    M, rhs = plan.system()
+    _check_system(M[0].cpu().numpy(), rhs[0].cpu().numpy(), Mo, ro, p.S)
+    c = coef[0].cpu().numpy()
+    _check_coef(c, co, Mf.shape[0] - FB)
+    fixed = np.setdiff1d(np.arange(Mf.shape[0]), sel)
+    assert np.all(c[fixed] == 0.0)
+    assert np.max(np.abs(D.cpu().numpy() - Do)) <= TOL_D * p.sigma
+    plan.close()
+
+
 def test_identical_images(cuda_device):
     """S = R  =>  a_{0,centre} = 1, everything else 0, D = 0 (degenerate but full-rank case)."""
     import torch
@@ -619,6 +662,12 @@ def test_argument_and_state_errors(cuda_device):
                 (64, 64, 33, 1, 1, 0), (16, 128, 3, 1, 1, 0)]:
         st, _ = B.sfft_plan_create(*bad)
         assert st == B.SFFT_ERR_INVALID_ARG, bad
+    for bad in [(128, 128, 4, 7, 1, 1, 0), (128, 128, 7, 35, 1, 1, 0), (64, 64, 3, 33, 1, 1, 0), (128, 128, 0, 3, 1, 1, 0)]:
+        st, _ = B.sfft_plan_create_rect(*bad)
+        assert st == B.SFFT_ERR_INVALID_ARG, bad
+    st, h = B.sfft_plan_create_rect(128, 128, 3, 7, 1, 1, 0)
+    assert st == B.SFFT_OK and B.sfft_plan_num_unknowns(h) == 150 and B.sfft_plan_num_solved(h) == 3 * 21 + 3
+    B.sfft_plan_destroy(h)
     st, h = B.sfft_plan_create(128, 128, 7, 1, 1, 0)
     assert st == B.SFFT_OK and B.sfft_plan_num_unknowns(h) == 150
     x = torch.zeros(128 * 128, dtype=torch.float64, device="cuda")

@@ -614,3 +614,37 @@ def test_decorrelation_whitens_the_noise():
     for lag in [(0, 1), (1, 0), (1, 1), (2, 0), (0, 3)]:
         assert abs(acorr(out, *lag)) < 5.0 / T                                     # white after (sampling error 1/T)
     assert abs(out.var() / (vS + vR * K.sum() ** 2) - 1.0) < 0.05
+
+
+# --------------------------------------------------------------------------- NEXT-4: rectangular kernels
+
+@pytest.mark.parametrize("L0,L1", [(3, 7), (5, 1)])
+def test_rectangular_kernel_selection_vs_direct_design_matrix(L0, L1):
+    """PAPER.md:86 (the delta basis spans L0 x L1 pixels): the oracle's rectangular system (a selection from the
+    enclosing square's) against a design matrix built directly for the L0 x L1 lag set with np.roll, its Gram matrix
+    and numpy lstsq; the expanded solution subtracts like the direct model.  Catches swapped axes (alpha <-> beta),
+    a selection that keeps the wrong rows, and a wrong expansion."""
+    H, W, DK, DB = 16, 20, 1, 1
+    w0, w1 = (L0 - 1) // 2, (L1 - 1) // 2
+    R, S = _rand_pair(H, W, 11)
+    cols = []
+    for T in _poly_T(H, W, DK):
+        Rt = T * R
+        for al in range(-w0, w0 + 1):
+            for be in range(-w1, w1 + 1):
+                sh = np.roll(Rt, (al, be), axis=(0, 1))          # sh(x,y) = Rt(x-al, y-be)
+                cols.append((sh if (al, be) == (0, 0) else sh - Rt).ravel())
+    cols += [T.ravel() for T in _poly_T(H, W, DB)]
+    Phi = np.array(cols)
+    L = max(L0, L1)
+    sel = oracle.rect_select(L0, L1, POLY, DK, DB)
+    assert len(sel) == Phi.shape[0] == 3 * L0 * L1 + 3 and np.all(np.diff(sel) > 0)
+    M, rhs = oracle.normal_from_lags(R, S, L, POLY, DK, DB)
+    Ms, rs = M[np.ix_(sel, sel)], rhs[sel]
+    np.testing.assert_allclose(Ms, Phi @ Phi.T, rtol=1e-11, atol=1e-5)
+    np.testing.assert_allclose(rs, Phi @ S.ravel(), rtol=1e-11, atol=1e-5)
+    cs = oracle.solve(Ms, rs)
+    cl = np.linalg.lstsq(Phi.T, S.ravel(), rcond=None)[0]
+    np.testing.assert_allclose(cs, cl, rtol=0, atol=1e-9 * np.max(np.abs(cl)))
+    D = oracle.difference(R, S, oracle.rect_expand(cs, L0, L1, POLY, DK, DB), L, POLY, DK, DB)
+    np.testing.assert_allclose(D, S - (Phi.T @ cl).reshape(H, W), rtol=0, atol=1e-8)
