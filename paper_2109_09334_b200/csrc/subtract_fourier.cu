@@ -77,7 +77,11 @@ struct FirDims { int H, Nh, nimg, nKa, FK, NO, pad; };
 // Output rows [xo0, xo0+NO) of a warp need the source rows xo0-w-pad .. xo0+NO-1+w, processed 4 at a time:
 // source row x'+q (q<4) adds khat_{t,a} z_t(x'+q) to output x'+q+a, i.e. to acc[q + ai] of a window that
 // starts at output x'-w; after the step the first four window entries are complete and leave.
-template <int L>
+// PDK >= 1: polynomial basis of total degree PDK (terms t(i,j), i outer: f_i(x) = u_x^i on the spectrum of image j).  The
+// terms are grouped by image, c_{j,a}(x') = sum_i khat_{(i,j),a} u_x'^i is formed per source row (f_0 = 1 costs nothing)
+// and ONE complex multiply-add per (image, tap, row) follows: 72 instead of 96 FMA per row and tap at DK = 2.
+// PDK = -1: any basis, one complex multiply-add per (term, tap, row) on the pre-weighted rows.
+template <int L, int PDK>
 __global__ void __launch_bounds__(kFirCols *kFirWarps, 2)
 k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const Seq *__restrict__ seqs,
         const double2 *__restrict__ khat, double2 *mhat, FirDims d) {
@@ -133,22 +137,61 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
         __syncwarp();
         const double2 *r = rtw + (size_t)(g & 1) * bufstride;
         const int xg = xs0 + 4 * g;
-        for (int t = 0; t < FK; ++t) {
-            const Seq sq = sseq[t];
-            double2 z[4];
+        if constexpr (PDK >= 1) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const double f = fw[sq.xw * 4 + q];
-                const double2 rv = r[(sq.img * 4 + q) * kFirCols];
-                z[q] = make_double2(f * rv.x, f * rv.y);
+            for (int j = 0; j <= PDK; ++j) {
+                // operands of the four rows: acc.x += c.x p0 + c.y p1, acc.y += c.x p2 + c.y p3 (the packed column 0 is
+                // two real filters: no cross terms)
+                double pz[4][4], f[PDK][4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const double2 rv = r[(j * 4 + q) * kFirCols];
+                    pz[q][0] = rv.x; pz[q][1] = packed ? 0.0 : -rv.y; pz[q][2] = packed ? 0.0 : rv.y; pz[q][3] = packed ? rv.y : rv.x;
+#pragma unroll
+                    for (int i = 1; i <= PDK - j; ++i) f[i - 1][q] = fw[i * 4 + q];
+                }
+                const double2 *kp = kh + col;
+#pragma unroll
+                for (int ai = 0; ai < L; ++ai) {
+                    double2 c[4];
+                    const double2 k0 = kp[(size_t)(ai * FK + j) * kFirCols];          // t(0, j) = j
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) c[q] = k0;
+#pragma unroll
+                    for (int i = 1; i <= PDK - j; ++i) {
+                        // t(i, j) = sum_{i' < i} (PDK + 1 - i') + j
+                        const double2 k = kp[(size_t)(ai * FK + i * (PDK + 1) - i * (i - 1) / 2 + j) * kFirCols];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) { c[q].x = fma(k.x, f[i - 1][q], c[q].x); c[q].y = fma(k.y, f[i - 1][q], c[q].y); }
+                    }
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        double2 &a = acc[ai + q];
+                        a.x = fma(c[q].x, pz[q][0], a.x);
+                        a.y = fma(c[q].x, pz[q][2], a.y);
+                        a.x = fma(c[q].y, pz[q][1], a.x);
+                        a.y = fma(c[q].y, pz[q][3], a.y);
+                    }
+                }
             }
-            const double2 *kp = kh + t * kFirCols + col;
-#pragma unroll
-            for (int ai = 0; ai < L; ++ai) {
-                const double2 k = kp[(size_t)ai * FK * kFirCols];
-                const double kb = packed ? 0.0 : -k.y, kc = packed ? k.y : k.x, kd = packed ? 0.0 : k.y;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) cmac(acc[ai + q], k.x, kb, kc, kd, z[q]);
+        } else {
+            for (int t = 0; t < FK; ++t) {
+                const Seq sq = sseq[t];
+                double2 z[4];
+    #pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const double f = fw[sq.xw * 4 + q];
+                    const double2 rv = r[(sq.img * 4 + q) * kFirCols];
+                    z[q] = make_double2(f * rv.x, f * rv.y);
+                }
+                const double2 *kp = kh + t * kFirCols + col;
+    #pragma unroll
+                for (int ai = 0; ai < L; ++ai) {
+                    const double2 k = kp[(size_t)ai * FK * kFirCols];
+                    const double kb = packed ? 0.0 : -k.y, kc = packed ? k.y : k.x, kd = packed ? 0.0 : k.y;
+    #pragma unroll
+                    for (int q = 0; q < 4; ++q) cmac(acc[ai + q], k.x, kb, kc, kd, z[q]);
+                }
             }
         }
         if (g >= lead) {
@@ -255,9 +298,9 @@ size_t fir_smem(const sfft_plan *p) {
            (size_t)kFirWarps * 2 * 4 * kFirMaxNKa * sizeof(double);
 }
 
-template <int L>
-cudaError_t launch_fir(sfft_plan *p, const FirDims &d, int ny) {
-    auto kern = k_fir_x<L>;
+template <int L, int PDK>
+cudaError_t launch_fir_k(sfft_plan *p, const FirDims &d, int ny) {
+    auto kern = k_fir_x<L, PDK>;
     const size_t smem = fir_smem(p);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -265,6 +308,14 @@ cudaError_t launch_fir(sfft_plan *p, const FirDims &d, int ny) {
         p->rhat, p->dt.xwt, p->dt.seqs, p->khat, p->rhat + (size_t)p->nKa * p->H * p->Nh, d);
     p->launches++;
     return cudaGetLastError();
+}
+
+template <int L>
+cudaError_t launch_fir(sfft_plan *p, const FirDims &d, int ny) {
+    // the grouped form needs the plan's polynomial term order (seqs[t] = (image j, x-power i), i outer)
+    if (p->basis == SFFT_BASIS_POLY && p->DK == 1) return launch_fir_k<L, 1>(p, d, ny);
+    if (p->basis == SFFT_BASIS_POLY && p->DK == 2) return launch_fir_k<L, 2>(p, d, ny);
+    return launch_fir_k<L, -1>(p, d, ny);
 }
 
 }  // namespace
