@@ -62,12 +62,13 @@ __device__ __forceinline__ void fft64_group(double2 (&v)[8], Slot ex, const doub
 // Transform phase of one step for one lane: rows t + 8r of the hop starting at staged row r0 (image row x0).
 //   MODE : 0 complex column, 1 DC part (.x) and 2 Nyquist part (.y) of the packed column 0, run as real columns
 //   SIDE : 0 = Q (64-row window), 1 = P (only the nkeep first rows, the rest of the window zero)
-//   XP   : power of the x-weight f_i(x) = u_x^i, u_x = (2x+1)/H - 1 (exact in double; DESIGN g8).  Computed here
+//   XP   : power of the x-weight f_i(x) = u_x^i, u_x = (2x+1)/H - 1 (exact in double for H a power of two, within an
+//          ulp or two otherwise; DESIGN g8).  Computed here
 //          instead of read from the plan's table: u is exact and u*u is its correctly rounded square, which is
 //          what the table holds, so both routes weight with the very same numbers (a1).
 template <int MODE, int SIDE, int XP>
 __device__ __forceinline__ void os_transform(const double2 *rw, double2 *dst, const double2 *tw, int t, int nkeep, int x0,
-                                             int hmask, double uscale, double uoff) {
+                                             int H, int hmask, double uscale, double uoff) {
     double2 v[8];
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
@@ -75,7 +76,7 @@ __device__ __forceinline__ void os_transform(const double2 *rw, double2 *dst, co
         if (MODE == 1) a.y = 0.0;
         if (MODE == 2) { a.x = a.y; a.y = 0.0; }
         if (XP > 0) {
-            const double u = fma((double)((x0 + t + 8 * r) & hmask), uscale, uoff), w = XP == 1 ? u : u * u;
+            const double u = fma((double)wrap_index(x0 + t + 8 * r, H, hmask), uscale, uoff), w = XP == 1 ? u : u * u;
             a.x *= w;
             if (MODE == 0) a.y *= w;
         }
@@ -89,10 +90,10 @@ __device__ __forceinline__ void os_transform(const double2 *rw, double2 *dst, co
 
 template <int MODE, int SIDE>
 __device__ __forceinline__ void os_transform_xp(int xp, const double2 *rw, double2 *dst, const double2 *tw, int t, int nkeep,
-                                                int x0, int hmask, double uscale, double uoff) {
-    if (xp <= 0) os_transform<MODE, SIDE, 0>(rw, dst, tw, t, nkeep, x0, hmask, uscale, uoff);
-    else if (xp == 1) os_transform<MODE, SIDE, 1>(rw, dst, tw, t, nkeep, x0, hmask, uscale, uoff);
-    else os_transform<MODE, SIDE, 2>(rw, dst, tw, t, nkeep, x0, hmask, uscale, uoff);
+                                                int x0, int H, int hmask, double uscale, double uoff) {
+    if (xp <= 0) os_transform<MODE, SIDE, 0>(rw, dst, tw, t, nkeep, x0, H, hmask, uscale, uoff);
+    else if (xp == 1) os_transform<MODE, SIDE, 1>(rw, dst, tw, t, nkeep, x0, H, hmask, uscale, uoff);
+    else os_transform<MODE, SIDE, 2>(rw, dst, tw, t, nkeep, x0, H, hmask, uscale, uoff);
 }
 
 // grid: x = column slot c (0: DC of packed column 0, Nh: its Nyquist part, else column c), y = x-range part, z = batch
@@ -108,6 +109,7 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
     const int c = blockIdx.x, xs = blockIdx.y, bz = blockIdx.z;
     const int col = (MODE == 2) ? 0 : c;
     const int H = d.H, HOP = d.HOP, RS = d.RS, STEP = kOsHops * d.HOP;
+    const int hmask = (H & (H - 1)) == 0 ? H - 1 : -1;     // wrap by mask when H is a power of two
 
     if (tid < 64) {
         double s, co;
@@ -130,7 +132,7 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
         const int x0 = xb + s * STEP;
         double2 *rbuf = raw + (s & 1) * kOsMaxImg * RS;
         for (int img = img0, r = rr0; img < d.nimg;) {
-            const int x = (x0 + r) & (H - 1);
+            const int x = wrap_index(x0 + r, H, hmask);
             const unsigned dst = (unsigned)__cvta_generic_to_shared(&rbuf[img * RS + r]);
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(&rb[((size_t)img * H + x) * d.Nh]));
             r += npf;
@@ -162,8 +164,8 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
             const double2 *rw = raw + (b * kOsMaxImg + sq.img) * RS + r0;
             double2 *dst = (side ? SP : SQ) + b * kOsSpec + seq * 4 + hop;
             // the conj side keeps only the HOP rows of this hop that lie inside the CTA's x-range
-            if (side) os_transform_xp<MODE, 1>(sq.xw, rw, dst, tw, t, min(HOP, xe - x0), x0, H - 1, uscale, uoff);
-            else os_transform_xp<MODE, 0>(sq.xw, rw, dst, tw, t, 64, x0, H - 1, uscale, uoff);
+            if (side) os_transform_xp<MODE, 1>(sq.xw, rw, dst, tw, t, min(HOP, xe - x0), x0, H, hmask, uscale, uoff);
+            else os_transform_xp<MODE, 0>(sq.xw, rw, dst, tw, t, 64, x0, H, hmask, uscale, uoff);
         }
         asm volatile("cp.async.wait_group 0;" ::: "memory");      // the rows of step s+1 (fetched during step s-1) landed
         __syncthreads();                                           // spectra of step s complete; raw[b] and S[b^1] free

@@ -19,7 +19,7 @@ __global__ void k_mask_rows(const double *__restrict__ R, const double *__restri
     const size_t row = ((size_t)b * H + x) * W;
     int m = 0;
     for (int dy = -rd; dy <= rd; ++dy) {
-        const int yy = (y + dy + W) & (W - 1);
+        const int yy = wrap_index(y + dy, W, (W & (W - 1)) == 0 ? W - 1 : -1);
         m |= (__ldg(&R[row + yy]) >= satR) | (__ldg(&S[row + yy]) >= satS);
     }
     t[row + y] = (unsigned char)m;
@@ -31,7 +31,7 @@ __global__ void k_mask_cols(const unsigned char *__restrict__ t, unsigned char *
     if (y >= W) return;
     const size_t img = (size_t)b * H * W;
     int m = 0;
-    for (int dx = -rd; dx <= rd; ++dx) m |= t[img + (size_t)((x + dx + H) & (H - 1)) * W + y];
+    for (int dx = -rd; dx <= rd; ++dx) m |= t[img + (size_t)(wrap_index(x + dx, H, (H & (H - 1)) == 0 ? H - 1 : -1)) * W + y];
     mask[img + (size_t)x * W + y] = (unsigned char)m;
 }
 
@@ -80,9 +80,9 @@ __global__ void k_fill(const double *R, const double *S, const unsigned char *__
     double sr = 0.0, ss = 0.0;
     int cnt = 0;
     for (int dx = -rb; dx <= rb; ++dx) {
-        const size_t row = img + (size_t)((x + dx + H) & (H - 1)) * W;
+        const size_t row = img + (size_t)(wrap_index(x + dx, H, (H & (H - 1)) == 0 ? H - 1 : -1)) * W;
         for (int dy = -rb; dy <= rb; ++dy) {
-            const size_t q = row + ((y + dy + W) & (W - 1));
+            const size_t q = row + (wrap_index(y + dy, W, (W & (W - 1)) == 0 ? W - 1 : -1));
             if (!mask[q]) { sr += R[q]; ss += S[q]; ++cnt; }
         }
     }

@@ -230,7 +230,7 @@ int fail_cuda(sfft_plan *p, cudaError_t e) {
 
 void free_tables(sfft_plan *p) {
     DeviceTables &d = p->dt;
-    cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.lagtw); cudaFree(d.cy); cudaFree(d.fx); cudaFree(d.cq); cudaFree(d.cwr);
+    cudaFree(d.xwt); cudaFree(d.gK); cudaFree(d.gB); cudaFree(d.twW); cudaFree(d.twM); cudaFree(d.chirp); cudaFree(d.bhat); cudaFree(d.lagtw); cudaFree(d.cy); cudaFree(d.fx); cudaFree(d.cq); cudaFree(d.cwr);
     cudaFree(d.phi0);
     cudaFree(d.seqs); cudaFree(d.jobs); cudaFree(d.units);
     cudaFree(d.ridx); cudaFree(d.fmap);
@@ -337,7 +337,9 @@ int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int b
 int sfft_plan_create_rect(sfft_plan **out, int H, int W, int L0, int L1, int DK, int DB, int basis) {
     if (!out) return SFFT_ERR_INVALID_ARG;
     *out = nullptr;
-    if (!is_pow2(H) || !is_pow2(W) || H < 32 || H > 8192 || W < 64 || W > 8192) return SFFT_ERR_INVALID_ARG;
+    if (H < 32 || H > 8192 || W < 64 || W > 8192 || (W & 1)) return SFFT_ERR_INVALID_ARG;
+    const bool pow2 = is_pow2(H) && is_pow2(W);
+    if (!is_pow2(W) && W > 4096) return SFFT_ERR_INVALID_ARG;      // chirp-z row transform: M = 2^k >= W - 1, M <= 4096
     if (L0 < 1 || L0 > 33 || (L0 % 2) == 0 || L1 < 1 || L1 > 33 || (L1 % 2) == 0) return SFFT_ERR_INVALID_ARG;
     const int L = std::max(L0, L1);      // every table is built for the enclosing square; the gather keeps the rectangle
     if (2 * L - 1 > std::min(H, W)) return SFFT_ERR_INVALID_ARG;
@@ -351,6 +353,8 @@ int sfft_plan_create_rect(sfft_plan **out, int H, int W, int L0, int L1, int DK,
     if (cudaGetDevice(&p->device) != cudaSuccess) { cudaGetLastError(); delete p; return SFFT_ERR_CUDA; }
     p->H = H; p->W = W; p->L = L; p->w = (L - 1) / 2; p->DK = DK; p->DB = DB; p->basis = basis;
     p->Lx = L0; p->Ly = L1;
+    p->pow2 = pow2;
+    if (!is_pow2(W)) { p->bsM = 512; while (p->bsM < W - 1) p->bsM *= 2; }
     p->Nh = W / 2;
     p->nKa = num_axis(basis, DK); p->nBa = num_axis(basis, DB);
     term_list(basis, DK, p->kti, p->ktj);
@@ -358,6 +362,8 @@ int sfft_plan_create_rect(sfft_plan **out, int H, int W, int L0, int L1, int DK,
     p->FK = (int)p->kti.size(); p->FB = (int)p->bti.size();
     p->n = p->FK * L * L + p->FB;
     p->ns = p->n;
+    // frames that are not powers of two run on the sectioned lag correlation and the direct subtract only
+    if (!pow2 && (basis != SFFT_BASIS_POLY || p->FK + 1 > 8 || p->nKa > 3)) { delete p; return SFFT_ERR_INVALID_ARG; }
     p->nimg = p->nKa + 1;
     p->ldl = (p->n + 1 + 7) & ~7;
     p->LT = subtract_kpad(p->nKa, L);
@@ -382,7 +388,7 @@ int sfft_plan_create_rect(sfft_plan **out, int H, int W, int L0, int L1, int DK,
     std::vector<double2> lagtw((size_t)(p->Nh + 1) * L);
     for (int m = 0; m <= p->Nh; ++m)
         for (int k = 0; k < L; ++k) {
-            int idx = (int)(((long long)m * k) & (W - 1));
+            int idx = (int)(((long long)m * k) % W);
             long double wm = (m == 0 || m == p->Nh) ? 1.0L : 2.0L;
             lagtw[(size_t)m * L + k] = make_double2((double)(wm * cw[idx] / W), (double)(wm * -sw[idx] / W));
         }
@@ -395,13 +401,13 @@ int sfft_plan_create_rect(sfft_plan **out, int H, int W, int L0, int L1, int DK,
         for (int j = 0; j < p->nBa; ++j)
             for (int b = 0; b < L; ++b) {
                 double *row = &cy[((size_t)(jb * p->nBa + j) * L + b) * W];
-                for (int y = 0; y < W; ++y) row[y] = gK[(size_t)jb * W + y] * gB[(size_t)j * W + ((y + b - wl + W) & (W - 1))];
+                for (int y = 0; y < W; ++y) row[y] = gK[(size_t)jb * W + y] * gB[(size_t)j * W + ((y + b - wl + W) % W)];
             }
     for (int ib = 0; ib < p->nKa; ++ib)
         for (int i = 0; i < p->nBa; ++i)
             for (int a = 0; a < L; ++a) {
                 double *row = &fx[((size_t)(ib * p->nBa + i) * L + a) * H];
-                for (int x = 0; x < H; ++x) row[x] = fK[(size_t)ib * H + x] * fB[(size_t)i * H + ((x + a - wl + H) & (H - 1))];
+                for (int x = 0; x < H; ++x) row[x] = fK[(size_t)ib * H + x] * fB[(size_t)i * H + ((x + a - wl + H) % H)];
             }
     // POLY shortcut of the first moment contraction (moments.cu): u(y+beta) = u(y) + beta*delta away from the wrap, so
     //   Q[x][(jb,j,beta)] = sum_k C(j,k) (beta delta)^(j-k) mu_{jb+k}(x) + sum_{wrapping y} R(x,y) u^jb [u(y')^j - (u + beta delta)^j]
@@ -443,10 +449,40 @@ int sfft_plan_create_rect(sfft_plan **out, int H, int W, int L0, int L1, int DK,
                     (double)(sx[p->bti[sb] * p->nBa + p->bti[s]] * sy[p->btj[sb] * p->nBa + p->btj[s]]);
     }
 
+    // chirp-z (Bluestein) row DFT for W not a power of two: with N = W/2 and c[n] = exp(-i pi n^2 / N),
+    //   Z[k] = sum_n z[n] exp(-2 pi i n k / N) = c[k] sum_n (z[n] c[n]) conj(c[k-n]),
+    // a circular convolution of length M >= 2N - 1 run with two M-point transforms (rowfft.cu)
+    std::vector<double2> twM, chirp, bhat;
+    if (p->bsM) {
+        const int M = p->bsM, N = W / 2;
+        const long double pi = 3.141592653589793238462643383279L;
+        twM.resize(2 * (size_t)M); chirp.resize(N); bhat.resize(M);
+        for (int k = 0; k < 2 * M; ++k) twM[k] = make_double2((double)cosl(pi * k / M), (double)-sinl(pi * k / M));
+        std::vector<long double> br(M, 0.0L), bi(M, 0.0L), tc(M), ts(M);
+        for (int n = 0; n < N; ++n) {
+            const long long q = ((long long)n * n) % (2LL * N);          // n^2 mod 2N: the angle is exact
+            const long double cr = cosl(pi * q / N), ci = sinl(pi * q / N);
+            chirp[n] = make_double2((double)cr, (double)-ci);
+            br[n] = cr; bi[n] = ci;
+            if (n) { br[M - n] = cr; bi[M - n] = ci; }
+        }
+        for (int k = 0; k < M; ++k) { tc[k] = cosl(2.0L * pi * k / M); ts[k] = -sinl(2.0L * pi * k / M); }
+        for (int q = 0; q < M; ++q) {
+            long double sr = 0.0L, si = 0.0L;
+            for (int m = 0; m < M; ++m) {
+                if (br[m] == 0.0L && bi[m] == 0.0L) continue;
+                const int idx = (int)(((long long)q * m) & (M - 1));
+                sr += br[m] * tc[idx] - bi[m] * ts[idx];
+                si += br[m] * ts[idx] + bi[m] * tc[idx];
+            }
+            bhat[q] = make_double2((double)sr, (double)si);
+        }
+    }
+
     cudaError_t e = cudaSuccess;
     DeviceTables &d = p->dt;
 #define UP(dst, vec) if (e == cudaSuccess) e = upload(&d.dst, vec.data(), vec.size())
-    UP(xwt, xwt); UP(gK, gK); UP(gB, gB); UP(twW, twW); UP(lagtw, lagtw); UP(cy, cy); UP(fx, fx); UP(cq, cq); UP(cwr, cwr); UP(phi0, phi0);
+    UP(xwt, xwt); UP(gK, gK); UP(gB, gB); UP(twW, twW); UP(twM, twM); UP(chirp, chirp); UP(bhat, bhat); UP(lagtw, lagtw); UP(cy, cy); UP(fx, fx); UP(cq, cq); UP(cwr, cwr); UP(phi0, phi0);
     std::vector<int> kdec((size_t)p->FK * L * L);
     for (int t = 0; t < p->FK; ++t)
         for (int a = 0; a < L * L; ++a) kdec[(size_t)t * L * L + a] = (t << 16) | ((a / L) << 8) | (a % L);
@@ -493,7 +529,7 @@ int sfft_plan_num_solved(const sfft_plan *p) { return p ? p->ns : -1; }
 int sfft_plan_set_corr_route(sfft_plan *p, int route) {
     if (!p || route < 0 || route > 2) return SFFT_ERR_INVALID_ARG;
     p->corr_route = route;
-    if (route == 2 && !corr_use_os(p)) { p->corr_route = 0; return SFFT_ERR_INVALID_ARG; }
+    if ((route == 2 && !corr_use_os(p)) || (route == 1 && !p->pow2)) { p->corr_route = 0; return SFFT_ERR_INVALID_ARG; }
     p->ws = nullptr; p->ws_bytes = 0; p->built = p->solved = false;      // the workspace partition depends on the split
     choose_split(p);
     return SFFT_OK;

@@ -144,7 +144,8 @@ k_rowfft_forward16(const double *__restrict__ R, const double *__restrict__ S, c
     double2 *tw2 = sm2, *buf = sm2 + C::TW2 + threadIdx.y * C::BUF;
     const int tid = threadIdx.x, img = blockIdx.x, x = blockIdx.y * RPC + threadIdx.y, bz = blockIdx.z;
     if (threadIdx.y == 0) fft_load_tw2<NH>(tw2, twW);
-    const double2 *src = reinterpret_cast<const double2 *>((img < nKa ? R : S) + ((size_t)bz * H + x) * W);
+    // (H need not be a multiple of RPC: a row slot past the end transforms the last row again and stores nothing)
+    const double2 *src = reinterpret_cast<const double2 *>((img < nKa ? R : S) + ((size_t)bz * H + min(x, H - 1)) * W);
     double2 v[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) v[r] = __ldg(&src[tid + r * T]);          // z[n] = a[2n] + i a[2n+1]
@@ -176,7 +177,7 @@ k_rowfft_forward16(const double *__restrict__ R, const double *__restrict__ S, c
     fft_core<NH>(v, buf, tw2, twW);
     double2 *dst = rhat + (((size_t)bz * (nKa + 1) + img) * H + x) * NH;
     // even/odd split (see k_rowfft_forward)
-    for (int k = tid; k <= NH / 2; k += T) {
+    for (int k = tid; k <= NH / 2 && x < H; k += T) {
         if (k == 0) {
             const double2 z0 = buf[0];
             dst[0] = make_double2(z0.x + z0.y, z0.x - z0.y);
@@ -199,9 +200,87 @@ cudaError_t launch_fwd16(sfft_plan *p, const double *dR, const double *dS) {
     auto kern = k_rowfft_forward16<NH>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    dim3 grid(dS ? p->nimg : p->nKa, p->H / RPC, p->nbatch);
+    dim3 grid(dS ? p->nimg : p->nKa, (p->H + RPC - 1) / RPC, p->nbatch);
     kern<<<grid, dim3(T, RPC), smem, p->stream>>>(dR, dS, p->dt.gK, p->dt.twW, p->rhat, p->H, p->nKa,
                                                   p->basis == SFFT_BASIS_POLY);
+    p->launches++;
+    return cudaGetLastError();
+}
+
+// W not a power of two (W even; true survey frames, e.g. 2046 x 4094): the complex N = W/2 point DFT of
+// z[n] = a[2n] + i a[2n+1] is run as a chirp-z (Bluestein) transform on the register FFT of fft_regs.cuh,
+//   Z[k] = c[k] sum_n (z[n] c[n]) conj(c[k-n]),  c[n] = exp(-i pi n^2 / N),
+// i.e. a circular convolution of length M = 2^k >= 2N - 1:  conv = IFFT_M( FFT_M(z c) * bhat ),  bhat = FFT_M(conj c
+// wrapped) a plan table, with the inverse transform taken as conj(FFT_M(conj .)) / M.  The even/odd split that follows
+// is the one of the power-of-two kernels with N in place of NH.  One CTA of M/16 threads per image row and image.
+// grid: x = image slot, y = row, z = batch entry.
+template <int M>
+__global__ void __launch_bounds__(FftCfg<M>::T)
+k_rowfft_forward_bs(const double *__restrict__ R, const double *__restrict__ S, const double *__restrict__ gK,
+                    const double2 *__restrict__ twW, const double2 *__restrict__ twM, const double2 *__restrict__ chirp,
+                    const double2 *__restrict__ bhat, double2 *__restrict__ rhat, int H, int W, int nKa) {
+    using C = FftCfg<M>;
+    constexpr int T = C::T;
+    extern __shared__ double2 sm3[];
+    double2 *tw2 = sm3, *buf = sm3 + C::TW2, *zs = buf + C::BUF;     // zs[N]: the N-point spectrum for the split
+    const int tid = threadIdx.x, img = blockIdx.x, x = blockIdx.y, bz = blockIdx.z, N = W / 2;
+    fft_load_tw2<M>(tw2, twM);
+    const double2 *src = reinterpret_cast<const double2 *>((img < nKa ? R : S) + ((size_t)bz * H + x) * W);
+    const double2 *g = reinterpret_cast<const double2 *>(gK + (size_t)(img < nKa ? img : 0) * W);
+    double2 v[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int n = tid + r * T;
+        v[r] = make_double2(0.0, 0.0);
+        if (n < N) {
+            double2 a = __ldg(&src[n]);
+            if (img < nKa) { const double2 gg = __ldg(&g[n]); a.x *= gg.x; a.y *= gg.y; }
+            v[r] = cmul(a, __ldg(&chirp[n]));
+        }
+    }
+    __syncthreads();                                                       // tw2 visible
+    fft_core<M>(v, buf, tw2, twM);
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int n = tid + r * T;
+        const double2 t = cmul(buf[n], __ldg(&bhat[n]));
+        v[r] = make_double2(t.x, -t.y);
+    }
+    __syncthreads();                                                       // buf consumed before it is rewritten
+    fft_core<M>(v, buf, tw2, twM);
+    constexpr double invM = 1.0 / M;
+    for (int k = tid; k < N; k += T) {
+        const double2 u = buf[k], c = __ldg(&chirp[k]);
+        zs[k] = cmul(make_double2(u.x * invM, -u.y * invM), c);
+    }
+    __syncthreads();
+    double2 *dst = rhat + (((size_t)bz * (nKa + 1) + img) * H + x) * N;
+    // even/odd split (see k_rowfft_forward), w = exp(-2 pi i / W)
+    for (int k = tid; k <= N / 2; k += T) {
+        if (k == 0) {
+            const double2 z0 = zs[0];
+            dst[0] = make_double2(z0.x + z0.y, z0.x - z0.y);
+        } else {
+            const double2 zk = zs[k], zn = zs[N - k];
+            const double2 E = make_double2(0.5 * (zk.x + zn.x), 0.5 * (zk.y - zn.y));
+            const double2 O = make_double2(0.5 * (zk.y + zn.y), -0.5 * (zk.x - zn.x));
+            const double2 wO = cmul(__ldg(&twW[k]), O);
+            dst[k] = make_double2(E.x + wO.x, E.y + wO.y);
+            if (k != N - k) dst[N - k] = make_double2(E.x - wO.x, -(E.y - wO.y));
+        }
+    }
+}
+
+template <int M>
+cudaError_t launch_fwd_bs(sfft_plan *p, const double *dR, const double *dS) {
+    using C = FftCfg<M>;
+    const size_t smem = (size_t)(C::TW2 + C::BUF + p->Nh) * sizeof(double2);
+    auto kern = k_rowfft_forward_bs<M>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid(dS ? p->nimg : p->nKa, p->H, p->nbatch);
+    kern<<<grid, C::T, smem, p->stream>>>(dR, dS, p->dt.gK, p->dt.twW, p->dt.twM, p->dt.chirp, p->dt.bhat, p->rhat, p->H, p->W,
+                                          p->nKa);
     p->launches++;
     return cudaGetLastError();
 }
@@ -209,6 +288,14 @@ cudaError_t launch_fwd16(sfft_plan *p, const double *dR, const double *dS) {
 }  // namespace
 
 cudaError_t launch_rowfft_forward(sfft_plan *p, const double *dR, const double *dS) {
+    switch (p->bsM) {
+        case 0: break;
+        case 512: return launch_fwd_bs<512>(p, dR, dS);
+        case 1024: return launch_fwd_bs<1024>(p, dR, dS);
+        case 2048: return launch_fwd_bs<2048>(p, dR, dS);
+        case 4096: return launch_fwd_bs<4096>(p, dR, dS);
+        default: return cudaErrorInvalidValue;
+    }
     switch (p->Nh) {
         case 32: return launch_fwd<32>(p, dR, dS);
         case 64: return launch_fwd<64>(p, dR, dS);

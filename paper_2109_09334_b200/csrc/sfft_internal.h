@@ -11,6 +11,12 @@
 namespace sfft {
 
 #ifdef __CUDACC__
+// v mod N (any sign); mask = N - 1 when N is a power of two, else < 0
+__device__ __forceinline__ int wrap_index(int v, int N, int mask) {
+    if (mask >= 0) return v & mask;
+    v %= N;
+    return v < 0 ? v + N : v;
+}
 // One FP64 tensor-core MMA (DMMA on sm_100a): C[8x8] += A[8x4] B[4x8].  Fragments: a = A[lane>>2][lane&3],
 // b = B[lane&3][lane>>2], c[q] = C[lane>>2][2*(lane&3) + q].
 __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
@@ -61,6 +67,9 @@ struct DeviceTables {
     double *gK = nullptr;       // [nKa][W]         kernel y-axis basis
     double *gB = nullptr;       // [nBa][W]         background y-axis basis
     double2 *twW = nullptr;     // [W]              exp(-2 pi i k / W)
+    double2 *twM = nullptr;     // [2 M]            exp(-2 pi i k / (2M)): twiddles of the M-point transforms of the chirp-z row DFT (W not a power of two)
+    double2 *chirp = nullptr;   // [W/2]            exp(-i pi n^2 / (W/2))
+    double2 *bhat = nullptr;    // [M]              M-point DFT of the wrapped conjugate chirp
     double2 *lagtw = nullptr;   // [Nh+1][L]        (w_m cos, w_m sin)(2 pi m k / W) / W
     double *cq = nullptr;       // [NC][nMom]       POLY: Q_c = sum_a cq[c][a] mu_a + border terms (binomial shift of g'_j by beta)
     double *cwr = nullptr;      // [NC][w]          POLY: coefficients of the |beta| row pixels whose shifted partner wraps
@@ -84,6 +93,8 @@ struct sfft_plan {
     bool corr_os = false; int os_hop = 0;   // the build takes the sectioned correlation (set by choose_split), its hop length
     int corr_route = 0;  // 0: chosen by the plan, 1: direct lag sums (corr.cu), 2: sectioned FFT64 correlation (corr_os.cu)
     int cpr = 0;         // constant photometric ratio: centre coefficients of the terms t >= 1 not free
+    bool pow2 = true;    // H and W are powers of two (mask wraps, radix-2 row transforms, every route available)
+    int bsM = 0;         // W not a power of two: length of the M-point transforms of the chirp-z (Bluestein) row DFT
     int Lx = 0, Ly = 0;  // kernel extent along x / y (rectangular kernels); L = max(Lx, Ly) is the enclosing square
     bool reduced = false;   // the solved system is a reduction of the full square layout (cpr and / or Lx != Ly)
     int rshare = -1;     // solved index of the shared centre unknown under cpr

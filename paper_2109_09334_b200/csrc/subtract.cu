@@ -58,7 +58,7 @@ __global__ void k_coef_rows(const double *__restrict__ kfold, const double *__re
     }
 }
 
-struct SubDims { int H, W, L, w, nKa, FB, n, KP, NKS, PS, ASTR, RS, NSRC; };
+struct SubDims { int H, W, L, w, nKa, FB, n, KP, NKS, PS, ASTR, RS, NSRC, hmask, wmask; };   // masks: N - 1 for powers of two, else -1
 
 // grid: x = column tile (64*NBW), y = 8-row block, z = batch.  block: 256 (warp = 8*NBW columns).
 template <int NBW>
@@ -91,13 +91,13 @@ __global__ void __launch_bounds__(256) k_subtract(const double *__restrict__ R, 
         __syncthreads();
         for (int i = tid; i < ns * nvc; i += 256) {
             const int dd = i / nvc, cs = i - dd * nvc;
-            const int xs = (x0 - d.w + s0 + dd) & (d.H - 1), y = (y0 - d.w + cs) & (d.W - 1);
+            const int xs = wrap_index(x0 - d.w + s0 + dd, d.H, d.hmask), y = wrap_index(y0 - d.w + cs, d.W, d.wmask);
             const double v = __ldg(&Rb[(size_t)xs * d.W + y]);
             for (int j = 0; j < d.nKa; ++j) Vs[((size_t)dd * d.nKa + j) * d.PS + cs] = v * __ldg(&gK[(size_t)j * d.W + y]);
         }
         for (int i = tid; i < ns * 8 * d.KP; i += 256) {
             const int kk = i % d.KP, rr = (i / d.KP) & 7, dd = i / (d.KP * 8);
-            const int xs = (x0 - d.w + s0 + dd) & (d.H - 1);
+            const int xs = wrap_index(x0 - d.w + s0 + dd, d.H, d.hmask);
             const int ai = rr + 2 * d.w - (s0 + dd);      // alpha + w,  alpha = (x0 + rr) - (x0 - w + s0 + dd)
             As[((size_t)dd * 8 + rr) * d.ASTR + kk] =
                 (ai >= 0 && ai < d.L) ? __ldg(&ct[((size_t)xs * d.L + ai) * d.KP + kk]) : 0.0;
@@ -115,12 +115,14 @@ __global__ void __launch_bounds__(256) k_subtract(const double *__restrict__ R, 
             }
         }
     }
-    // epilogue: D = S - model - background
+    // epilogue: D = S - model - background (the last tiles of a frame that is not a multiple of the tile overhang)
     const int x = x0 + r;
+    if (x >= d.H) return;
     const double *cb = coef + (size_t)bz * d.n + (d.n - d.FB);
 #pragma unroll
     for (int nb = 0; nb < NBW; ++nb) {
         const int y = y0 + wcol + 8 * nb + 2 * kq;
+        if (y >= d.W) continue;                          // W is even: y + 1 < W as well
         double bg0 = 0.0, bg1 = 0.0;
         for (int s = 0; s < d.FB; ++s) {
             const double cf = cb[s] * __ldg(&xwt[(size_t)(d.nKa + bti[s]) * d.H + x]);
@@ -145,7 +147,7 @@ cudaError_t launch_sub(sfft_plan *p, const double *d_coef, const double *dR, con
     auto kern = k_subtract<NBW>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    dim3 grid(p->W / TY, p->H / 8, p->nbatch);
+    dim3 grid((p->W + TY - 1) / TY, (p->H + 7) / 8, p->nbatch);
     kern<<<grid, 256, smem, p->stream>>>(dR, dS, dD, p->ctab, d_coef, p->dt.gK, p->dt.xwt, p->dt.gB, p->dt.bti, p->dt.btj, d);
     p->launches++;
     return cudaGetLastError();
@@ -169,6 +171,8 @@ cudaError_t launch_subtract(sfft_plan *p, const double *d_coef, const double *dR
     d.KP = subtract_kpad(p->nKa, p->L); d.NKS = d.KP / 4;
     d.ASTR = ((d.KP + 15) / 16) * 16 + 4;
     d.NSRC = p->L + 7;
+    d.hmask = (p->H & (p->H - 1)) == 0 ? p->H - 1 : -1;
+    d.wmask = (p->W & (p->W - 1)) == 0 ? p->W - 1 : -1;
     cudaError_t e = launch_fold_coef(p, d_coef);
     if (e != cudaSuccess) return e;
     k_coef_rows<<<dim3(p->H, p->nbatch), 256, 0, p->stream>>>(p->kfold, p->dt.xwt, p->dt.kti, p->dt.ktj, p->ctab, p->H,

@@ -325,6 +325,7 @@ cudaError_t launch_fir(sfft_plan *p, const FirDims &d, int ny) {
 // pixel, plus the transforms, on the plain FMA pipe at ~half the efficiency of the tensor-core contraction)
 // is below the direct form's (L+7) * KP tensor-core MACs per pixel.
 bool subtract_use_fourier(const sfft_plan *p) {
+    if (!p->pow2) return false;            // frames that are not powers of two take the direct contraction
     if (p->Nh < 512 || p->L < 9 || p->L > 25 || p->FK > kFirMaxFK || p->nKa > kFirMaxNKa || p->nBa > 16) return false;
     if (fir_smem(p) > 200 * 1024) return false;
     const double direct = (double)(p->L + 7) * subtract_kpad(p->nKa, p->L);

@@ -166,6 +166,25 @@ def test_parity_full_size(cuda_device, cfg):
 
 
 @pytest.mark.slow
+def test_parity_decam_ccd_frame_2046x4094(cuda_device):
+    """NEXT-4 at the true DECam CCD size (2046 x 4094 = 2*3*11*31 x 2*23*89), config-3 recipe and model
+    (15 x 15 delta basis, DK = DB = 2, n = 1356): full M / rhs / c element-wise, D at 4 006 sampled pixels."""
+    import torch
+    p = synth.make_pair(3, H=2046, W=4094)
+    bid = oracle.POLY
+    Mo, ro = oracle.normal_from_lags(p.R, p.S, p.L, bid, p.DK, p.DB)
+    co = oracle.solve(Mo, ro)
+    M, rhs, c, D = _gpu_all(torch, p, p.L, p.basis, p.DK, p.DB)
+    _check_system(M[0], rhs[0], Mo, ro, p.S)
+    _check_coef(c[0], co, 6 * p.L * p.L)
+    rng = np.random.default_rng(2046)
+    px = np.r_[rng.integers(0, p.H, 4000), [0, 0, p.H - 1, p.H - 1, 3, p.H - 2]]
+    py = np.r_[rng.integers(0, p.W, 4000), [0, p.W - 1, 0, p.W - 1, p.W - 4, 5]]
+    Dref = oracle.difference_at(p.R, p.S, co, p.L, bid, p.DK, p.DB, px, py)
+    assert np.max(np.abs(D[px, py] - Dref)) <= TOL_D * p.sigma
+
+
+@pytest.mark.slow
 def test_parity_config5_batch64_in_one_call(cuda_device):
     """BASELINE.json configs[4] as stated: 64 independent 1024x1024 sub-field pairs (each seeded as in config 2),
     cubic B-splines with 4 interior knots per axis, 11x11 delta basis, n = 7808, processed in ONE call
@@ -324,6 +343,26 @@ def test_parity_constant_photometric_ratio(cuda_device, cfg, H, W, L, basis, DK,
     plan.close()
 
 
+@pytest.mark.parametrize("cfg,H,W,L,DK,DB", [
+    (1, 96, 130, 7, 1, 1),        # neither axis a power of two; chirp-z rows with M = 512
+    (2, 100, 1022, 5, 2, 1),      # W/2 = 511 = 7 x 73, M = 1024
+    (2, 50, 4094, 3, 1, 1),       # the DECam row length 4094 = 2 x 23 x 89, M = 4096
+    (3, 186, 372, 15, 2, 2),      # 2046 x 4094 scaled by 1/11: wide kernel, several hops and a ragged last one
+    (2, 90, 1024, 5, 1, 1),       # only H is not a power of two (rows per CTA do not divide H)
+    (2, 128, 1000, 9, 2, 0),      # only W is not a power of two
+])
+def test_parity_frames_not_powers_of_two(cuda_device, cfg, H, W, L, DK, DB):
+    """NEXT-4 (true CCD frames such as 2046 x 4094): any H, even W - chirp-z row transforms, general
+    wrap-around in the sectioned lag correlation, ragged tiles in the direct subtract."""
+    import torch
+    p = synth.make_pair(cfg, H=H, W=W)
+    Mo, ro, co, Do = _oracle_all(p.R, p.S, L, "poly", DK, DB)
+    M, rhs, c, D = _gpu_all(torch, p, L, "poly", DK, DB)
+    _check_system(M[0], rhs[0], Mo, ro, p.S)
+    _check_coef(c[0], co, Mo.shape[0] - oracle.num_terms(oracle.POLY, DB))
+    assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
+
+
 @pytest.mark.parametrize("cfg,H,W,L0,L1,basis,DK,DB,cpr", [
     (2, 128, 256, 5, 9, "poly", 2, 1, False),       # wider along y; direct-route subtract
     (2, 64, 1024, 13, 7, "poly", 1, 1, False),      # wider along x; Fourier-route subtract (W >= 1024, L = 13)
@@ -472,7 +511,8 @@ def _saturate(p, sat, nsat=12, seed=5):
     return np.minimum(R, sat * 4), np.minimum(S, sat * 4)
 
 
-@pytest.mark.parametrize("cfg,H,W,L,rd,rb,nb", [(1, None, None, None, 2, 6, 1), (2, 64, 1024, 9, 1, 4, 1), (5, 128, 128, 5, 3, 8, 3)])
+@pytest.mark.parametrize("cfg,H,W,L,rd,rb,nb", [(1, None, None, None, 2, 6, 1), (2, 64, 1024, 9, 1, 4, 1), (5, 128, 128, 5, 3, 8, 3),
+                                                 (1, 96, 130, 7, 2, 6, 1)])
 def test_mask_fill_and_masked_fit_flow(cuda_device, cfg, H, W, L, rd, rb, nb):
     """NEXT-2 (DESIGN g21): the CUDA mask/fill against the oracle (mask bit-exact, filled pixels to
     rounding), then the paper's two-step flow end to end: fit on the masked pair, apply to the original pair."""
@@ -658,7 +698,7 @@ def test_numerically_rank_deficient_input_reports_not_spd(cuda_device):
 
 def test_argument_and_state_errors(cuda_device):
     import torch
-    for bad in [(100, 128, 7, 1, 1, 0), (128, 128, 6, 1, 1, 0), (128, 128, 7, -1, 1, 0), (128, 128, 7, 1, 1, 2),
+    for bad in [(100, 129, 7, 1, 1, 0), (100, 4100, 7, 1, 1, 0), (100, 130, 7, 1, 1, 1), (100, 130, 7, 3, 1, 0), (128, 128, 6, 1, 1, 0), (128, 128, 7, -1, 1, 0), (128, 128, 7, 1, 1, 2),
                 (64, 64, 33, 1, 1, 0), (16, 128, 3, 1, 1, 0)]:
         st, _ = B.sfft_plan_create(*bad)
         assert st == B.SFFT_ERR_INVALID_ARG, bad
