@@ -66,9 +66,10 @@ __device__ __forceinline__ void fft64_group(double2 (&v)[8], Slot ex, const doub
 //          ulp or two otherwise; DESIGN g8).  Computed here
 //          instead of read from the plan's table: u is exact and u*u is its correctly rounded square, which is
 //          what the table holds, so both routes weight with the very same numbers (a1).
-template <int MODE, int SIDE, int XP>
+//   P2   : H is a power of two (wrap by mask); otherwise by conditional subtraction (x0 < H + 64 for every live hop)
+template <int MODE, int SIDE, int XP, bool P2>
 __device__ __forceinline__ void os_transform(const double2 *rw, double2 *dst, const double2 *tw, int t, int nkeep, int x0,
-                                             int H, int hmask, double uscale, double uoff) {
+                                             int H, double uscale, double uoff) {
     double2 v[8];
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
@@ -76,7 +77,10 @@ __device__ __forceinline__ void os_transform(const double2 *rw, double2 *dst, co
         if (MODE == 1) a.y = 0.0;
         if (MODE == 2) { a.x = a.y; a.y = 0.0; }
         if (XP > 0) {
-            const double u = fma((double)wrap_index(x0 + t + 8 * r, H, hmask), uscale, uoff), w = XP == 1 ? u : u * u;
+            int xx = x0 + t + 8 * r;
+            if (P2) xx &= H - 1;
+            else { xx -= xx >= H ? H : 0; xx -= xx >= H ? H : 0; }
+            const double u = fma((double)xx, uscale, uoff), w = XP == 1 ? u : u * u;
             a.x *= w;
             if (MODE == 0) a.y *= w;
         }
@@ -88,16 +92,16 @@ __device__ __forceinline__ void os_transform(const double2 *rw, double2 *dst, co
     for (int k2 = 0; k2 < 8; ++k2) dst[(t + 8 * k2) * kOsBinStride] = v[k2];
 }
 
-template <int MODE, int SIDE>
+template <int MODE, int SIDE, bool P2>
 __device__ __forceinline__ void os_transform_xp(int xp, const double2 *rw, double2 *dst, const double2 *tw, int t, int nkeep,
-                                                int x0, int H, int hmask, double uscale, double uoff) {
-    if (xp <= 0) os_transform<MODE, SIDE, 0>(rw, dst, tw, t, nkeep, x0, H, hmask, uscale, uoff);
-    else if (xp == 1) os_transform<MODE, SIDE, 1>(rw, dst, tw, t, nkeep, x0, H, hmask, uscale, uoff);
-    else os_transform<MODE, SIDE, 2>(rw, dst, tw, t, nkeep, x0, H, hmask, uscale, uoff);
+                                                int x0, int H, double uscale, double uoff) {
+    if (xp <= 0) os_transform<MODE, SIDE, 0, P2>(rw, dst, tw, t, nkeep, x0, H, uscale, uoff);
+    else if (xp == 1) os_transform<MODE, SIDE, 1, P2>(rw, dst, tw, t, nkeep, x0, H, uscale, uoff);
+    else os_transform<MODE, SIDE, 2, P2>(rw, dst, tw, t, nkeep, x0, H, uscale, uoff);
 }
 
 // grid: x = column slot c (0: DC of packed column 0, Nh: its Nyquist part, else column c), y = x-range part, z = batch
-template <int MODE>
+template <int MODE, bool P2>
 __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, const Seq *__restrict__ seqs,
                                              double2 *__restrict__ G, const OsDims &d, double2 *smo) {
     double2 *SQ = smo;                                   // [2][64][33]  spectra of the 64-row windows
@@ -109,7 +113,6 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
     const int c = blockIdx.x, xs = blockIdx.y, bz = blockIdx.z;
     const int col = (MODE == 2) ? 0 : c;
     const int H = d.H, HOP = d.HOP, RS = d.RS, STEP = kOsHops * d.HOP;
-    const int hmask = (H & (H - 1)) == 0 ? H - 1 : -1;     // wrap by mask when H is a power of two
 
     if (tid < 64) {
         double s, co;
@@ -132,7 +135,7 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
         const int x0 = xb + s * STEP;
         double2 *rbuf = raw + (s & 1) * kOsMaxImg * RS;
         for (int img = img0, r = rr0; img < d.nimg;) {
-            const int x = wrap_index(x0 + r, H, hmask);
+            const int x = P2 ? ((x0 + r) & (H - 1)) : (x0 + r) % H;
             const unsigned dst = (unsigned)__cvta_generic_to_shared(&rbuf[img * RS + r]);
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(&rb[((size_t)img * H + x) * d.Nh]));
             r += npf;
@@ -164,8 +167,8 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
             const double2 *rw = raw + (b * kOsMaxImg + sq.img) * RS + r0;
             double2 *dst = (side ? SP : SQ) + b * kOsSpec + seq * 4 + hop;
             // the conj side keeps only the HOP rows of this hop that lie inside the CTA's x-range
-            if (side) os_transform_xp<MODE, 1>(sq.xw, rw, dst, tw, t, min(HOP, xe - x0), x0, H, hmask, uscale, uoff);
-            else os_transform_xp<MODE, 0>(sq.xw, rw, dst, tw, t, 64, x0, H, hmask, uscale, uoff);
+            if (side) os_transform_xp<MODE, 1, P2>(sq.xw, rw, dst, tw, t, min(HOP, xe - x0), x0, H, uscale, uoff);
+            else os_transform_xp<MODE, 0, P2>(sq.xw, rw, dst, tw, t, 64, x0, H, uscale, uoff);
         }
         asm volatile("cp.async.wait_group 0;" ::: "memory");      // the rows of step s+1 (fetched during step s-1) landed
         __syncthreads();                                           // spectra of step s complete; raw[b] and S[b^1] free
@@ -213,13 +216,14 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
     }
 }
 
+template <bool P2>
 __global__ void __launch_bounds__(512, 1)
 k_corr_os(const double2 *__restrict__ rhat, const Seq *__restrict__ seqs, double2 *__restrict__ G, OsDims d) {
     extern __shared__ double2 smo[];
     const int c = blockIdx.x;                            // uniform per CTA
-    if (c == 0) corr_os_body<1>(rhat, seqs, G, d, smo);
-    else if (c == d.Nh) corr_os_body<2>(rhat, seqs, G, d, smo);
-    else corr_os_body<0>(rhat, seqs, G, d, smo);
+    if (c == 0) corr_os_body<1, P2>(rhat, seqs, G, d, smo);
+    else if (c == d.Nh) corr_os_body<2, P2>(rhat, seqs, G, d, smo);
+    else corr_os_body<0, P2>(rhat, seqs, G, d, smo);
 }
 
 size_t corr_os_smem(const OsDims &d) {
@@ -257,10 +261,13 @@ cudaError_t launch_corr_os(sfft_plan *p) {
     OsDims d{p->H, p->Nh, p->nimg, p->nseq, p->L, p->E, p->Sx, corr_os_hop(p), 0};
     d.RS = (kOsHops - 1) * d.HOP + 64;
     const size_t smem = corr_os_smem(d);
-    cudaError_t e = cudaFuncSetAttribute(k_corr_os, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const bool p2 = (p->H & (p->H - 1)) == 0;
+    cudaError_t e = cudaFuncSetAttribute(p2 ? k_corr_os<true> : k_corr_os<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid(p->Nh + 1, p->Sx, p->nbatch);
-    k_corr_os<<<grid, 512, smem, p->stream>>>(p->rhat, p->dt.seqs, p->G, d);
+    if (p2) k_corr_os<true><<<grid, 512, smem, p->stream>>>(p->rhat, p->dt.seqs, p->G, d);
+    else k_corr_os<false><<<grid, 512, smem, p->stream>>>(p->rhat, p->dt.seqs, p->G, d);
     p->launches++;
     return cudaGetLastError();
 }
