@@ -25,6 +25,8 @@
 // A diagonal entry that is not positive and finite, or a pivot of the scaled matrix (unit diagonal) that is not
 // finite or lies below kPivotFloor * n (rounding-noise level of the assembled entries: the system is numerically
 // rank-deficient even where the noise happens to be positive), writes its index to flag[2*b] (SFFT_ERR_NOT_SPD).
+#include <cuda.h>          // CUtensorMap (types only: the encoder is fetched through cudaGetDriverEntryPoint)
+
 #include <algorithm>
 
 #include "sfft_internal.h"
@@ -585,13 +587,8 @@ __global__ void __launch_bounds__(256, 2) k_chol_slab(double *__restrict__ Lf, c
 // waits for CTAs with a smaller linear index (in-order dispatch): no co-residency requirement beyond one CTA.
 constexpr int kBsStages = 4;
 constexpr unsigned long long kBsSentinel = 0xFFF8DEADBEEF5AFEull;
-constexpr size_t kBsSmem = (size_t)(1 + kBsStages) * NB * NB * sizeof(double);
+constexpr size_t kBsSmem = (size_t)(1 + kBsStages) * NB * NB * sizeof(double) + 128;
 
-__device__ __forceinline__ double ld_volatile_f64(const double *p) {
-    double v;
-    asm volatile("ld.volatile.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
-    return v;
-}
 __device__ __forceinline__ void ld_volatile_f64x2(const double *p, double &a, double &b) {
     asm volatile("ld.volatile.global.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "l"(p) : "memory");
 }
@@ -599,41 +596,75 @@ __device__ __forceinline__ void st_volatile_f64(double *p, double v) {
     asm volatile("st.volatile.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
 
+// mbarrier + bulk-copy (TMA engine) primitives: one thread arms the barrier with the byte count, the copies complete
+// on it, every consumer waits on the phase parity.
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// one 64 x 64 tile of the factor (tensor map over Lf as [(n+1) nbat rows][ldl columns]) as a single TMA box copy
+__device__ __forceinline__ void tma_tile_g2s(void *dst, const CUtensorMap *tm, int col, int row, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::
+                     "r"(smem_u32(dst)), "l"(tm), "r"(col), "r"(row), "r"(smem_u32(bar))
+                 : "memory");
+}
+
 __global__ void __launch_bounds__(256)
-k_chol_backsolve_lb(const double *__restrict__ Lf, const double *__restrict__ Winv, const double *__restrict__ dscale,
-                    double *__restrict__ coef, double *ybuf, int n, int ldl, int nblk, int nbat) {
+k_chol_backsolve_lb(const __grid_constant__ CUtensorMap tmL, const double *__restrict__ Lf, const double *__restrict__ Winv,
+                    const double *__restrict__ dscale, double *__restrict__ coef, double *ybuf, int n, int ldl, int nblk,
+                    int nbat) {
     extern __shared__ double sm[];
-    double *Ws = sm, *T = sm + NB * NB;                 // W_b [k][i]; tile ring [stage][k][col]
+    double *Ws = reinterpret_cast<double *>(((uintptr_t)sm + 127) & ~(uintptr_t)127);     // TMA destinations: 128-byte aligned
+    double *T = Ws + NB * NB;                           // W_b [k][i]; tile ring [stage][k][col]
     __shared__ double zs[NB], red[4][NB], ysh[2][NB];
     const int id = blockIdx.x, bz = id % nbat, x = id / nbat, blk = nblk - 1 - x;
     const int tid = threadIdx.x, col = tid & 63, q = tid >> 6;
     const double *L = Lf + (size_t)bz * (n + 1) * ldl;
     double *yb = ybuf + (size_t)bz * nblk * NB;
     const int i0 = blk * NB, nbk = min(NB, n - i0);
-    {
-        const double *W = Winv + ((size_t)bz * nblk + blk) * NB * NB;
-        for (int i = tid; i < NB * NB / 2; i += 256) cp_async16(&Ws[2 * i], &W[2 * i]);
-        asm volatile("cp.async.commit_group;");
+    // Staging by the TMA engine: W_b as one 32 KB bulk copy, a tile as one 64 x 64 box of the tensor map over the factor,
+    // issued by one thread and completing on the stage's mbarrier (no per-thread copies or address arithmetic).
+    __shared__ unsigned long long bars[kBsStages + 1];   // [stage], then W
+    if (tid == 0) {
+        for (int i = 0; i <= kBsStages; ++i) mbar_init(&bars[i], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 32) {
+        mbar_expect_tx(&bars[kBsStages], NB * NB * sizeof(double));
+        bulk_g2s(Ws, Winv + ((size_t)bz * nblk + blk) * NB * NB, NB * NB * sizeof(double), &bars[kBsStages]);
     }
     auto fetch = [&](int t) {                              // tile of block j = nblk-1-t into stage t % kBsStages
-        if (t < x) {
-            const int j0 = (nblk - 1 - t) * NB;
-            double *dst = T + (size_t)(t % kBsStages) * NB * NB;
-#pragma unroll
-            for (int r = 0; r < NB * NB / 2 / 256; ++r) {
-                const int i = tid + 256 * r, k = i >> 5, c = (i & 31) * 2;
-                if (j0 + k < n) cp_async16(&dst[k * NB + c], &L[(size_t)(j0 + k) * ldl + i0 + c]);
-                else { dst[k * NB + c] = 0.0; dst[k * NB + c + 1] = 0.0; }
-            }
-        }
-        asm volatile("cp.async.commit_group;");
+        if (t >= x || tid != 32) return;
+        const int j0 = (nblk - 1 - t) * NB, st = t % kBsStages;
+        mbar_expect_tx(&bars[st], NB * NB * sizeof(double));
+        tma_tile_g2s(T + (size_t)st * NB * NB, &tmL, i0, bz * (n + 1) + j0, &bars[st]);
     };
 #pragma unroll
     for (int t = 0; t < kBsStages - 1; ++t) fetch(t);
     if (tid < NB) zs[tid] = (tid < nbk) ? L[(size_t)n * ldl + i0 + tid] : 0.0;
     double a0 = 0.0, a1 = 0.0;
     for (int t = 0; t < x; ++t) {
-        asm volatile("cp.async.wait_group %0;" ::"n"(kBsStages - 2) : "memory");     // tile t (and W) landed
         if (tid < 32) {
             // one warp polls the 64 values of block j (a hot line for every CTA below j: keep the request count low)
             const double *yj = yb + (size_t)(nblk - 1 - t) * NB + 2 * tid;
@@ -645,7 +676,13 @@ k_chol_backsolve_lb(const double *__restrict__ Lf, const double *__restrict__ Wi
             ysh[t & 1][2 * tid] = v0;
             ysh[t & 1][2 * tid + 1] = v1;
         }
-        __syncthreads();        // tile t and y_j visible to every thread; stage (t-1) % S and ysh[(t-1) & 1] are free again
+        mbar_wait(&bars[t % kBsStages], (unsigned)(t / kBsStages) & 1u);      // tile t landed
+        if (t == 0 && n - (nblk - 1) * NB < NB) {
+            // last block: the box runs past the last unknown (rhs row, next system); those rows meet y = 0, keep them finite
+            const int nv = n - (nblk - 1) * NB;
+            for (int i = tid; i < (NB - nv) * NB; i += 256) T[nv * NB + i] = 0.0;
+        }
+        __syncthreads();        // y_j (and zero rows) visible to every thread; stage (t-1) % S and ysh[(t-1) & 1] are free again
         fetch(t + kBsStages - 1);
         const double *yv = &ysh[t & 1][16 * q];
         const double *tp = T + (size_t)(t % kBsStages) * NB * NB + (16 * q) * NB + col;
@@ -655,7 +692,7 @@ k_chol_backsolve_lb(const double *__restrict__ Lf, const double *__restrict__ Wi
             a1 = fma(tp[(k + 1) * NB], yv[k + 1], a1);
         }
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    mbar_wait(&bars[kBsStages], 0u);                       // W landed
     red[q][col] = a0 + a1;
     __syncthreads();
     if (tid < NB) zs[tid] -= (red[0][tid] + red[1][tid]) + (red[2][tid] + red[3][tid]);
@@ -725,8 +762,27 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     }
     e = cudaFuncSetAttribute(k_chol_backsolve_lb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBsSmem);
     if (e != cudaSuccess) return e;
-    k_chol_backsolve_lb<<<dim3(nblk * nbat), 256, kBsSmem, p->stream>>>(p->Lf, p->Winv, p->dscale, d_out, p->ybuf, n, ldl, nblk,
-                                                                       nbat);
+    // tensor map of the factor buffer: FP64 [(n+1) nbat rows][ldl columns], 64 x 64 boxes, zeros out of bounds
+    typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                 const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeFn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
+        if (e != cudaSuccess) return e;
+        if (!fn || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+        encode = (EncodeFn)fn;
+    }
+    alignas(64) CUtensorMap tmL;
+    const cuuint64_t gdim[2] = {(cuuint64_t)ldl, (cuuint64_t)(n + 1) * nbat}, gstr[1] = {(cuuint64_t)ldl * sizeof(double)};
+    const cuuint32_t box[2] = {NB, NB}, estr[2] = {1, 1};
+    if (encode(&tmL, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->Lf, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorInvalidValue;
+    k_chol_backsolve_lb<<<dim3(nblk * nbat), 256, kBsSmem, p->stream>>>(tmL, p->Lf, p->Winv, p->dscale, d_out, p->ybuf, n, ldl,
+                                                                       nblk, nbat);
     p->launches++;
     e = cudaGetLastError();
     if (e == cudaSuccess && p->reduced) e = launch_expand_coef(p, p->coefr, d_coef);
