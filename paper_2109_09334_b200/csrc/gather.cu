@@ -9,6 +9,8 @@
 // with Om_{tb,t}(rho) = Om_{t,tb}(-rho) for tb > t.  Real-space scaling: M = Phi^T Phi.
 // One warp fills a 32-entry run of a matrix row, so stores are 256-byte coalesced; both
 // triangles are written from the (min,max)-ordered index pair, which makes M exactly symmetric.
+#include <algorithm>
+
 #include "sfft_internal.h"
 
 namespace sfft {
@@ -87,40 +89,50 @@ __global__ void k_gather(const double *__restrict__ tab, const double *__restric
     }
 }
 
-// Kernel-kernel part of M for the unconstrained system, block by block: CTA (t, tb, chunk) fills kGatherRows rows of
-// the L^2 x L^2 block M[(tb, .)][(t, .)] from the Omega table of the pair (min, max)(tb, t) staged in shared memory
-// (one table read per CTA instead of four L2 reads per entry; rows leave in 256-byte runs).  Entries are formed from
-// the (lower, higher)-ordered unknown pair exactly as in m_entry, so M stays exactly symmetric.
+// Kernel-kernel part of M for the unconstrained system: CTA (t-group, tb, chunk) fills kGatherRows rows of the blocks
+// M[(tb, .)][(t, .)], t in the group, from the Omega tables of the pairs (min, max)(tb, t) staged in shared memory (one
+// table read per CTA instead of four L2 reads per entry).  A warp writes its row across ALL blocks of the group, i.e.
+// one contiguous run of TG L^2 entries: the block boundaries (L^2 entries = a fraction of a 32-byte sector) are then
+// written by the same warp back to back instead of by different CTAs at different times, which is what made the
+// 31 GB write of config 5 run at 16 % of the HBM roofline.  Entries are formed from the (lower, higher)-ordered
+// unknown pair exactly as in m_entry, so M stays exactly symmetric.
 constexpr int kGatherRows = 32;
 __global__ void __launch_bounds__(256) k_gather_kk(const double *__restrict__ tab, double *__restrict__ M, GatherDims d,
-                                                   int nchunk) {
-    extern __shared__ double som[];                       // [nO][nO] Omega of the ordered pair, then int dec[LL]
-    int *dec = reinterpret_cast<int *>(som + d.nO * d.nO);
-    const int t = blockIdx.x, tb = blockIdx.y, b = blockIdx.z / nchunk, chunk = blockIdx.z - b * nchunk;
-    const int tlo = min(tb, t), thi = max(tb, t), pair = tlo * d.FK - tlo * (tlo - 1) / 2 + (thi - tlo);
-    const double *om = tab + (size_t)b * d.tab_size + d.off_om + (size_t)pair * d.nO * d.nO;
-    for (int i = threadIdx.x; i < d.nO * d.nO; i += 256) som[i] = __ldg(&om[i]);
+                                                   int nchunk, int TG) {
+    extern __shared__ double som[];                       // [TG][nO][nO] Omega of the ordered pairs, then int dec[LL]
+    const int nO2 = d.nO * d.nO;
+    int *dec = reinterpret_cast<int *>(som + (size_t)TG * nO2);
+    const int t0 = blockIdx.x * TG, tg = min(TG, d.FK - t0), tb = blockIdx.y, b = blockIdx.z / nchunk,
+              chunk = blockIdx.z - b * nchunk;
+    for (int i = threadIdx.x; i < tg * nO2; i += 256) {
+        const int tl = i / nO2, t = t0 + tl, tlo = min(tb, t), thi = max(tb, t);
+        const int pair = tlo * d.FK - tlo * (tlo - 1) / 2 + (thi - tlo);
+        som[i] = __ldg(&tab[(size_t)b * d.tab_size + d.off_om + (size_t)pair * nO2 + (i - tl * nO2)]);
+    }
     for (int a = threadIdx.x; a < d.LL; a += 256) dec[a] = ((a / d.L - d.w) << 16) | ((a % d.L - d.w) & 0xffff);
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, c0 = (d.L - 1) * d.nO + (d.L - 1);   // index of lag (0,0)
-    const double o0 = som[c0];
     const int r1 = min(d.LL, (chunk + 1) * kGatherRows);
     for (int ab = chunk * kGatherRows + warp; ab < r1; ab += 8) {
-        const int kb = tb * d.LL + ab;
-        double *row = M + ((size_t)b * d.ns + kb) * d.ns + (size_t)t * d.LL;
-        for (int a = lane; a < d.LL; a += 32) {
-            const int k = t * d.LL + a;
-            // (first, second) = the unknowns in increasing index order
-            const int fa = kb <= k ? ab : a, sa = kb <= k ? a : ab;
-            const int df = dec[fa], ds = dec[sa];
-            const int alb = df >> 16, beb = (short)(df & 0xffff), al = ds >> 16, be = (short)(ds & 0xffff);
-            const bool cb = (alb == 0 && beb == 0), c = (al == 0 && be == 0);
-            double v;
-            if (cb && c) v = o0;
-            else if (c) v = som[c0 + alb * d.nO + beb] - o0;
-            else if (cb) v = som[c0 - al * d.nO - be] - o0;
-            else v = (som[c0 + (alb - al) * d.nO + (beb - be)] - som[c0 + alb * d.nO + beb]) - (som[c0 - al * d.nO - be] - o0);
-            row[a] = v;
+        const int kb = tb * d.LL + ab, dab = dec[ab];
+        double *row = M + ((size_t)b * d.ns + kb) * d.ns + (size_t)t0 * d.LL;
+        for (int tl = 0; tl < tg; ++tl) {
+            const double *so = som + (size_t)tl * nO2;
+            const double o0 = so[c0];
+            const int t = t0 + tl;
+            for (int a = lane; a < d.LL; a += 32) {
+                const int k = t * d.LL + a;
+                // (first, second) = the unknowns in increasing index order
+                const int df = kb <= k ? dab : dec[a], ds = kb <= k ? dec[a] : dab;
+                const int alb = df >> 16, beb = (short)(df & 0xffff), al = ds >> 16, be = (short)(ds & 0xffff);
+                const bool cb = (alb == 0 && beb == 0), c = (al == 0 && be == 0);
+                double v;
+                if (cb && c) v = o0;
+                else if (c) v = so[c0 + alb * d.nO + beb] - o0;
+                else if (cb) v = so[c0 - al * d.nO - be] - o0;
+                else v = (so[c0 + (alb - al) * d.nO + (beb - be)] - so[c0 + alb * d.nO + beb]) - (so[c0 - al * d.nO - be] - o0);
+                row[tl * d.LL + a] = v;
+            }
         }
     }
 }
@@ -161,8 +173,14 @@ cudaError_t launch_gather(sfft_plan *p) {
     GatherDims d = gather_dims(p);
     if (!p->reduced) {
         const int nchunk = (d.LL + kGatherRows - 1) / kGatherRows;
-        const size_t smem = (size_t)d.nO * d.nO * sizeof(double) + (size_t)d.LL * sizeof(int);
-        k_gather_kk<<<dim3(p->FK, p->FK, p->nbatch * nchunk), 256, smem, p->stream>>>(p->tab, p->M, d, nchunk);
+        // blocks per CTA: as many Omega tables as fit ~96 KB, at most 16, and enough CTAs left to fill the machine
+        int TG = std::max(1, std::min(16, (int)((96 * 1024) / ((size_t)d.nO * d.nO * sizeof(double)))));
+        TG = std::min(TG, p->FK);
+        while (TG > 1 && (long)((p->FK + TG - 1) / TG) * p->FK * p->nbatch * nchunk < 2 * 148) TG = (TG + 1) / 2;
+        const size_t smem = (size_t)TG * d.nO * d.nO * sizeof(double) + (size_t)d.LL * sizeof(int);
+        cudaError_t e = cudaFuncSetAttribute(k_gather_kk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_gather_kk<<<dim3((p->FK + TG - 1) / TG, p->FK, p->nbatch * nchunk), 256, smem, p->stream>>>(p->tab, p->M, d, nchunk, TG);
         k_gather_bg<<<dim3((p->n + 127) / 128, p->FB, p->nbatch), 128, 0, p->stream>>>(p->tab, p->dt.phi0, p->dt.kdec, p->M,
                                                                                      p->rhs, d);
         p->launches += 2;
