@@ -65,16 +65,17 @@ __global__ void k_lagsum_final(const double *__restrict__ part, const LagUnit *_
     const int eps = j - u.hw, k = eps < 0 ? -eps : eps;
     const double *src = part + ((size_t)bz * nch * L + k) * 2 * E + u.e;
     double P = 0.0, Q = 0.0;
-    for (int c8 = 0; c8 < nch; c8 += 8) {
-        double p8[8], q8[8];
+    // 32 partials (64 loads) in flight per thread: the kernel is a handful of L2 round trips long
+    for (int c8 = 0; c8 < nch; c8 += 32) {
+        double p8[32], q8[32];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
+        for (int q = 0; q < 32; ++q) {
             const bool ok = c8 + q < nch;
             p8[q] = ok ? src[(size_t)(c8 + q) * L * 2 * E] : 0.0;
             q8[q] = ok ? src[(size_t)(c8 + q) * L * 2 * E + E] : 0.0;
         }
 #pragma unroll
-        for (int q = 0; q < 8; ++q) { P += p8[q]; Q += q8[q]; }      // fixed order: deterministic
+        for (int q = 0; q < 32; ++q) { P += p8[q]; Q += q8[q]; }      // fixed order: deterministic
     }
     const int s = (eps == 0) ? 0 : ((eps > 0) == (u.sgn > 0) ? 1 : -1);
     tab[(size_t)bz * tab_size + u.dst_off + j] = P - s * Q;
