@@ -99,7 +99,9 @@ __device__ __forceinline__ void fft_load_tw2(double2 *tw2, const double2 *__rest
 // Forward FFT of NH points: on entry v[r] = z[tid + r*T]; on exit the spectrum Z[0..NH) is in buf (natural
 // order, unpadded) and visible to all threads.  buf must not be in use by other threads on entry (the
 // caller separates calls by a barrier).
-template <int NH>
+// STORE = false: the last pass leaves its results in registers instead, v[q*R3 + r] = Z[k + 256 r] with
+// k = tid + T q (q < NB3, r < R3), and buf is free again on exit.
+template <int NH, bool STORE = true>
 __device__ __forceinline__ void fft_core(double2 (&v)[16], double2 *buf, const double2 *tw2,
                                          const double2 *__restrict__ twW) {
     using C = FftCfg<NH>;
@@ -171,9 +173,12 @@ __device__ __forceinline__ void fft_core(double2 (&v)[16], double2 *buf, const d
         }
         fft_reg<R3>(u);
 #pragma unroll
-        for (int r = 0; r < R3; ++r) buf[(j - k) * R3 + k + 256 * r] = u[r];
+        for (int r = 0; r < R3; ++r) {
+            if (STORE) buf[(j - k) * R3 + k + 256 * r] = u[r];      // (T NB3 = 256: j = k, the index is k + 256 r)
+            else v[q * R3 + r] = u[r];
+        }
     }
-    __syncthreads();
+    if (STORE) __syncthreads();
 }
 
 }  // namespace sfft

@@ -174,20 +174,44 @@ k_rowfft_forward16(const double *__restrict__ R, const double *__restrict__ S, c
         }
     }
     __syncthreads();                                                       // tw2 visible
-    fft_core<NH>(v, buf, tw2, twW);
+    fft_core<NH, false>(v, buf, tw2, twW);
+    // Even/odd split (see k_rowfft_forward) from the registers of the last pass: this thread holds Z[k + 256 r] of its
+    // butterflies k = tid + T q, whose partners Z[NH - k - 256 r] belong to butterfly 256 - k (k = 0: to itself, at
+    // R3 - r; k = 128: to itself, at R3 - 1 - r).  Only the butterflies k >= 128 (and k = 0) go through shared memory,
+    // those with k <= 128 read their partners and produce both X[idx] and X[NH - idx]: half the exchange of a full
+    // write and read of the spectrum.  Slot of (k, r): buf[r * 257 + k] (conflict-free in k).
+    constexpr int R3 = C::R3, NB3 = C::NB3;
+#pragma unroll
+    for (int q = 0; q < NB3; ++q) {
+        const int k = tid + T * q;
+        if (k >= 128 || k == 0) {
+#pragma unroll
+            for (int r = 0; r < R3; ++r) buf[r * 257 + k] = v[q * R3 + r];
+        }
+    }
+    __syncthreads();
     double2 *dst = rhat + (((size_t)bz * (nKa + 1) + img) * H + x) * NH;
-    // even/odd split (see k_rowfft_forward)
-    for (int k = tid; k <= NH / 2 && x < H; k += T) {
-        if (k == 0) {
-            const double2 z0 = buf[0];
-            dst[0] = make_double2(z0.x + z0.y, z0.x - z0.y);
-        } else {
-            const double2 zk = buf[k], zn = buf[NH - k];
-            const double2 E = make_double2(0.5 * (zk.x + zn.x), 0.5 * (zk.y - zn.y));
-            const double2 O = make_double2(0.5 * (zk.y + zn.y), -0.5 * (zk.x - zn.x));
-            const double2 wO = cmul(__ldg(&twW[k]), O);
-            dst[k] = make_double2(E.x + wO.x, E.y + wO.y);
-            if (k != NH - k) dst[NH - k] = make_double2(E.x - wO.x, -(E.y - wO.y));
+    if (x < H) {
+#pragma unroll
+        for (int q = 0; q < NB3; ++q) {
+            const int k = tid + T * q;
+            if (k > 128) continue;
+#pragma unroll
+            for (int r = 0; r < R3; ++r) {
+                const int idx = k + 256 * r;
+                const double2 zk = v[q * R3 + r];
+                if (idx == 0) {
+                    dst[0] = make_double2(zk.x + zk.y, zk.x - zk.y);
+                    continue;
+                }
+                // partner Z[NH - idx]
+                const double2 zn = k == 0 ? buf[(R3 - r) * 257] : (k == 128 ? buf[(R3 - 1 - r) * 257 + 128] : buf[(R3 - 1 - r) * 257 + 256 - k]);
+                const double2 E = make_double2(0.5 * (zk.x + zn.x), 0.5 * (zk.y - zn.y));
+                const double2 O = make_double2(0.5 * (zk.y + zn.y), -0.5 * (zk.x - zn.x));
+                const double2 wO = cmul(__ldg(&twW[idx]), O);
+                dst[idx] = make_double2(E.x + wO.x, E.y + wO.y);
+                if (idx != NH - idx) dst[NH - idx] = make_double2(E.x - wO.x, -(E.y - wO.y));
+            }
         }
     }
 }
