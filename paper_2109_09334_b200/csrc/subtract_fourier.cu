@@ -232,6 +232,15 @@ k_rowfft_inverse_sub(const double2 *__restrict__ mhat, const double *__restrict_
         cj[threadIdx.y][tid] = s;
     }
     const double2 *X = mhat + ((size_t)bz * nimg * H + x) * NH;
+    {
+        // the row of S is only needed in the epilogue: pull it towards L2 now (one request per 128-byte line), so that
+        // its latency is not exposed a second time after the transform
+        const double2 *Sp = reinterpret_cast<const double2 *>(S + ((size_t)bz * H + x) * W);
+        if ((tid & 7) == 0) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) asm volatile("prefetch.global.L2 [%0];" ::"l"(Sp + tid + r * T));
+        }
+    }
     double2 v[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
