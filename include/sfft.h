@@ -106,7 +106,8 @@ int sfft_plan_num_background_terms(const sfft_plan *plan); /* F_B */
 size_t sfft_plan_workspace_bytes(const sfft_plan *plan);
 
 /* Lend a device buffer (>= workspace_bytes, 256-byte aligned) to the plan.  The caller keeps
- * ownership and must keep it alive until the plan is destroyed or another buffer is set. */
+ * ownership and must keep it alive until the plan is destroyed or another buffer is set.  May enqueue a
+ * clearing of part of the buffer on the plan's stream (set the stream first). */
 int sfft_plan_set_workspace(sfft_plan *plan, void *d_ws, size_t bytes);
 
 /* Steps a1-a5: assemble the normal system of Eq. 18 in real-space scaling,

@@ -293,9 +293,9 @@ class Plan:
         self.ws_bytes = sfft_plan_workspace_bytes(self.h)
         self.ws = torch.empty(self.ws_bytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (self.ws.data_ptr() + 255) & ~255
-        self._check(sfft_plan_set_workspace(self.h, ptr, self.ws_bytes), "sfft_plan_set_workspace")
         self.stream = torch.cuda.current_stream(self.device)
         self._check(sfft_plan_set_stream(self.h, self.stream.cuda_stream), "sfft_plan_set_stream")
+        self._check(sfft_plan_set_workspace(self.h, ptr, self.ws_bytes), "sfft_plan_set_workspace")
         self._check(sfft_plan_set_reuse_spectra(self.h, reuse_spectra), "sfft_plan_set_reuse_spectra")
         self.staging = None
 

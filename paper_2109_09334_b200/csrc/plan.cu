@@ -559,6 +559,13 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     p->dscale = (double *)(b + l.dscale); p->coefr = (double *)(b + l.coefr); p->ybuf = (double *)(b + l.ybuf); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
     p->built = p->solved = false;
     p->rhat_from_build = false;
+    if (!p->corr_os) {
+        // the direct lag-sum kernel never writes the (S, S) pair and the lags beyond w against S, which the
+        // y-direction sums read along with everything else (their results are not used): keep those entries defined
+        if (wrong_device(p)) return SFFT_ERR_STATE;
+        cudaError_t e = cudaMemsetAsync(p->G, 0, l.lagpart - l.G, p->stream);
+        if (e != cudaSuccess) return fail_cuda(p, e);
+    }
     return SFFT_OK;
 }
 
