@@ -120,7 +120,8 @@ __device__ __forceinline__ void corr_os_body(const double2 *__restrict__ rhat, c
         tw64[tid] = make_double2(co, s);
     }
     if (tid < d.nseq) sseq[tid] = seqs[tid];
-    for (int i = tid; i < 4 * kOsSpec; i += 512) smo[i] = make_double2(0.0, 0.0);
+    // (the spectrum slots of absent sequences - slot 7 of 8 for seven sequences - are never written: whatever they
+    // hold only reaches accumulator rows / columns p, q >= nseq, which are never stored)
     // this CTA's x-range: Sx parts of whole hops
     const int hops_total = (H + HOP - 1) / HOP, hpp = (hops_total + d.Sx - 1) / d.Sx;
     const int xb = min(H, xs * hpp * HOP), xe = min(H, xb + hpp * HOP);
