@@ -431,6 +431,15 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
 
 // T[r][0..63] = L[row0 + r][col0 ..] for r < nr (else 0) by asynchronous 16-byte copies (stride LDT)
 __device__ __forceinline__ void tile_fetch_async(double *T, const double *L, int ldl, int row0, int col0, int nr) {
+    if (nr == NB) {                      // full tile: one address, constant strides
+        const int r = threadIdx.x >> 5, c = (threadIdx.x & 31) * 2;
+        const double *src = L + (size_t)(row0 + r) * ldl + col0 + c;
+        double *dst = T + r * LDT + c;
+#pragma unroll
+        for (int q = 0; q < NB * NB / 2 / 256; ++q) cp_async16(dst + 8 * q * LDT, src + (size_t)8 * q * ldl);
+        asm volatile("cp.async.commit_group;");
+        return;
+    }
 #pragma unroll
     for (int q = 0; q < NB * NB / 2 / 256; ++q) {
         const int i = threadIdx.x + 256 * q, r = i >> 5, c = (i & 31) * 2;
@@ -470,39 +479,61 @@ __global__ void __launch_bounds__(256, 2) k_chol_update_row(double *__restrict__
     if (nri <= 0) return;
     tile_fetch_async(Ti, L, ldl, i0, jp0, nri);
     if (tj0 < ti) tile_fetch_async((tj0 & 1) ? Tj1 : Tj0, L, ldl, j1 + tj0 * NB, jp0, max(0, min(NB, n - (j1 + tj0 * NB))));
+    // interior tiles (strictly below the diagonal, every row and column inside the system): no bounds tests, addresses
+    // from two hoisted row pointers - the per-tile instruction overhead decides how well the two resident CTAs keep the
+    // tensor pipe busy
+    const bool rows_full = (i0 + NB <= n + 1);
+    double *crow0 = L + (size_t)(i0 + wm + r8) * ldl + wn + 2 * kq, *crow1 = crow0 + (size_t)8 * ldl;
     for (int tj = tj0; tj <= tj1; ++tj) {
         const int c0 = j1 + tj * NB;
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();                 // tile tj (and Ti) visible; MMAs of tile tj-1 done by every warp
         if (tj + 1 <= tj1 && tj + 1 < ti)
             tile_fetch_async((tj & 1) ? Tj0 : Tj1, L, ldl, c0 + NB, jp0, max(0, min(NB, n - (c0 + NB))));
+        const bool interior = rows_full && tj < ti && c0 + NB <= n;
         // C tile into registers ahead of the MMAs
         double2 cv[2][4];
-#pragma unroll
-        for (int a = 0; a < 2; ++a)
+        if (interior) {
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                const int i = i0 + wm + 8 * a + r8, j = c0 + wn + 8 * c + 2 * kq;
-                cv[a][c] = make_double2(0.0, 0.0);
-                if (i <= n && j + 1 < n && j + 1 <= i) cv[a][c] = *reinterpret_cast<const double2 *>(&L[(size_t)i * ldl + j]);
-                else if (i <= n && j < n && j <= i) cv[a][c].x = L[(size_t)i * ldl + j];
+                cv[0][c] = *reinterpret_cast<const double2 *>(crow0 + c0 + 8 * c);
+                cv[1][c] = *reinterpret_cast<const double2 *>(crow1 + c0 + 8 * c);
             }
+        } else {
+#pragma unroll
+            for (int a = 0; a < 2; ++a)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int i = i0 + wm + 8 * a + r8, j = c0 + wn + 8 * c + 2 * kq;
+                    cv[a][c] = make_double2(0.0, 0.0);
+                    if (i <= n && j + 1 < n && j + 1 <= i) cv[a][c] = *reinterpret_cast<const double2 *>(&L[(size_t)i * ldl + j]);
+                    else if (i <= n && j < n && j <= i) cv[a][c].x = L[(size_t)i * ldl + j];
+                }
+        }
         double acc[2][4][2];
 #pragma unroll
         for (int a = 0; a < 2; ++a)
 #pragma unroll
             for (int c = 0; c < 4; ++c) acc[a][c][0] = acc[a][c][1] = 0.0;
         mma_64(Ti, tj == ti ? Ti : ((tj & 1) ? Tj1 : Tj0), acc);
-#pragma unroll
-        for (int a = 0; a < 2; ++a)
+        if (interior) {
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                const int i = i0 + wm + 8 * a + r8, j = c0 + wn + 8 * c + 2 * kq;
-                if (i > n) continue;
-                double *dst = &L[(size_t)i * ldl + j];
-                if (j + 1 < n && j + 1 <= i) *reinterpret_cast<double2 *>(dst) = make_double2(cv[a][c].x - acc[a][c][0], cv[a][c].y - acc[a][c][1]);
-                else if (j < n && j <= i) dst[0] = cv[a][c].x - acc[a][c][0];
+                *reinterpret_cast<double2 *>(crow0 + c0 + 8 * c) = make_double2(cv[0][c].x - acc[0][c][0], cv[0][c].y - acc[0][c][1]);
+                *reinterpret_cast<double2 *>(crow1 + c0 + 8 * c) = make_double2(cv[1][c].x - acc[1][c][0], cv[1][c].y - acc[1][c][1]);
             }
+        } else {
+#pragma unroll
+            for (int a = 0; a < 2; ++a)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int i = i0 + wm + 8 * a + r8, j = c0 + wn + 8 * c + 2 * kq;
+                    if (i > n) continue;
+                    double *dst = &L[(size_t)i * ldl + j];
+                    if (j + 1 < n && j + 1 <= i) *reinterpret_cast<double2 *>(dst) = make_double2(cv[a][c].x - acc[a][c][0], cv[a][c].y - acc[a][c][1]);
+                    else if (j < n && j <= i) dst[0] = cv[a][c].x - acc[a][c][0];
+                }
+        }
     }
 }
 
