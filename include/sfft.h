@@ -58,8 +58,8 @@ enum {
  * Restrictions (INVALID_ARG otherwise): 32 <= H <= 8192, 64 <= W <= 8192, W even; L odd, 1 <= L <= 33,
  * 2L-1 <= min(H, W); DK, DB in [0, 8].  Frames whose H or W is not a power of two (NEXT-4; true CCD frames such as
  * 2046 x 4094) additionally need W <= 4096 when W is not a power of two, the polynomial basis and
- * DK <= 2: their rows are transformed by a chirp-z (Bluestein) DFT, the lag correlation takes the sectioned route
- * and sfft_subtract the direct contraction; sfft_decorrelate needs tiles that divide the frame.
+ * DK <= 2: their rows are transformed by a chirp-z (Bluestein) DFT (forward and inverse) and the lag correlation
+ * takes the sectioned route; sfft_decorrelate needs tiles that divide the frame.
  * Builds constant tables on the host and uploads them (synchronous). */
 int sfft_plan_create(sfft_plan **out, int H, int W, int L, int DK, int DB, int basis);
 

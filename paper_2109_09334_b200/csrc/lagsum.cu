@@ -55,6 +55,7 @@ __global__ void __launch_bounds__(128) k_lagsum_partial(const double2 *__restric
         if (k < L) { dst[(size_t)(2 * k) * E] = P[k]; dst[(size_t)(2 * k + 1) * E] = Q[k]; }
 }
 
+template <int NF>
 __global__ void k_lagsum_final(const double *__restrict__ part, const LagUnit *__restrict__ units, double *__restrict__ tab,
                                int nunits, int nO, int L, int E, int nch, size_t tab_size) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x, bz = blockIdx.y;
@@ -65,17 +66,19 @@ __global__ void k_lagsum_final(const double *__restrict__ part, const LagUnit *_
     const int eps = j - u.hw, k = eps < 0 ? -eps : eps;
     const double *src = part + ((size_t)bz * nch * L + k) * 2 * E + u.e;
     double P = 0.0, Q = 0.0;
-    // 32 partials (64 loads) in flight per thread: the kernel is a handful of L2 round trips long
-    for (int c8 = 0; c8 < nch; c8 += 32) {
-        double p8[32], q8[32];
+    // NF partials (2 NF loads) in flight per thread.  Many chunks and few outputs (single large frames): NF = 32, the
+    // kernel is a handful of L2 round trips long; few chunks and many outputs (batches of small frames): NF = 8, the
+    // kernel is throughput bound and lives on occupancy.  Same summation order either way (deterministic).
+    for (int c8 = 0; c8 < nch; c8 += NF) {
+        double p8[NF], q8[NF];
 #pragma unroll
-        for (int q = 0; q < 32; ++q) {
+        for (int q = 0; q < NF; ++q) {
             const bool ok = c8 + q < nch;
             p8[q] = ok ? src[(size_t)(c8 + q) * L * 2 * E] : 0.0;
             q8[q] = ok ? src[(size_t)(c8 + q) * L * 2 * E + E] : 0.0;
         }
 #pragma unroll
-        for (int q = 0; q < 32; ++q) { P += p8[q]; Q += q8[q]; }      // fixed order: deterministic
+        for (int q = 0; q < NF; ++q) { P += p8[q]; Q += q8[q]; }
     }
     const int s = (eps == 0) ? 0 : ((eps > 0) == (u.sgn > 0) ? 1 : -1);
     tab[(size_t)bz * tab_size + u.dst_off + j] = P - s * Q;
@@ -102,8 +105,12 @@ cudaError_t launch_lagsum(sfft_plan *p) {
     if (e != cudaSuccess) return e;
     const int nO = 2 * p->L - 1, total = (int)p->units.size() * nO;
     dim3 grid((total + 255) / 256, p->nbatch);
-    k_lagsum_final<<<grid, 256, 0, p->stream>>>(p->lagpart, p->dt.units, p->tab, (int)p->units.size(), nO, p->L, p->E,
-                                               p->nch, p->tab_size);
+    if (p->nch > 32)
+        k_lagsum_final<32><<<grid, 256, 0, p->stream>>>(p->lagpart, p->dt.units, p->tab, (int)p->units.size(), nO, p->L, p->E,
+                                                       p->nch, p->tab_size);
+    else
+        k_lagsum_final<8><<<grid, 256, 0, p->stream>>>(p->lagpart, p->dt.units, p->tab, (int)p->units.size(), nO, p->L, p->E,
+                                                      p->nch, p->tab_size);
     p->launches++;
     return cudaGetLastError();
 }

@@ -42,7 +42,7 @@ __global__ void k_kernel_spectrum(const double *__restrict__ kfold, const double
                                   double2 *__restrict__ khat, int Nh, int L, int FK) {
     const int m = blockIdx.x * blockDim.x + threadIdx.x, ai = blockIdx.y / FK, t = blockIdx.y - ai * FK, b = blockIdx.z;
     if (m >= Nh) return;
-    const int w = (L - 1) / 2, W = 2 * Nh;
+    const int w = (L - 1) / 2, W = 2 * Nh, wmask = (W & (W - 1)) == 0 ? W - 1 : -1;
     const double *k = kfold + (((size_t)b * FK + t) * L + ai) * L;
     double re = 0.0, im = 0.0;
     if (m == 0) {
@@ -54,7 +54,7 @@ __global__ void k_kernel_spectrum(const double *__restrict__ kfold, const double
     } else {
         for (int bi = 0; bi < L; ++bi) {
             const double v = __ldg(&k[bi]);
-            const double2 tw = __ldg(&twW[(m * (bi - w)) & (W - 1)]);
+            const double2 tw = __ldg(&twW[wrap_index(m * (bi - w), W, wmask)]);
             re = fma(v, tw.x, re);
             im = fma(v, tw.y, im);
         }
@@ -81,7 +81,11 @@ struct FirDims { int H, Nh, nimg, nKa, FK, NO, pad; };
 // terms are grouped by image, c_{j,a}(x') = sum_i khat_{(i,j),a} u_x'^i is formed per source row (f_0 = 1 costs nothing)
 // and ONE complex multiply-add per (image, tap, row) follows: 72 instead of 96 FMA per row and tap at DK = 2.
 // PDK = -1: any basis, one complex multiply-add per (term, tap, row) on the pre-weighted rows.
-template <int L, int PDK>
+// GEN = false: H a power of two (source rows wrap by mask), Nh a multiple of 32.  GEN = true: any H and Nh - rows wrap
+// by modulo, columns past the end repeat the last one and store nothing, and the x-range of a warp need not be a
+// multiple of 4 (the last group stores its live rows only).  A template parameter: the general tests cost the
+// power-of-two kernel 16 registers and 4 % otherwise.
+template <int L, int PDK, bool GEN>
 __global__ void __launch_bounds__(kFirCols *kFirWarps, 2)
 k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const Seq *__restrict__ seqs,
         const double2 *__restrict__ khat, double2 *mhat, FirDims d) {
@@ -91,17 +95,18 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
     double2 *rt = smf + (size_t)L * d.FK * kFirCols;     // [2][warp][nKa][4][32]
     __shared__ Seq sseq[kFirMaxFK];
     const int tid = threadIdx.x, col = tid & 31, wq = tid >> 5, bz = blockIdx.z;
-    const int m = blockIdx.x * kFirCols + col;
-    const bool packed = (m == 0);          // column 0 holds (X[0], X[W/2]), both real
     const int H = d.H, Nh = d.Nh, FK = d.FK, nKa = d.nKa;
+    const int mreal = blockIdx.x * kFirCols + col, m = GEN ? min(mreal, Nh - 1) : mreal;
+    const bool packed = (m == 0);          // column 0 holds (X[0], X[W/2]), both real
     for (int i = tid; i < L * FK * kFirCols; i += kFirCols * kFirWarps)
-        kh[i] = __ldg(&khat[((size_t)bz * L * FK + (i >> 5)) * Nh + blockIdx.x * kFirCols + (i & 31)]);
+        kh[i] = __ldg(&khat[((size_t)bz * L * FK + (i >> 5)) * Nh +
+                            (GEN ? min(blockIdx.x * kFirCols + (i & 31), Nh - 1) : blockIdx.x * kFirCols + (i & 31))]);
     if (tid < FK) sseq[tid] = seqs[tid];
     __syncthreads();
     const int xo0 = (blockIdx.y * kFirWarps + wq) * d.NO;
     if (xo0 >= H) return;
     const int nout = min(d.NO, H - xo0);
-    const int xs0 = xo0 - w - d.pad, lead = (2 * w + d.pad) / 4, ngroups = nout / 4 + lead;
+    const int xs0 = xo0 - w - d.pad, lead = (2 * w + d.pad) / 4, ngroups = (GEN ? (nout + 3) / 4 : nout / 4) + lead;
     const double2 *rb = rhat + (size_t)bz * d.nimg * H * Nh + m;
     double2 *out = mhat + (size_t)bz * d.nimg * H * Nh + m;               // slot nKa of the spectrum stack
     double2 *rtw = rt + (size_t)wq * nKa * 4 * kFirCols + col;
@@ -112,14 +117,14 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
     double *fws = reinterpret_cast<double *>(smf + (size_t)L * FK * kFirCols + 2 * bufstride) + wq * 2 * 4 * kFirMaxNKa;
     const int lane = col;
     auto fetch_w = [&](int g) -> double {
-        return lane < nKa * 4 ? __ldg(&xwt[(size_t)(lane >> 2) * H + ((xs0 + 4 * g + (lane & 3)) & (H - 1))]) : 0.0;
+        return lane < nKa * 4 ? __ldg(&xwt[(size_t)(lane >> 2) * H + (GEN ? wrap_index(xs0 + 4 * g + (lane & 3), H, -1) : ((xs0 + 4 * g + (lane & 3)) & (H - 1)))]) : 0.0;
     };
     auto issue = [&](int g) {
         double2 *dst = rtw + (size_t)(g & 1) * bufstride;
         for (int j = 0; j < nKa; ++j)
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const int x = (xs0 + 4 * g + q) & (H - 1);
+                const int x = GEN ? wrap_index(xs0 + 4 * g + q, H, -1) : ((xs0 + 4 * g + q) & (H - 1));
                 cp_async16(dst + (j * 4 + q) * kFirCols, rb + ((size_t)j * H + x) * Nh);
             }
         cp_async_commit();
@@ -197,7 +202,8 @@ k_fir_x(const double2 *__restrict__ rhat, const double *__restrict__ xwt, const 
         if (g >= lead) {
             const int xe = xg - w;
 #pragma unroll
-            for (int q = 0; q < 4; ++q) out[(size_t)(xe + q) * Nh] = acc[q];
+            for (int q = 0; q < 4; ++q)
+                if (!GEN || (xe + q < xo0 + nout && mreal < Nh)) out[(size_t)(xe + q) * Nh] = acc[q];
         }
 #pragma unroll
         for (int i = 0; i + 4 < NA; ++i) acc[i] = acc[i + 4];
@@ -222,7 +228,8 @@ k_rowfft_inverse_sub(const double2 *__restrict__ mhat, const double *__restrict_
     extern __shared__ double2 sm2[];
     __shared__ double cj[RPC][16];
     double2 *tw2 = sm2, *buf = sm2 + C::TW2 + threadIdx.y * C::BUF;
-    const int tid = threadIdx.x, x = blockIdx.x * RPC + threadIdx.y, bz = blockIdx.y;
+    // (H need not be a multiple of RPC: a row slot past the end works on the last row again and stores nothing)
+    const int tid = threadIdx.x, xslot = blockIdx.x * RPC + threadIdx.y, x = min(xslot, H - 1), bz = blockIdx.y;
     if (threadIdx.y == 0) fft_load_tw2<NH>(tw2, twW);
     if (tid < nBa) {                 // background of this row as nBa coefficients of the y-basis
         const double *cb = coef + (size_t)bz * n + (n - FB);
@@ -283,8 +290,95 @@ k_rowfft_inverse_sub(const double2 *__restrict__ mhat, const double *__restrict_
                 b1 = fma(c, g.y, b1);
             }
         }
-        Dr[nn] = make_double2(sv.x - zz.x * inv - b0, sv.y + zz.y * inv - b1);
+        if (xslot < H) Dr[nn] = make_double2(sv.x - zz.x * inv - b0, sv.y + zz.y * inv - b1);
     }
+}
+
+// The same for W not a power of two (W even): the N = W/2 point inverse transform is conj(DFT_N(conj Z)) / N with the
+// DFT run as a chirp-z (Bluestein) transform on two M-point register FFTs, exactly as in k_rowfft_forward_bs
+// (rowfft.cu): DFT_N(v)[k] = c[k] conv[k], conv = IFFT_M(FFT_M(v c) * bhat).  One CTA of M/16 threads per row.
+template <int M>
+__global__ void __launch_bounds__(FftCfg<M>::T)
+k_rowfft_inverse_sub_bs(const double2 *__restrict__ mhat, const double *__restrict__ S, double *__restrict__ D,
+                        const double *__restrict__ coef, const double *__restrict__ xwt, const double *__restrict__ gB,
+                        const int *__restrict__ bti, const int *__restrict__ btj, const double2 *__restrict__ twW,
+                        const double2 *__restrict__ twM, const double2 *__restrict__ chirp, const double2 *__restrict__ bhat,
+                        int H, int W, int nimg, int nKa, int nBa, int FB, int n) {
+    using C = FftCfg<M>;
+    constexpr int T = C::T;
+    extern __shared__ double2 sm4[];
+    __shared__ double cj[16];
+    double2 *tw2 = sm4, *buf = sm4 + C::TW2;
+    const int tid = threadIdx.x, x = blockIdx.x, bz = blockIdx.y, N = W / 2;
+    fft_load_tw2<M>(tw2, twM);
+    if (tid < nBa) {                 // background of this row as nBa coefficients of the y-basis
+        const double *cb = coef + (size_t)bz * n + (n - FB);
+        double s = 0.0;
+        for (int q = 0; q < FB; ++q)
+            if (btj[q] == tid) s = fma(cb[q], __ldg(&xwt[(size_t)(nKa + bti[q]) * H + x]), s);
+        cj[tid] = s;
+    }
+    const double2 *X = mhat + ((size_t)bz * nimg * H + x) * N;
+    double2 v[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int k = tid + r * T;
+        v[r] = make_double2(0.0, 0.0);
+        if (k < N) {
+            const double2 xk = __ldg(&X[k]);
+            double2 z;
+            if (k == 0) {
+                z = make_double2(0.5 * (xk.x + xk.y), -0.5 * (xk.x - xk.y));           // conj(E + iO), E, O real
+            } else {
+                const double2 xn = __ldg(&X[N - k]), tw = __ldg(&twW[k]);
+                const double2 E = make_double2(0.5 * (xk.x + xn.x), 0.5 * (xk.y - xn.y));
+                const double2 Dm = make_double2(0.5 * (xk.x - xn.x), 0.5 * (xk.y + xn.y));
+                const double2 O = make_double2(Dm.x * tw.x + Dm.y * tw.y, Dm.y * tw.x - Dm.x * tw.y);   // Dm * conj(tw)
+                z = make_double2(E.x - O.y, -(E.y + O.x));                               // conj(E + iO)
+            }
+            v[r] = cmulf(z, __ldg(&chirp[k]));
+        }
+    }
+    __syncthreads();                                                       // tw2, cj visible
+    fft_core<M>(v, buf, tw2, twM);
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int k = tid + r * T;
+        const double2 t = cmulf(buf[k], __ldg(&bhat[k]));
+        v[r] = make_double2(t.x, -t.y);
+    }
+    __syncthreads();                                                       // buf consumed before it is rewritten
+    fft_core<M>(v, buf, tw2, twM);
+    const size_t o = ((size_t)bz * H + x) * W;
+    const double2 *Sr = reinterpret_cast<const double2 *>(S + o);
+    double2 *Dr = reinterpret_cast<double2 *>(D + o);
+    const double inv = 1.0 / ((double)M * (double)N);
+    for (int nn = tid; nn < N; nn += T) {
+        const double2 u = buf[nn];
+        const double2 y = cmulf(make_double2(u.x, -u.y), __ldg(&chirp[nn]));           // M * DFT_N(v)[nn]
+        const double2 sv = Sr[nn];
+        double b0 = 0.0, b1 = 0.0;
+        for (int j = 0; j < nBa; ++j) {
+            const double2 g = __ldg(reinterpret_cast<const double2 *>(gB + (size_t)j * W) + nn);
+            b0 = fma(cj[j], g.x, b0);
+            b1 = fma(cj[j], g.y, b1);
+        }
+        Dr[nn] = make_double2(sv.x - y.x * inv - b0, sv.y + y.y * inv - b1);             // z = conj(y) / (M N)
+    }
+}
+
+template <int M>
+cudaError_t launch_inv_bs(sfft_plan *p, const double *d_coef, const double *dS, double *dD) {
+    using C = FftCfg<M>;
+    const size_t smem = (size_t)(C::TW2 + C::BUF) * sizeof(double2);
+    auto kern = k_rowfft_inverse_sub_bs<M>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<dim3(p->H, p->nbatch), C::T, smem, p->stream>>>(
+        p->rhat + (size_t)p->nKa * p->H * p->Nh, dS, dD, d_coef, p->dt.xwt, p->dt.gB, p->dt.bti, p->dt.btj, p->dt.twW, p->dt.twM,
+        p->dt.chirp, p->dt.bhat, p->H, p->W, p->nimg, p->nKa, p->nBa, p->FB, p->n);
+    p->launches++;
+    return cudaGetLastError();
 }
 
 template <int NH>
@@ -295,7 +389,7 @@ cudaError_t launch_inv(sfft_plan *p, const double *d_coef, const double *dS, dou
     auto kern = k_rowfft_inverse_sub<NH>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<dim3(p->H / RPC, p->nbatch), dim3(T, RPC), smem, p->stream>>>(
+    kern<<<dim3((p->H + RPC - 1) / RPC, p->nbatch), dim3(T, RPC), smem, p->stream>>>(
         p->rhat + (size_t)p->nKa * p->H * p->Nh, dS, dD, d_coef, p->dt.xwt, p->dt.gB, p->dt.bti, p->dt.btj, p->dt.twW,
         p->H, p->nimg, p->nKa, p->nBa, p->FB, p->n, p->basis == SFFT_BASIS_POLY);
     p->launches++;
@@ -307,16 +401,22 @@ size_t fir_smem(const sfft_plan *p) {
            (size_t)kFirWarps * 2 * 4 * kFirMaxNKa * sizeof(double);
 }
 
-template <int L, int PDK>
-cudaError_t launch_fir_k(sfft_plan *p, const FirDims &d, int ny) {
-    auto kern = k_fir_x<L, PDK>;
+template <int L, int PDK, bool GEN>
+cudaError_t launch_fir_k2(sfft_plan *p, const FirDims &d, int ny) {
+    auto kern = k_fir_x<L, PDK, GEN>;
     const size_t smem = fir_smem(p);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<dim3(p->Nh / kFirCols, ny, p->nbatch), kFirCols * kFirWarps, smem, p->stream>>>(
+    kern<<<dim3((p->Nh + kFirCols - 1) / kFirCols, ny, p->nbatch), kFirCols * kFirWarps, smem, p->stream>>>(
         p->rhat, p->dt.xwt, p->dt.seqs, p->khat, p->rhat + (size_t)p->nKa * p->H * p->Nh, d);
     p->launches++;
     return cudaGetLastError();
+}
+
+template <int L, int PDK>
+cudaError_t launch_fir_k(sfft_plan *p, const FirDims &d, int ny) {
+    const bool simple = (p->H & (p->H - 1)) == 0 && p->Nh % kFirCols == 0;
+    return simple ? launch_fir_k2<L, PDK, false>(p, d, ny) : launch_fir_k2<L, PDK, true>(p, d, ny);
 }
 
 template <int L>
@@ -334,7 +434,6 @@ cudaError_t launch_fir(sfft_plan *p, const FirDims &d, int ny) {
 // pixel, plus the transforms, on the plain FMA pipe at ~half the efficiency of the tensor-core contraction)
 // is below the direct form's (L+7) * KP tensor-core MACs per pixel.
 bool subtract_use_fourier(const sfft_plan *p) {
-    if (!p->pow2) return false;            // frames that are not powers of two take the direct contraction
     if (p->Nh < 512 || p->L < 9 || p->L > 25 || p->FK > kFirMaxFK || p->nKa > kFirMaxNKa || p->nBa > 16) return false;
     if (fir_smem(p) > 200 * 1024) return false;
     const double direct = (double)(p->L + 7) * subtract_kpad(p->nKa, p->L);
@@ -360,7 +459,7 @@ cudaError_t launch_subtract_fourier(sfft_plan *p, const double *d_coef, const do
     prof_mark(p, 9);
     // x-ranges: whole waves of 2 CTAs per SM, each warp pays a halo of 2w + pad source rows
     FirDims d{p->H, p->Nh, p->nimg, p->nKa, p->FK, 0, (4 - (2 * w) % 4) % 4};
-    const int ncb = p->Nh / kFirCols * p->nbatch;
+    const int ncb = (p->Nh + kFirCols - 1) / kFirCols * p->nbatch;
     double best = 1e300; int bny = 1;
     for (int ny = 1; ny <= 64; ++ny) {
         int NO = ((p->H + kFirWarps * ny - 1) / (kFirWarps * ny) + 3) / 4 * 4;
@@ -376,6 +475,13 @@ cudaError_t launch_subtract_fourier(sfft_plan *p, const double *d_coef, const do
         default: return cudaErrorInvalidValue;
     }
     if (e != cudaSuccess) return e;
+    switch (p->bsM) {
+        case 0: break;
+        case 1024: return launch_inv_bs<1024>(p, d_coef, dS, dD);
+        case 2048: return launch_inv_bs<2048>(p, d_coef, dS, dD);
+        case 4096: return launch_inv_bs<4096>(p, d_coef, dS, dD);
+        default: return cudaErrorInvalidValue;
+    }
     switch (p->Nh) {
         case 512: return launch_inv<512>(p, d_coef, dS, dD);
         case 1024: return launch_inv<1024>(p, d_coef, dS, dD);

@@ -350,6 +350,10 @@ def test_parity_constant_photometric_ratio(cuda_device, cfg, H, W, L, basis, DK,
     (3, 186, 372, 15, 2, 2),      # 2046 x 4094 scaled by 1/11: wide kernel, several hops and a ragged last one
     (2, 90, 1024, 5, 1, 1),       # only H is not a power of two (rows per CTA do not divide H)
     (2, 128, 1000, 9, 2, 0),      # only W is not a power of two
+    (2, 100, 2046, 9, 2, 1),      # Fourier-route subtract on chirp-z rows (W/2 = 1023 >= 512, L >= 9): FIR with a ragged
+                                  # last column block and x-range, inverse chirp-z transform
+    (2, 90, 1024, 9, 1, 1),       # Fourier route, W a power of two, H not a multiple of the rows per CTA
+    (3, 62, 4094, 15, 2, 2),      # Fourier route at the DECam row length, M = 4096
 ])
 def test_parity_frames_not_powers_of_two(cuda_device, cfg, H, W, L, DK, DB):
     """NEXT-4 (true CCD frames such as 2046 x 4094): any H, even W - chirp-z row transforms, general
