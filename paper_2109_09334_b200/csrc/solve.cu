@@ -742,7 +742,10 @@ k_chol_backsolve_lb(const __grid_constant__ CUtensorMap tmL, const double *__res
     }
     __syncthreads();
     if (tid < NB) {
-        const double y = (tid < nbk) ? (red[0][tid] + red[1][tid]) + (red[2][tid] + red[3][tid]) : 0.0;
+        double y = (tid < nbk) ? (red[0][tid] + red[1][tid]) + (red[2][tid] + red[3][tid]) : 0.0;
+        // a NaN that happens to carry the sentinel's payload (propagated from the input) must not read as "not yet
+        // published" to the CTAs waiting for it
+        if ((unsigned long long)__double_as_longlong(y) == kBsSentinel) y = __longlong_as_double(0x7ff8000000000000ll);
         st_volatile_f64(&yb[(size_t)blk * NB + tid], y);
         if (tid < nbk) coef[(size_t)bz * n + i0 + tid] = y * dscale[(size_t)bz * n + i0 + tid];
     }

@@ -700,6 +700,24 @@ def test_numerically_rank_deficient_input_reports_not_spd(cuda_device):
     plan.close()
 
 
+@pytest.mark.timeout(300)
+def test_nan_input_with_sentinel_payload_does_not_stall_the_back_substitution(cuda_device):
+    """The look-back back substitution marks "block not yet published" with a NaN bit pattern.  A NaN of that very payload
+    in the input propagates through the arithmetic: the solve must still terminate and report SFFT_ERR_NOT_SPD."""
+    import struct
+    import torch
+    p = synth.make_pair(1)
+    R = p.R.copy()
+    R[17, 23] = struct.unpack("<d", struct.pack("<Q", 0xFFF8DEADBEEF5AFE))[0]
+    plan = B.Plan(p.H, p.W, p.L, p.DK, p.DB, p.basis)
+    dR, dS = torch.from_numpy(R).cuda(), torch.from_numpy(p.S).cuda()
+    plan.build_system(dR, dS)
+    plan.solve()
+    st, _ = plan.status(check=False)
+    assert st == B.SFFT_ERR_NOT_SPD
+    plan.close()
+
+
 def test_argument_and_state_errors(cuda_device):
     import torch
     for bad in [(100, 129, 7, 1, 1, 0), (100, 4100, 7, 1, 1, 0), (100, 130, 7, 1, 1, 1), (100, 130, 7, 3, 1, 0), (128, 128, 6, 1, 1, 0), (128, 128, 7, -1, 1, 0), (128, 128, 7, 1, 1, 2),
