@@ -73,6 +73,9 @@ CASES = [
     (2, 256, 1024, 11, None, 1, 0),                   # Fourier route, 2w % 4 == 2 (padded lead-in), several x-ranges
     (3, 128, 2048, 15, None, 2, 2),                   # Fourier route, L = 15
     (4, 64, 4096, 17, None, 2, 2),                    # Fourier route at the headline width and kernel size
+    (2, 128, 128, 33, None, 0, 0),                    # the largest kernel (L = 33: 65 lags per axis, 32-row hops)
+    (2, 64, 1024, 25, None, 1, 1),                    # the widest kernel of the Fourier-route subtract (L = 25)
+    (2, 128, 256, 27, None, 1, 0),                    # L = 27: direct subtract with 27 taps
     (5, 128, 128, 5, "bspline", 1, 0),                # B-spline weights
     (5, 256, 256, 5, "bspline", 4, 4),                # config-5 basis (8x8 functions), n = 1664
 ]
