@@ -370,6 +370,44 @@ def test_parity_frames_not_powers_of_two(cuda_device, cfg, H, W, L, DK, DB):
     assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
 
 
+def test_combination_batch_rect_cpr_on_a_frame_not_a_power_of_two(cuda_device):
+    """The section-8(f) options together: a batch of 2 pairs of 90 x 132 pixels, a 5 x 7 kernel, the constant
+    photometric ratio; and the smallest frame the plan accepts (32 x 64)."""
+    import torch
+    L0, L1, DK, DB = 5, 7, 2, 1
+    L = max(L0, L1)
+    pairs = [synth.make_pair(2, H=90, W=132, seed=77 + e) for e in range(2)]
+    R, S = np.stack([q.R for q in pairs]), np.stack([q.S for q in pairs])
+    plan = B.Plan(90, 132, (L0, L1), DK, DB, "poly", nbatch=2, const_phot_ratio=True)
+    dR, dS = torch.from_numpy(R).cuda(), torch.from_numpy(S).cuda()
+    plan.build_system(dR, dS)
+    coef = plan.solve()
+    D = plan.subtract(coef, dR, dS).cpu().numpy()
+    plan.status()
+    FK, FB = oracle.num_terms(oracle.POLY, DK), oracle.num_terms(oracle.POLY, DB)
+    a0 = ((L - 1) // 2) * L + (L - 1) // 2
+    sel = oracle.rect_select(L0, L1, oracle.POLY, DK, DB)
+    sel = np.array([k for k in sel if not (k < FK * L * L and k % (L * L) == a0 and k // (L * L) > 0)])
+    assert plan.ns == len(sel)
+    for e in range(2):
+        Mf, rf = oracle.normal_from_lags(R[e], S[e], L, oracle.POLY, DK, DB)
+        Mo, ro = Mf[np.ix_(sel, sel)], rf[sel]
+        co = np.zeros(Mf.shape[0])
+        co[sel] = oracle.solve(Mo, ro)
+        M, rhs = plan.system(batch=e)
+        _check_system(M.cpu().numpy(), rhs.cpu().numpy(), Mo, ro, S[e])
+        _check_coef(coef[e].cpu().numpy(), co, Mf.shape[0] - FB)
+        Do = oracle.difference(R[e], S[e], co, L, oracle.POLY, DK, DB)
+        assert np.max(np.abs(D[e] - Do)) <= TOL_D * pairs[e].sigma
+    plan.close()
+    p = synth.make_pair(1, H=32, W=64)
+    Mo, ro, co, Do = _oracle_all(p.R, p.S, 3, "poly", 1, 1)
+    M, rhs, c, D = _gpu_all(torch, p, 3, "poly", 1, 1)
+    _check_system(M[0], rhs[0], Mo, ro, p.S)
+    _check_coef(c[0], co, Mo.shape[0] - 3)
+    assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
+
+
 @pytest.mark.parametrize("cfg,H,W,L0,L1,basis,DK,DB,cpr", [
     (2, 128, 256, 5, 9, "poly", 2, 1, False),       # wider along y; direct-route subtract
     (2, 64, 1024, 13, 7, "poly", 1, 1, False),      # wider along x; Fourier-route subtract (W >= 1024, L = 13)
