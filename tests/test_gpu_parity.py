@@ -605,7 +605,8 @@ def test_mask_fill_and_masked_fit_flow(cuda_device, cfg, H, W, L, rd, rb, nb):
 
 
 @pytest.mark.parametrize("cfg,H,W,L,DK,tile,coadd", [(1, 128, 128, 7, 1, 32, False), (2, 256, 512, 11, 2, 128, True),
-                                                        (2, 512, 512, 9, 2, 512, False), (2, 64, 1024, 5, 0, 64, True)])
+                                                        (2, 512, 512, 9, 2, 512, False), (2, 64, 1024, 5, 0, 64, True),
+                                                        (1, 96, 160, 7, 1, 32, False)])
 def test_decorrelation_parity(cuda_device, cfg, H, W, L, DK, tile, coadd):
     """NEXT-3 (App. C, Eq. C20; DESIGN g22): fit, subtract, then decorrelate on the GPU; the oracle decorrelates the
     GPU's difference image with the GPU's coefficients (both already checked against the oracle elsewhere), so this
