@@ -760,6 +760,49 @@ def test_nan_input_with_sentinel_payload_does_not_stall_the_back_substitution(cu
     plan.close()
 
 
+def test_step_is_capturable_in_a_cuda_graph(cuda_device):
+    """build -> solve -> subtract captured once in a CUDA graph (side-stream fork / join of the moment stage,
+    programmatic dependent launches of the panel chain, TMA tile copies of the back substitution) and replayed on
+    new contents of the same buffers gives the result of the direct calls."""
+    import torch
+    p = synth.make_pair(2, H=128, W=1024)
+    q = synth.make_pair(2, H=128, W=1024, seed=5)
+    plan = B.Plan(p.H, p.W, 9, 2, 1, "poly")
+    dR, dS = torch.from_numpy(p.R).cuda(), torch.from_numpy(p.S).cuda()
+    dD = torch.empty_like(dS)
+    coef = torch.empty((1, plan.n), dtype=torch.float64, device="cuda")
+
+    def step():
+        plan.build_system(dR, dS)
+        plan.solve(coef)
+        plan.subtract(coef, dR, dS, dD)
+
+    step()
+    plan.status()
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        B.sfft_plan_set_stream(plan.h, s.cuda_stream)
+        step()
+        torch.cuda.synchronize()
+        g.capture_begin()
+        step()
+        g.capture_end()
+    torch.cuda.synchronize()
+    dR.copy_(torch.from_numpy(q.R))
+    dS.copy_(torch.from_numpy(q.S))
+    g.replay()
+    torch.cuda.synchronize()
+    Dg, cg = dD.clone(), coef.clone()
+    B.sfft_plan_set_stream(plan.h, plan.stream.cuda_stream)
+    step()
+    plan.status()
+    assert torch.equal(dD, Dg) and torch.equal(coef, cg)
+    Mo, ro, co, Do = _oracle_all(q.R, q.S, 9, "poly", 2, 1)
+    assert np.max(np.abs(Dg.cpu().numpy() - Do)) <= TOL_D * q.sigma
+    plan.close()
+
+
 def test_argument_and_state_errors(cuda_device):
     import torch
     for bad in [(100, 129, 7, 1, 1, 0), (100, 4100, 7, 1, 1, 0), (100, 130, 7, 1, 1, 1), (100, 130, 7, 3, 1, 0), (128, 128, 6, 1, 1, 0), (128, 128, 7, -1, 1, 0), (128, 128, 7, 1, 1, 2),
