@@ -168,6 +168,36 @@ int sfft_plan_set_reuse_spectra(sfft_plan *plan, int on);
 int sfft_mask_fill(sfft_plan *plan, const double *d_R, const double *d_S, double sat_R, double sat_S, int rd, int rb,
                    double *d_Rm, double *d_Sm, unsigned char *d_mask);
 
+/* The same mask/fill for ONE pair (nbatch = 1), for callers that have no way to obtain device memory for the
+ * library: no plan, no workspace, and no cudaMalloc / cudaFree / allocating library routine anywhere in the call.
+ * Who needs this: a process whose device memory was all handed to one pool at start-up (a late cudaMalloc there
+ * fails, or falls outside the pool's accounting), and a loop that must never stall (cudaMalloc and cudaFree
+ * synchronise the whole device).  sfft_plan_create uploads tables into memory it allocates and sfft_mask_fill wants a
+ * lent workspace, so neither serves such a caller; this call takes the five images and nothing else.
+ *   Its scratch (row-grown seed flags, one byte per pixel, plus 8 KiB of partial sums) lives in an array that is part
+ *   of the library image: SFFT_STATIC_MAX_PIXELS + 8192 bytes (16 MiB + 8 KiB) of device memory on EVERY GPU on which
+ *   the process uses this library, held from the moment the library's device code is loaded there until the process
+ *   exits, whether or not this call is ever made.
+ *   Limits: 1 <= H, W <= 16384 and H*W <= SFFT_STATIC_MAX_PIXELS (4096 x 4096, which covers the 2046 x 4094 CCD
+ *   frame); anything larger is refused with SFFT_ERR_INVALID_ARG and a message naming the limit
+ *   (sfft_static_last_error).  rd, rb, sat_*, the pointer roles, aliasing and layout are those of sfft_mask_fill,
+ *   and so is the result, bit for bit (the same kernels run).  Any H and W are accepted (indices wrap by modulo).
+ *   Set-up: the first call on each device looks up the device address of the scratch array (once per device, cached;
+ *   the device that is current at the call is the one used, and d_* and cuda_stream must belong to it).  That
+ *   look-up may make the CUDA runtime load the library's device code, so issue the first call on a device ahead of
+ *   any stream capture and ahead of the section that must not stall.
+ *   Sharing: every call on a device uses the same scratch, and the scratch keeps the previous call's contents.
+ *   Nothing in it has to start at zero: each call writes every entry it later reads (H*W flags, 768 partial sums,
+ *   2 means) before reading it, so no clearing pass is run.  Two calls that can overlap on the GPU (different
+ *   streams, or different host threads without ordering) race on it and both results are garbage: order them on one
+ *   stream or with events.
+ *   cuda_stream: cudaStream_t cast to void* (NULL = legacy default stream).  Work is enqueued, not synchronised.
+ * sfft_static_last_error: message of the last failing sfft_mask_fill_static call of the calling thread ("" if none). */
+#define SFFT_STATIC_MAX_PIXELS (4096L * 4096L)
+int sfft_mask_fill_static(const double *d_R, const double *d_S, int H, int W, double sat_R, double sat_S, int rd,
+                          int rb, double *d_Rm, double *d_Sm, unsigned char *d_mask, void *cuda_stream);
+const char *sfft_static_last_error(void);
+
 /* NEXT-3, noise decorrelation of a difference image (App. C; readings DESIGN g22).  With
  *   D = sum_j S_j (*) G_j - [sum_i R_i (*) H_i] (*) K                                            (C17)
  *   Q0^ = sqrt( sigma_D^2 / { sum_j varS_j |G_j^|^2 + sum_i varR_i |K^|^2 |H_i^|^2 } )           (C20)

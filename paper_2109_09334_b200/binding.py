@@ -20,7 +20,7 @@ EXPORTS = [
     "sfft_plan_create", "sfft_plan_create_rect", "sfft_plan_set_batch", "sfft_plan_set_stream", "sfft_plan_set_const_phot_ratio", "sfft_plan_set_corr_route", "sfft_plan_num_solved", "sfft_plan_num_unknowns",
     "sfft_plan_num_kernel_terms", "sfft_plan_num_background_terms", "sfft_plan_workspace_bytes",
     "sfft_plan_set_workspace", "sfft_build_system", "sfft_get_system", "sfft_get_lag_table", "sfft_solve",
-    "sfft_subtract", "sfft_mask_fill", "sfft_decorrelate", "sfft_plan_set_reuse_spectra", "sfft_plan_status", "sfft_plan_host_staging_bytes", "sfft_plan_set_host_staging",
+    "sfft_subtract", "sfft_mask_fill", "sfft_mask_fill_static", "sfft_static_last_error", "sfft_decorrelate", "sfft_plan_set_reuse_spectra", "sfft_plan_status", "sfft_plan_host_staging_bytes", "sfft_plan_set_host_staging",
     "sfft_run_host", "sfft_run_host_async", "sfft_run_host_wait", "sfft_run_host_f32", "sfft_run_host_async_f32", "sfft_plan_launch_count", "sfft_plan_destroy",
     "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
 ]
@@ -72,6 +72,8 @@ def load_library(build_if_missing=True):
         "sfft_solve": (ci, [vp, vp]),
         "sfft_subtract": (ci, [vp, vp, vp, vp, vp]),
         "sfft_mask_fill": (ci, [vp, vp, vp, ctypes.c_double, ctypes.c_double, ci, ci, vp, vp, vp]),
+        "sfft_mask_fill_static": (ci, [vp, vp, ci, ci, ctypes.c_double, ctypes.c_double, ci, ci, vp, vp, vp, vp]),
+        "sfft_static_last_error": (ctypes.c_char_p, []),
         "sfft_decorrelate": (ci, [vp, vp, vp, vp, ci, ci, vp, ci, vp, ci, vp, ci, vp]),
         "sfft_plan_set_reuse_spectra": (ci, [vp, ci]),
         "sfft_plan_status": (ci, [vp, pci]),
@@ -180,6 +182,36 @@ def sfft_mask_fill(plan, d_R, d_S, sat_R, sat_S, rd, rb, d_Rm, d_Sm, d_mask):
     return load_library().sfft_mask_fill(plan, ctypes.c_void_p(d_R), ctypes.c_void_p(d_S), float(sat_R), float(sat_S),
                                          int(rd), int(rb), ctypes.c_void_p(d_Rm), ctypes.c_void_p(d_Sm),
                                          ctypes.c_void_p(d_mask))
+
+
+SFFT_STATIC_MAX_PIXELS = 4096 * 4096
+
+
+def sfft_mask_fill_static(d_R, d_S, H, W, sat_R, sat_S, rd, rb, d_Rm, d_Sm, d_mask, stream_ptr=0):
+    """sfft_mask_fill for one pair without a plan or a workspace: the call allocates no device memory (its scratch is
+    an array inside the library, good for H*W <= SFFT_STATIC_MAX_PIXELS).  All five images are device pointers the
+    caller owns.  See include/sfft.h for who this is for and for the sharing rules."""
+    return load_library().sfft_mask_fill_static(ctypes.c_void_p(d_R), ctypes.c_void_p(d_S), int(H), int(W), float(sat_R),
+                                                float(sat_S), int(rd), int(rb), ctypes.c_void_p(d_Rm), ctypes.c_void_p(d_Sm),
+                                                ctypes.c_void_p(d_mask), ctypes.c_void_p(stream_ptr))
+
+
+def sfft_static_last_error():
+    return load_library().sfft_static_last_error().decode()
+
+
+def mask_fill_static(R, S, sat_R, sat_S, rd, rb, Rm, Sm, mask):
+    """sfft_mask_fill_static on torch tensors, on torch's current stream.  For code that may not allocate on the
+    device: the caller brings R, S (H x W float64, CUDA, contiguous) AND the outputs Rm, Sm (same, may be R, S
+    themselves) and mask (uint8); nothing is created here.  Raises SfftError carrying the library's message, e.g. when
+    the frame is larger than the built-in scratch."""
+    import torch
+    assert R.dim() == 2 and R.is_cuda and all(t.is_cuda and t.is_contiguous() and t.shape == R.shape for t in (S, Rm, Sm, mask))
+    assert all(t.dtype == torch.float64 for t in (R, S, Rm, Sm)) and mask.dtype == torch.uint8
+    st = sfft_mask_fill_static(R.data_ptr(), S.data_ptr(), R.shape[0], R.shape[1], sat_R, sat_S, rd, rb, Rm.data_ptr(),
+                               Sm.data_ptr(), mask.data_ptr(), torch.cuda.current_stream(R.device).cuda_stream)
+    if st != SFFT_OK:
+        raise SfftError(st, "sfft_mask_fill_static", sfft_static_last_error())
 
 
 def sfft_decorrelate(plan, d_coef, d_D, d_Ddc, tile, var_S, G, var_R, H):

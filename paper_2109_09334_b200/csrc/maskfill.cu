@@ -6,6 +6,8 @@
 //   (no unmasked pixel there: mean of all unmasked pixels of the image); unmasked pixels are copied.
 // The square growth is separable (rows, then columns).  HBM-bound streaming passes over the pair; the fill gathers
 // only at the (few) masked pixels.
+#include <mutex>
+
 #include "sfft_internal.h"
 
 namespace sfft {
@@ -112,3 +114,77 @@ cudaError_t launch_mask_fill(sfft_plan *p, const double *dR, const double *dS, d
 }
 
 }  // namespace sfft
+
+// ---- sfft_mask_fill_static: the mask/fill of one pair with its scratch inside the library image ---------------
+// For callers that cannot give the library device memory and must not have it allocate any (a process whose memory
+// all belongs to one pool, a loop that may not stall on cudaMalloc's device-wide synchronisation): no plan, no
+// workspace, no cudaMalloc / cudaFree.  The kernels are the ones launch_mask_fill runs; only the scratch differs.
+constexpr size_t kStaticHead = 8192;      // partial sums [256][3] doubles (6144 B) + the two means, rounded up
+constexpr int kStaticMaxDev = 64;
+
+// Scratch of sfft_mask_fill_static: [0, kStaticHead) partial sums and means, then one flag byte per pixel.  Shared by
+// every call on the device and never cleared (each call writes what it reads).  Costs its size on every GPU that loads
+// this library, until the process exits.
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticHead + SFFT_STATIC_MAX_PIXELS];
+
+namespace {
+
+// In host code `g_static_scratch` is only a handle for the runtime, not somewhere a kernel may write: the address
+// kernels get is asked for once per device (with that device current) and kept here.
+std::mutex g_static_mu;
+unsigned char *g_static_ptr[kStaticMaxDev] = {};
+thread_local std::string g_static_err;
+
+int static_fail(int status, const std::string &msg) {
+    g_static_err = msg;
+    return status;
+}
+
+}  // namespace
+
+extern "C" const char *sfft_static_last_error(void) { return g_static_err.c_str(); }
+
+extern "C" int sfft_mask_fill_static(const double *d_R, const double *d_S, int H, int W, double sat_R, double sat_S,
+                                     int rd, int rb, double *d_Rm, double *d_Sm, unsigned char *d_mask,
+                                     void *cuda_stream) {
+    if (!d_R || !d_S || !d_Rm || !d_Sm || !d_mask)
+        return static_fail(SFFT_ERR_INVALID_ARG, "sfft_mask_fill_static: null image pointer");
+    if (H < 1 || W < 1 || H > 16384 || W > 16384 || (long)H * (long)W > SFFT_STATIC_MAX_PIXELS)
+        return static_fail(SFFT_ERR_INVALID_ARG,
+                           "sfft_mask_fill_static: frame of " + std::to_string(H) + " x " + std::to_string(W) +
+                               " pixels exceeds the built-in scratch (1 <= H, W <= 16384 and H*W <= " +
+                               std::to_string(SFFT_STATIC_MAX_PIXELS) + "); use sfft_mask_fill with a workspace");
+    if (rd < 0 || rd > 64 || rb < 1 || rb > 128 || !(sat_R == sat_R) || !(sat_S == sat_S))
+        return static_fail(SFFT_ERR_INVALID_ARG, "sfft_mask_fill_static: need 0 <= rd <= 64, 1 <= rb <= 128, sat_* not NaN");
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return static_fail(SFFT_ERR_CUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+    if (dev < 0 || dev >= kStaticMaxDev) return static_fail(SFFT_ERR_CUDA, "sfft_mask_fill_static: device ordinal above 63");
+    unsigned char *scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        if (!g_static_ptr[dev]) {       // first call on this device: its copy of the array has its own address
+            void *sym = nullptr;
+            e = cudaGetSymbolAddress(&sym, g_static_scratch);
+            if (e != cudaSuccess || !sym) {
+                cudaGetLastError();
+                return static_fail(SFFT_ERR_CUDA, std::string("cudaGetSymbolAddress(scratch): ") + cudaGetErrorString(e));
+            }
+            g_static_ptr[dev] = static_cast<unsigned char *>(sym);
+        }
+        scratch = g_static_ptr[dev];
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int nblk = 256;
+    double *part = reinterpret_cast<double *>(scratch), *gmean = part + (size_t)nblk * 3;
+    unsigned char *t = scratch + kStaticHead;
+    const dim3 grid((W + 255) / 256, H, 1);
+    sfft::k_mask_rows<<<grid, 256, 0, st>>>(d_R, d_S, t, H, W, rd, sat_R, sat_S);
+    sfft::k_mask_cols<<<grid, 256, 0, st>>>(t, d_mask, H, W, rd);
+    sfft::k_unmasked_partial<<<dim3(nblk, 1), 256, 0, st>>>(d_R, d_S, d_mask, part, (size_t)H * W, nblk);
+    sfft::k_unmasked_mean<<<1, 32, 0, st>>>(part, gmean, nblk);
+    sfft::k_fill<<<grid, 256, 0, st>>>(d_R, d_S, d_mask, gmean, d_Rm, d_Sm, H, W, rb);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return static_fail(SFFT_ERR_CUDA, std::string("sfft_mask_fill_static launch: ") + cudaGetErrorString(e));
+    return SFFT_OK;
+}
