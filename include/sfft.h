@@ -92,7 +92,8 @@ int sfft_plan_num_solved(const sfft_plan *plan);
 /* Route of the x-direction lag correlation (steps a3+a4): 0 = chosen by the plan (default), 1 = direct lag sums
  * on the FP64 tensor cores, 2 = sectioned (overlap-save) correlation with 64-point FFTs along x, available for
  * polynomial bases with at most 8 column sequences (F_K + 1 <= 8), SFFT_ERR_INVALID_ARG otherwise.  Both routes
- * evaluate the same sums (App. B); the setter exists so that parity tests and benchmarks can
+ * evaluate the same sums (App. B) and agree to rounding (bit for bit in their x-weights only when H
+ * is a power of two); the setter exists so that parity tests and benchmarks can
  * run either on the same input.  Invalidates the workspace (call before sfft_plan_workspace_bytes). */
 int sfft_plan_set_corr_route(sfft_plan *plan, int route);
 
@@ -106,8 +107,10 @@ int sfft_plan_num_background_terms(const sfft_plan *plan); /* F_B */
 size_t sfft_plan_workspace_bytes(const sfft_plan *plan);
 
 /* Lend a device buffer (>= workspace_bytes, 256-byte aligned) to the plan.  The caller keeps
- * ownership and must keep it alive until the plan is destroyed or another buffer is set.  May enqueue a
- * clearing of part of the buffer on the plan's stream (set the stream first). */
+ * ownership and must keep it alive until the plan is destroyed or another buffer is set.  Enqueues a
+ * clearing of part of the buffer on the plan's stream (set the stream first), and the plan relies on the contents
+ * from then on: while the buffer is lent the caller must not write to it (lend it again with this call after using
+ * it for something else). */
 int sfft_plan_set_workspace(sfft_plan *plan, void *d_ws, size_t bytes);
 
 /* Steps a1-a5: assemble the normal system of Eq. 18 in real-space scaling,
@@ -135,7 +138,9 @@ int sfft_get_lag_table(const sfft_plan *plan, int which, const double **d_table,
  * Jacobi-scaled matrix (unit diagonal) that is not finite or falls below 64 n eps (eps = 2^-52: the level
  * at which a pivot is rounding noise of the assembled entries, i.e. the system is numerically
  * rank-deficient), raises a device flag reported by sfft_plan_status as SFFT_ERR_NOT_SPD; d_coef is then
- * undefined. */
+ * undefined.  The back substitution is a chain of CTAs that wait for one another through global memory; each takes
+ * its place in the chain from a counter when it starts running, so it only waits for CTAs that have started
+ * already and the call cannot deadlock on the order in which the grid is dispatched. */
 int sfft_solve(sfft_plan *plan, double *d_coef);
 
 /* Steps a7-a8: D = S - sum_t sum_ab k_{t,ab} R^t((x-a)%H,(y-b)%W) - sum_s b_s T'_s  (Eqs. 1, 12)

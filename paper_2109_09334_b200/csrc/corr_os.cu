@@ -65,7 +65,9 @@ __device__ __forceinline__ void fft64_group(double2 (&v)[8], Slot ex, const doub
 //   XP   : power of the x-weight f_i(x) = u_x^i, u_x = (2x+1)/H - 1 (exact in double for H a power of two, within an
 //          ulp or two otherwise; DESIGN g8).  Computed here
 //          instead of read from the plan's table: u is exact and u*u is its correctly rounded square, which is
-//          what the table holds, so both routes weight with the very same numbers (a1).
+//          what the table holds, so for H a power of two both routes weight with the very same numbers (a1).  For
+//          other H the table is rounded from long double and fma(x, 2/H, 1/H - 1) can differ from it in the last
+//          bit: the two routes then agree to rounding (1e-16 relative), not bit for bit.
 //   P2   : H is a power of two (wrap by mask); otherwise by conditional subtraction (x0 < H + 64 for every live hop)
 template <int MODE, int SIDE, int XP, bool P2>
 __device__ __forceinline__ void os_transform(const double2 *rw, double2 *dst, const double2 *tw, int t, int nkeep, int x0,

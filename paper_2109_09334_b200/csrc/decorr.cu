@@ -262,10 +262,19 @@ cudaError_t launch_decorrelate(sfft_plan *p, const double *d_coef, const double 
     double2 *twT = ahat + (size_t)nb * P / 2;
     double *sg = reinterpret_cast<double *>(twT + T), *sh = sg + (size_t)T * NH1;
     double *dG = sh + (size_t)T * NH1, *dvS = dG + (size_t)nS * LG * LG, *dH = dvS + nS, *dvR = dH + (size_t)nR * LH * LH;
-    cudaError_t e = cudaMemcpyAsync(dG, h_G, sizeof(double) * nS * LG * LG, cudaMemcpyHostToDevice, p->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dvS, h_varS, sizeof(double) * nS, cudaMemcpyHostToDevice, p->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dH, h_H, sizeof(double) * nR * LH * LH, cudaMemcpyHostToDevice, p->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dvR, h_varR, sizeof(double) * nR, cudaMemcpyHostToDevice, p->stream);
+    // The caller's tables (a few KB, laid out on the device as G, varS, H, varR back to back) are copied into a buffer
+    // the plan owns and uploaded from there: with page-locked caller arrays an asynchronous copy would still be reading
+    // them after this call has returned, and the header promises they are free again by then.  The previous call's
+    // upload may still be reading that buffer: wait for the stream before overwriting it.
+    const size_t nG = (size_t)nS * LG * LG, nH = (size_t)nR * LH * LH, ntab = nG + nS + nH + nR;
+    cudaError_t e = p->decorr_host.empty() ? cudaSuccess : cudaStreamSynchronize(p->stream);
+    if (e != cudaSuccess) return e;
+    p->decorr_host.resize(ntab);
+    std::copy(h_G, h_G + nG, p->decorr_host.begin());
+    std::copy(h_varS, h_varS + nS, p->decorr_host.begin() + nG);
+    std::copy(h_H, h_H + nH, p->decorr_host.begin() + nG + nS);
+    std::copy(h_varR, h_varR + nR, p->decorr_host.begin() + nG + nS + nH);
+    e = cudaMemcpyAsync(dG, p->decorr_host.data(), sizeof(double) * ntab, cudaMemcpyHostToDevice, p->stream);
     if (e != cudaSuccess) return e;
     e = launch_fold_coef(p, d_coef);                      // pixel kernels of Eqs. 3-4 (kfold)
     if (e != cudaSuccess) return e;

@@ -266,7 +266,7 @@ WsLayout ws_layout(const sfft_plan *p) {
     // only the subtract route the plan takes gets its table
     l.ctab = take(subtract_use_fourier(p) ? 0 : nb * (size_t)p->H * p->L * p->LT * sizeof(double));
     l.khat = take(subtract_use_fourier(p) ? nb * (size_t)p->L * p->FK * p->Nh * sizeof(double2) : 0);
-    l.flag = take(nb * sizeof(int) * 2);
+    l.flag = take((nb + 1) * sizeof(int) * 2);      // per system (first bad pivot, spare), then the back substitution's ticket
     l.total = off;
     return l;
 }
@@ -362,7 +362,8 @@ int sfft_plan_create_rect(sfft_plan **out, int H, int W, int L0, int L1, int DK,
     p->FK = (int)p->kti.size(); p->FB = (int)p->bti.size();
     p->n = p->FK * L * L + p->FB;
     p->ns = p->n;
-    // frames that are not powers of two run on the sectioned lag correlation and the direct subtract only
+    // frames that are not powers of two need the sectioned lag correlation (polynomial basis, at most 8 column
+    // sequences, DK <= 2); their subtract takes either route (chirp-z inverse rows on the Fourier route)
     if (!pow2 && (basis != SFFT_BASIS_POLY || p->FK + 1 > 8 || p->nKa > 3)) { delete p; return SFFT_ERR_INVALID_ARG; }
     p->nimg = p->nKa + 1;
     p->ldl = (p->n + 1 + 7) & ~7;
@@ -559,6 +560,9 @@ int sfft_plan_set_workspace(sfft_plan *p, void *d_ws, size_t bytes) {
     p->dscale = (double *)(b + l.dscale); p->coefr = (double *)(b + l.coefr); p->ybuf = (double *)(b + l.ybuf); p->kfold = (double *)(b + l.kfold); p->ctab = (double *)(b + l.ctab); p->khat = (double2 *)(b + l.khat); p->flag = (int *)(b + l.flag);
     p->built = p->solved = false;
     p->rhat_from_build = false;
+    if (wrong_device(p)) return SFFT_ERR_STATE;
+    // "no failure" marks: sfft_plan_status may be asked before the first build has cleared them
+    if (cudaMemsetAsync(p->flag, 0xff, sizeof(int) * 2 * p->nbatch, p->stream) != cudaSuccess) return fail_cuda(p, cudaGetLastError());
     if (!p->corr_os) {
         // the direct lag-sum kernel never writes the (S, S) pair and the lags beyond w against S, which the
         // y-direction sums read along with everything else (their results are not used): keep those entries defined

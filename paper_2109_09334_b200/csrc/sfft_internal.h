@@ -149,6 +149,7 @@ struct sfft_plan {
     int prof_steps = 0, prof_cur = -1;          // stage profiling (sfft_plan_profile)
     std::vector<cudaEvent_t> prof_events;       // [prof_steps][kProfMarks]
     std::string cuda_err;
+    std::vector<double> decorr_host;            // sfft_decorrelate's copy of the caller's host tables (source of its uploads)
 };
 
 namespace sfft {

@@ -42,8 +42,9 @@ constexpr double kPivotFloor = 64.0 * 2.220446049250313e-16;   // x n: smallest 
 __device__ __forceinline__ bool pivot_ok(double p, double pmin) { return p > pmin && p < 1e300; }
 
 __global__ void k_scale_diag(const double *__restrict__ M, double *__restrict__ dscale, int *flag, int n,
-                             unsigned long long *__restrict__ ybuf, int ny, unsigned long long sentinel) {
+                             unsigned long long *__restrict__ ybuf, int ny, unsigned long long sentinel, int *ticket) {
     int i = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (i == 0 && b == 0) *ticket = 0;                     // start-order counter of the look-back back substitution
     if (i < ny) ybuf[(size_t)b * ny + i] = sentinel;       // "not yet published" marks of the look-back back substitution
     if (i >= n) return;
     double d = M[((size_t)b * n + i) * n + i];
@@ -614,8 +615,10 @@ __global__ void __launch_bounds__(256, 2) k_chol_slab(double *__restrict__ Lf, c
 // registers over all j), then y_b = W_b^T z_b, c_b = D y_b.  The y values themselves are the flags: the buffer is
 // filled with a sentinel NaN pattern (k_scale_diag) and every consumer thread polls the 16 values it needs with
 // volatile loads, so a step of the dependent chain costs one L2 round trip, two 64 x 64 matrix-vector products
-// and three barriers instead of a cluster barrier and a round of global loads.  CTAs are ordered so that a CTA only
-// waits for CTAs with a smaller linear index (in-order dispatch): no co-residency requirement beyond one CTA.
+// and three barriers instead of a cluster barrier and a round of global loads.  A CTA takes its place in the chain
+// from a ticket drawn when it STARTS (atomicAdd on a counter zeroed by k_scale_diag), not from blockIdx: it only
+// ever waits for CTAs with a smaller ticket, which are running or done already, so progress does not depend on the
+// order in which the hardware dispatches the grid and needs no co-residency beyond one CTA.
 constexpr int kBsStages = 4;
 constexpr unsigned long long kBsSentinel = 0xFFF8DEADBEEF5AFEull;
 constexpr size_t kBsSmem = (size_t)(1 + kBsStages) * NB * NB * sizeof(double) + 128;
@@ -663,13 +666,16 @@ __device__ __forceinline__ void tma_tile_g2s(void *dst, const CUtensorMap *tm, i
 __global__ void __launch_bounds__(256)
 k_chol_backsolve_lb(const __grid_constant__ CUtensorMap tmL, const double *__restrict__ Lf, const double *__restrict__ Winv,
                     const double *__restrict__ dscale, double *__restrict__ coef, double *ybuf, int n, int ldl, int nblk,
-                    int nbat) {
+                    int nbat, int *ticket) {
     extern __shared__ double sm[];
     double *Ws = reinterpret_cast<double *>(((uintptr_t)sm + 127) & ~(uintptr_t)127);     // TMA destinations: 128-byte aligned
     double *T = Ws + NB * NB;                           // W_b [k][i]; tile ring [stage][k][col]
     __shared__ double zs[NB], red[4][NB], ysh[2][NB];
-    const int id = blockIdx.x, bz = id % nbat, x = id / nbat, blk = nblk - 1 - x;
+    __shared__ int s_ticket;
     const int tid = threadIdx.x, col = tid & 63, q = tid >> 6;
+    if (tid == 0) s_ticket = atomicAdd(ticket, 1);
+    __syncthreads();
+    const int id = s_ticket, bz = id % nbat, x = id / nbat, blk = nblk - 1 - x;
     const double *L = Lf + (size_t)bz * (n + 1) * ldl;
     double *yb = ybuf + (size_t)bz * nblk * NB;
     const int i0 = blk * NB, nbk = min(NB, n - i0);
@@ -759,7 +765,8 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
     const int n = p->ns, ldl = p->ldl, nbat = p->nbatch, nblk = solve_num_blocks(n);
     double *d_out = p->reduced ? p->coefr : d_coef;      // reduced solution first when the photometric ratio is constrained
     k_scale_diag<<<dim3((n + 255) / 256, nbat), 256, 0, p->stream>>>(p->M, p->dscale, p->flag, n,
-                                                                    (unsigned long long *)p->ybuf, nblk * NB, kBsSentinel);
+                                                                    (unsigned long long *)p->ybuf, nblk * NB, kBsSentinel,
+                                                                    p->flag + 2 * nbat);
     k_scale_copy<<<dim3((n + 127) / 128, (n + 1 + 15) / 16, nbat), 256, 0, p->stream>>>(p->M, p->rhs, p->dscale, p->Lf, n, ldl);
     p->launches += 2;
     cudaError_t e = cudaFuncSetAttribute(k_chol_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kStepSmem);
@@ -816,7 +823,7 @@ cudaError_t launch_solve(sfft_plan *p, double *d_coef) {
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorInvalidValue;
     k_chol_backsolve_lb<<<dim3(nblk * nbat), 256, kBsSmem, p->stream>>>(tmL, p->Lf, p->Winv, p->dscale, d_out, p->ybuf, n, ldl,
-                                                                       nblk, nbat);
+                                                                       nblk, nbat, p->flag + 2 * nbat);
     p->launches++;
     e = cudaGetLastError();
     if (e == cudaSuccess && p->reduced) e = launch_expand_coef(p, p->coefr, d_coef);

@@ -477,7 +477,6 @@ cudaError_t launch_subtract_fourier(sfft_plan *p, const double *d_coef, const do
     if (e != cudaSuccess) return e;
     switch (p->bsM) {
         case 0: break;
-        case 1024: return launch_inv_bs<1024>(p, d_coef, dS, dD);
         case 2048: return launch_inv_bs<2048>(p, d_coef, dS, dD);
         case 4096: return launch_inv_bs<4096>(p, d_coef, dS, dD);
         default: return cudaErrorInvalidValue;
