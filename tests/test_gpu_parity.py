@@ -40,12 +40,12 @@ def _check_coef(c, co, na):
     assert np.max(np.abs(c[na:] - co[na:])) <= TOL_C * np.max(np.abs(co[na:]))
 
 
-def _gpu_all(torch, p, L, basis, DK, DB, R=None, S=None, corr_route=0):
+def _gpu_all(torch, p, L, basis, DK, DB, R=None, S=None, corr_route=0, reuse_spectra=False):
     R = p.R if R is None else R
     S = p.S if S is None else S
     nb = 1 if R.ndim == 2 else R.shape[0]
     H, W = R.shape[-2:]
-    plan = B.Plan(H, W, L, DK, DB, basis, nbatch=nb, corr_route=corr_route)
+    plan = B.Plan(H, W, L, DK, DB, basis, nbatch=nb, corr_route=corr_route, reuse_spectra=reuse_spectra)
     dR, dS = torch.from_numpy(np.ascontiguousarray(R)).cuda(), torch.from_numpy(np.ascontiguousarray(S)).cuda()
     plan.build_system(dR, dS)
     coef = plan.solve()
@@ -78,6 +78,12 @@ CASES = [
     (2, 128, 256, 27, None, 1, 0),                    # L = 27: direct subtract with 27 taps
     (5, 128, 128, 5, "bspline", 1, 0),                # B-spline weights
     (5, 256, 256, 5, "bspline", 4, 4),                # config-5 basis (8x8 functions), n = 1664
+    # the edges of what sfft_plan_create accepts (DK, DB <= 8, H <= 8192)
+    (2, 64, 128, 5, "poly", 4, 4),                    # 15 kernel terms: 16 column sequences on the direct lag sums
+    (2, 64, 128, 3, "poly", 8, 8),                    # highest polynomial degree: 45 terms, 17 row moments per image
+    (2, 128, 128, 3, "poly", 6, 6),                   # 13 row moments per image
+    (5, 128, 128, 3, "bspline", 8, 8),                # most B-spline knots: 12 x 12 = 144 kernel terms, n = 1440
+    (2, 8192, 64, 5, "poly", 1, 1),                   # tallest frame (H = 8192)
 ]
 
 
@@ -148,43 +154,38 @@ def test_parity_config2_full(cuda_device):
     assert np.max(np.abs(D - Do)) <= TOL_D * p.sigma
 
 
-@pytest.mark.slow
-@pytest.mark.parametrize("cfg", [3, 4])
-def test_parity_full_size(cuda_device, cfg):
-    """Configs 3 and 4 at BASELINE.json's full size, in the launch configuration bench.py times.
-    The oracle's full direct-sum system takes about a minute or two of host time per config."""
-    import torch
-    p = synth.make_pair(cfg)
+def _full_frame_both_modes(torch, p):
+    """Full-size check shared by configs 3, 4 and the CCD frame: the oracle's full normal system, solution and FULL
+    difference image (every pixel) against the CUDA path in both subtract modes -- the default, which transforms
+    the reference again, and reuse_spectra=True, the launch configuration bench.py times (fit and apply on the same
+    pair, the build's row spectra reused)."""
     bid = oracle.POLY
     Mo, ro = oracle.normal_from_lags(p.R, p.S, p.L, bid, p.DK, p.DB)
     co = oracle.solve(Mo, ro)
-    M, rhs, c, D = _gpu_all(torch, p, p.L, p.basis, p.DK, p.DB)
-    _check_system(M[0], rhs[0], Mo, ro, p.S)
-    _check_coef(c[0], co, 6 * p.L * p.L)
-    rng = np.random.default_rng(cfg)
-    px = np.r_[rng.integers(0, p.H, 4000), [0, 0, p.H - 1, p.H - 1, 3, p.H - 2]]       # random + corners/borders
-    py = np.r_[rng.integers(0, p.W, 4000), [0, p.W - 1, 0, p.W - 1, p.W - 4, 5]]
-    Dref = oracle.difference_at(p.R, p.S, co, p.L, bid, p.DK, p.DB, px, py)
-    assert np.max(np.abs(D[px, py] - Dref)) <= TOL_D * p.sigma
+    Do = oracle.difference(p.R, p.S, co, p.L, bid, p.DK, p.DB)
+    for reuse in (False, True):
+        M, rhs, c, D = _gpu_all(torch, p, p.L, p.basis, p.DK, p.DB, reuse_spectra=reuse)
+        _check_system(M[0], rhs[0], Mo, ro, p.S)
+        _check_coef(c[0], co, 6 * p.L * p.L)
+        assert D.shape == Do.shape and np.max(np.abs(D - Do)) <= TOL_D * p.sigma, f"reuse_spectra={reuse}"
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_parity_full_size(cuda_device, cfg):
+    """Configs 3 and 4 at BASELINE.json's full size: M, rhs, c and every pixel of D, in the default mode and in the
+    launch configuration bench.py times (reuse_spectra=True).  The oracle's full direct-sum system takes about a
+    minute or two of host time per config, its full difference image a few seconds."""
+    import torch
+    _full_frame_both_modes(torch, synth.make_pair(cfg))
 
 
 @pytest.mark.slow
 def test_parity_decam_ccd_frame_2046x4094(cuda_device):
     """NEXT-4 at the true DECam CCD size (2046 x 4094 = 2*3*11*31 x 2*23*89), config-3 recipe and model
-    (15 x 15 delta basis, DK = DB = 2, n = 1356): full M / rhs / c element-wise, D at 4 006 sampled pixels."""
+    (15 x 15 delta basis, DK = DB = 2, n = 1356): full M / rhs / c element-wise, D on every pixel, both subtract modes."""
     import torch
-    p = synth.make_pair(3, H=2046, W=4094)
-    bid = oracle.POLY
-    Mo, ro = oracle.normal_from_lags(p.R, p.S, p.L, bid, p.DK, p.DB)
-    co = oracle.solve(Mo, ro)
-    M, rhs, c, D = _gpu_all(torch, p, p.L, p.basis, p.DK, p.DB)
-    _check_system(M[0], rhs[0], Mo, ro, p.S)
-    _check_coef(c[0], co, 6 * p.L * p.L)
-    rng = np.random.default_rng(2046)
-    px = np.r_[rng.integers(0, p.H, 4000), [0, 0, p.H - 1, p.H - 1, 3, p.H - 2]]
-    py = np.r_[rng.integers(0, p.W, 4000), [0, p.W - 1, 0, p.W - 1, p.W - 4, 5]]
-    Dref = oracle.difference_at(p.R, p.S, co, p.L, bid, p.DK, p.DB, px, py)
-    assert np.max(np.abs(D[px, py] - Dref)) <= TOL_D * p.sigma
+    _full_frame_both_modes(torch, synth.make_pair(3, H=2046, W=4094))
 
 
 @pytest.mark.slow
@@ -642,6 +643,32 @@ def test_decorrelation_parity(cuda_device, cfg, H, W, L, DK, tile, coadd):
     for bad_tile in (48, 16, 1024):
         assert B.sfft_decorrelate(plan.h, coef.data_ptr(), D.data_ptr(), D2.data_ptr(), bad_tile, var_S, G, var_R, Hk) == B.SFFT_ERR_INVALID_ARG
     assert B.sfft_decorrelate(plan.h, coef.data_ptr(), D.data_ptr(), D2.data_ptr(), tile, var_S, np.ones((len(var_S), 2, 2)), var_R, Hk) == B.SFFT_ERR_INVALID_ARG
+    plan.close()
+
+
+@pytest.mark.parametrize("cfg,H,W,L,DK,tile", [(1, 128, 128, 7, 1, 32), (2, 256, 512, 9, 2, 128)])
+def test_decorrelation_chained_from_the_oracle_fit(cuda_device, cfg, H, W, L, DK, tile):
+    """The whole chain on each side, nothing handed across: oracle fit -> oracle D -> oracle decorrelation against
+    GPU build -> solve -> subtract -> sfft_decorrelate.  Tolerance: the decorrelated image is D convolved with a
+    unit-sum kernel Q whose taps depend smoothly on the fitted kernel, so the 1e-6 sigma allowed on D and the 1e-8
+    relative allowed on the coefficients carry through with a factor sum|Q| of order one: 4e-6 sigma."""
+    import torch
+    from oracle import decorr
+    p = synth.make_pair(cfg, H=H, W=W)
+    DB = 1
+    _, _, co, Do = _oracle_all(p.R, p.S, L, "poly", DK, DB)
+    g = np.array([[0.0, 0.1, 0.0], [0.1, 0.6, 0.1], [0.0, 0.1, 0.0]])
+    var_S, G, var_R, Hk = [120.0, 130.0], np.stack([g / 2, np.roll(g, 1, axis=1) / 2]), [125.0], np.ones((1, 1, 1))
+    ref = decorr.decorrelate(Do, co, L, oracle.POLY, DK, tile, var_S, G, var_R, Hk)
+    plan = B.Plan(H, W, L, DK, DB, "poly")
+    dR, dS = torch.from_numpy(p.R).cuda(), torch.from_numpy(p.S).cuda()
+    plan.build_system(dR, dS)
+    coef = plan.solve()
+    D = plan.subtract(coef, dR, dS)
+    Ddc = plan.decorrelate(coef, D, tile, var_S, G, var_R, Hk)
+    plan.status()
+    assert np.max(np.abs(ref - Do)) > 1e-3 * p.sigma
+    assert np.max(np.abs(Ddc.cpu().numpy().reshape(H, W) - ref)) <= 4 * TOL_D * p.sigma
     plan.close()
 
 
