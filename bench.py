@@ -41,8 +41,26 @@ NCU_TRAFFIC_SOURCE = {"rowfft": _R02C, "subtract": _R02B + " (k_fir_x)", "corr":
 REFERENCE_BUDGET_S = 200.0      # wall-clock cap of the --impl reference arm (the oracle is slow by construction)
 
 
+# BASELINE.json's five configs plus the paper's own CCD frame (DECam, 2046 x 4094 pixels, neither a
+# power of two), rendered with the config-3 recipe and fitted with the config-3 model: `--config decam` (or 6).
+DECAM = 6
+CONFIGS = dict(synth.CONFIGS)
+CONFIGS[DECAM] = dict(synth.CONFIGS[3], H=2046, W=4094, recipe=3)
+
+
+def make_bench_pair(cfg_index, **kw):
+    c = CONFIGS[cfg_index]
+    if "recipe" in c:
+        return synth.make_pair(c["recipe"], H=c["H"], W=c["W"], **kw)
+    return synth.make_pair(cfg_index, **kw)
+
+
+def parse_config(text):
+    return DECAM if str(text).lower() == "decam" else int(text)
+
+
 def metric_name(cfg_index):
-    c = synth.CONFIGS[cfg_index]
+    c = CONFIGS[cfg_index]
     size = f"{c['H']}x{c['W']}" if c["H"] != c["W"] else f"{c['H']}^2"
     what = "difference-image pairs/s" if c["batch"] == 1 else f"sub-field pairs/s (batch of {c['batch']} per call)"
     return f"{what} at {size} FP64 (build+solve+subtract, L={c['L']}, {c['basis']} DK={c['DK']} DB={c['DB']})"
@@ -58,7 +76,7 @@ def shard_units(nunits, rank, world):
 def rank_units(cfg_index, rank, world):
     """Units (pairs / sub-fields) rank `rank` of `world` processes per step, as (first, count, scaling):
     a single-pair config gives every rank its own pair (weak); the config-5 batch is sliced (strong)."""
-    nb = synth.CONFIGS[cfg_index]["batch"]
+    nb = CONFIGS[cfg_index]["batch"]
     if nb == 1:
         return rank, 1, "weak"
     lo, hi = shard_units(nb, rank, world)
@@ -70,7 +88,7 @@ L2_BYTES = 126e6
 
 def step_footprint_bytes(cfg_index, nb=None):
     """Bytes one step touches at least: the images R, S, D and the row-spectrum stack (nKa + 1 half spectra)."""
-    c = synth.CONFIGS[cfg_index]
+    c = CONFIGS[cfg_index]
     nb = c["batch"] if nb is None else nb
     nKa = c["DK"] + 1 if c["basis"] == "poly" else c["DK"] + 4
     return nb * c["H"] * c["W"] * 8.0 * (3 + nKa + 1)
@@ -82,7 +100,7 @@ def needs_l2_flush(cfg_index, nb=None):
 
 def config_dict(cfg_index):
     """The `config` object of the JSON line: the same for both arms (it names the workload and the timing protocol)."""
-    c = synth.CONFIGS[cfg_index]
+    c = CONFIGS[cfg_index]
     fp = step_footprint_bytes(cfg_index)
     l2 = ("L2 flushed between timed steps (a 256 MB device buffer is overwritten; each step is timed by its own pair of "
           "CUDA events)" if needs_l2_flush(cfg_index)
@@ -94,15 +112,16 @@ def config_dict(cfg_index):
 
 
 def workload_name(cfg_index):
-    c = synth.CONFIGS[cfg_index]
-    return (f"config{cfg_index}: {c['H']}x{c['W']} FP64 pair, {c['L']}x{c['L']} delta-basis, "
+    c = CONFIGS[cfg_index]
+    name = "DECam CCD frame (PAPER.md:393), config-3 recipe and model" if cfg_index == DECAM else f"config{cfg_index}"
+    return (f"{name}: {c['H']}x{c['W']} FP64 pair, {c['L']}x{c['L']} delta-basis, "
             f"{c['basis']} DK={c['DK']} DB={c['DB']}" + (f", batch {c['batch']}" if c["batch"] > 1 else ""))
 
 
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
-    def __init__(self, index=0, period=0.02):
+    def __init__(self, index=0, period=0.002):
         super().__init__(daemon=True)
         self.index, self.period, self.stop_flag = index, period, False
         self.sm, self.reasons, self.sm_max, self.ok = [], set(), None, False
@@ -158,7 +177,7 @@ def oracle_pass(cfg_index, pair, crop=None):
     batch-of-64 config, whose full oracle pass takes hours).  Returns (seconds per unit of the workload,
     description, cores)."""
     import oracle
-    c = synth.CONFIGS[cfg_index]
+    c = CONFIGS[cfg_index]
     bid = oracle.POLY if c["basis"] == "poly" else oracle.BSPLINE
     R = pair.R if pair.R.ndim == 2 else pair.R[0]
     S = pair.S if pair.S.ndim == 2 else pair.S[0]
@@ -190,7 +209,7 @@ def oracle_pass(cfg_index, pair, crop=None):
 
 
 def oracle_crop_for(cfg_index):
-    return None if synth.CONFIGS[cfg_index]["batch"] == 1 else 256
+    return None if CONFIGS[cfg_index]["batch"] == 1 else 256
 
 
 def run_reference(args):
@@ -201,8 +220,8 @@ def run_reference(args):
     if rank != 0:
         return
     cfg = args.config
-    single = synth.CONFIGS[cfg]["batch"] == 1
-    pair = synth.make_pair(cfg) if single else synth.make_pair(cfg, subfield=0)
+    single = CONFIGS[cfg]["batch"] == 1
+    pair = make_bench_pair(cfg) if single else synth.make_pair(cfg, subfield=0)
     crop = args.ref_crop if args.ref_crop > 0 else oracle_crop_for(cfg)
     t_begin = time.perf_counter()
     times, warm_done = [], 0
@@ -310,7 +329,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--config", type=parse_config, default=4, help="1..5 (BASELINE.json configs), or decam (2046x4094)")
     ap.add_argument("--ref-crop", type=int, default=0, help="time the oracle on a crop (0: full pair; config 5: 256)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-pipelined", action="store_true")
@@ -336,13 +355,13 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     cfg = args.config
-    c = synth.CONFIGS[cfg]
+    c = CONFIGS[cfg]
     first, nb, scaling = rank_units(cfg, rank, world)
     total_units = world if c["batch"] == 1 else c["batch"]
     if nb < 1:
         raise SystemExit(f"bench.py: rank {rank} of {world} has no unit of config {cfg}")
     if c["batch"] == 1:
-        pair = synth.make_pair(cfg)
+        pair = make_bench_pair(cfg)
     else:
         pair = synth.make_batch(cfg, nbatch=nb, first=first, workers=min(16, os.cpu_count() or 1))
     # fit and apply on the same pair: the subtract may reuse the build's row spectra (explicit opt-in)
@@ -479,6 +498,70 @@ def main():
         pipelined = {"pairs_in_flight": 2, "value": world * 2 * nb / float(tp.item()), "unit": "pairs/s",
                      "note": "two plans on two streams, wall clock around K double steps; not the headline value"}
 
+    def time_steps(fn, steps, warm=3):
+        """ms per call of fn over `steps` back-to-back calls, CUDA events on the current stream, after `warm` calls."""
+        for _ in range(warm):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        a.record()
+        for _ in range(steps):
+            fn()
+        b.record()
+        torch.cuda.synchronize(dev)
+        return a.elapsed_time(b) / steps
+
+    # ---- the paper's two-step flow (PAPER.md:218, 222), beside the headline and never instead of it: mask the
+    # saturated sources and fill them with the local background, fit on the masked pair, apply to the ORIGINAL pair.
+    # The subtract cannot reuse the build's spectra here (they are the masked reference's): reuse_spectra = False ----
+    masked_flow = None
+    if world == 1 and c["batch"] == 1 and not args.no_pipelined:
+        sat = 3000.0
+        planm = B.Plan(c["H"], c["W"], c["L"], c["DK"], c["DB"], c["basis"], nbatch=1, device=dev, reuse_spectra=False)
+        dRm, dSm = torch.empty_like(dR), torch.empty_like(dS)
+        dmask = torch.empty(dR.shape, dtype=torch.uint8, device=dev)
+
+        def masked_step():
+            st = B.sfft_mask_fill(planm.h, dR.data_ptr(), dS.data_ptr(), sat, sat, 2, 6, dRm.data_ptr(), dSm.data_ptr(),
+                                  dmask.data_ptr())
+            if st != B.SFFT_OK:
+                raise B.SfftError(st, "sfft_mask_fill")
+            planm.build_system(dRm, dSm)
+            planm.solve(coef)
+            planm.subtract(coef, dR, dS, dD)
+
+        mms = time_steps(masked_step, args.steps)
+        planm.status()
+        masked_flow = {"ms_per_step": mms, "value": 1.0 / (mms * 1e-3), "unit": "pairs/s",
+                       "masked_pixels": int(dmask.sum().item()), "saturation_adu": sat, "grow_px": 2, "fill_half_window_px": 6,
+                       "api": "sfft_mask_fill -> sfft_build_system(masked pair) -> sfft_solve -> sfft_subtract(original "
+                              "pair), reuse_spectra = 0 (the reference is transformed again)"}
+        planm.close()
+        del dRm, dSm, dmask
+
+    # ---- several pairs per call through the batch axis (single-pair configs): the dependent panel chain of the
+    # solve is shared by the batch.  Entries are circular shifts of the pair (the model is circular: same fit) ----
+    batched = None
+    if world == 1 and c["batch"] == 1 and not args.no_pipelined:
+        batched = {}
+        for nbat in (2, 4):
+            planb = B.Plan(c["H"], c["W"], c["L"], c["DK"], c["DB"], c["basis"], nbatch=nbat, device=dev, reuse_spectra=True)
+            bR = torch.stack([torch.roll(dR, shifts=(17 * e, 29 * e), dims=(0, 1)) for e in range(nbat)]).contiguous()
+            bS = torch.stack([torch.roll(dS, shifts=(17 * e, 29 * e), dims=(0, 1)) for e in range(nbat)]).contiguous()
+            bD, bC = torch.empty_like(bS), torch.empty((nbat, planb.n), dtype=torch.float64, device=dev)
+
+            def batch_step():
+                planb.build_system(bR, bS)
+                planb.solve(bC)
+                planb.subtract(bC, bR, bS, bD)
+
+            bms = time_steps(batch_step, max(3, args.steps // 2))
+            planb.status()
+            batched[f"nbatch{nbat}"] = {"ms_per_call": bms, "value": nbat / (bms * 1e-3), "unit": "pairs/s"}
+            planb.close()
+            del bR, bS, bD, bC
+        batched["note"] = "one plan, nbatch pairs per build/solve/subtract call; not the headline value"
+
     # ---- end to end through sfft_run_host: pinned host buffers, H2D + D2H inside the timed region ----
     hR = torch.from_numpy(np.ascontiguousarray(pair.R)).pin_memory()
     hS = torch.from_numpy(np.ascontiguousarray(pair.S)).pin_memory()
@@ -552,7 +635,7 @@ def main():
             pass
         names = B.STAGE_NAMES
         stages = {names[i]: round(float(stage_ms[i]), 4) for i in range(len(names))}
-        top = int(np.argmax(stage_ms))
+        top = int(np.argmax(stage_ms[:8]))          # (entries 8, 9 are the two halves of stage 7)
         # algorithmic work of each stage per pair; P pixels, FP64
         P = c["H"] * c["W"]
         nKa = (c["DK"] + 1) if c["basis"] == "poly" else (c["DK"] + 4)
@@ -571,6 +654,8 @@ def main():
             # subtract: SURVEY 8(d) Fourier-route figure, L*FK complex MACs per spectrum point (8 flop each)
             "subtract": ("alu", 8.0 * L * FK * c["H"] * (c["W"] // 2) * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
             "solve": ("alu", (plan.ns ** 3 / 3.0) * nb / 1e12, FP64_PEAK_TFLOPS, "TFLOP/s"),
+            # inverse row transforms fused with the difference: read the filtered half spectrum and S, write D
+            "subtract_inverse": ("hbm", 3 * P * 8.0 * nb / 1e9, hbm_peak, "GB/s"),
         }
         tname = names[top]
         bound, work, peak, unit = alg.get(tname, ("hbm", 0.0, hbm_peak, "GB/s"))
@@ -616,7 +701,7 @@ def main():
             "clocks": clocks,
             "roofline": roofline,
             "stage_roofline": rf_all,
-            "pipelined": pipelined, "cuda_graph": graph_info,
+            "pipelined": pipelined, "cuda_graph": graph_info, "masked_flow": masked_flow, "batched": batched,
             "stage_ms": stages,
         }
         if not args.no_compare and world == 1:

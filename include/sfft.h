@@ -259,8 +259,10 @@ int sfft_run_host_async_f32(sfft_plan *plan, const float *h_R, const float *h_S,
  * ms[step][SFFT_NUM_STAGES] (row-major; -1 where a stage did not run) for the *nrecorded steps seen.
  * Stage order: 0 row FFT (a1+a2), 1 x-direction lag correlation on the FP64 tensor cores (a3+a4), 2 y-direction
  * pruned inverse DFT to the lag tables (a4), 3 basis-function moments Lambda/Delta (a4'), 4 lag gather (a5),
- * 5 solve (a6), 6 kernel folding + per-row coefficient table (a7), 7 convolve-and-subtract (a7+a8). */
-#define SFFT_NUM_STAGES 8
+ * 5 solve (a6), 6 kernel folding + per-row coefficient table (a7), 7 convolve-and-subtract (a7+a8), and the two parts
+ * of stage 7 when the subtract takes the Fourier route (-1 on the direct route): 8 FIR along x on the row spectra,
+ * 9 inverse row transforms fused with the difference. */
+#define SFFT_NUM_STAGES 10
 int sfft_plan_profile(sfft_plan *plan, int nsteps);
 int sfft_plan_profile_read(sfft_plan *plan, double *ms, int *nrecorded);
 

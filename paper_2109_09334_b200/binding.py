@@ -24,8 +24,9 @@ EXPORTS = [
     "sfft_run_host", "sfft_run_host_async", "sfft_run_host_wait", "sfft_run_host_f32", "sfft_run_host_async_f32", "sfft_plan_launch_count", "sfft_plan_destroy",
     "sfft_strerror", "sfft_last_cuda_error", "sfft_version", "sfft_plan_profile", "sfft_plan_profile_read",
 ]
-SFFT_NUM_STAGES = 8
-STAGE_NAMES = ["rowfft", "corr", "lagsum", "moments", "gather", "solve", "subtract_prep", "subtract"]
+SFFT_NUM_STAGES = 10
+STAGE_NAMES = ["rowfft", "corr", "lagsum", "moments", "gather", "solve", "subtract_prep", "subtract", "subtract_fir",
+               "subtract_inverse"]
 
 _lib = None
 

@@ -656,8 +656,9 @@ int sfft_plan_profile_read(sfft_plan *p, double *ms, int *nrecorded) {
     if (e != cudaSuccess) return fail_cuda(p, e);
     int nrec = std::min(p->prof_cur + 1, p->prof_steps);
     if (nrecorded) *nrecorded = nrec;
-    // stages: 0 rowfft, 1 corr, 2 lagsum, 3 moments, 4 gather, 5 solve, 6 subtract-prep, 7 subtract
-    static const int from[SFFT_NUM_STAGES] = {0, 1, 2, 3, 4, 6, 8, 9}, to[SFFT_NUM_STAGES] = {1, 2, 3, 4, 5, 7, 9, 10};
+    // stages: 0 rowfft, 1 corr, 2 lagsum, 3 moments, 4 gather, 5 solve, 6 subtract-prep, 7 subtract, and the two halves
+    // of 7 on the Fourier route (mark 11 lies between them; never recorded on the direct route): 8 FIR, 9 inverse rows
+    static const int from[SFFT_NUM_STAGES] = {0, 1, 2, 3, 4, 6, 8, 9, 9, 11}, to[SFFT_NUM_STAGES] = {1, 2, 3, 4, 5, 7, 9, 10, 11, 10};
     for (int s = 0; s < nrec; ++s)
         for (int g = 0; g < SFFT_NUM_STAGES; ++g) {
             float t = 0.f;

@@ -26,7 +26,7 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
 }
 #endif
 
-constexpr int kProfMarks = 11;     // event marks per profiled step (see sfft_plan_profile_read)
+constexpr int kProfMarks = 12;     // event marks per profiled step (see sfft_plan_profile_read)
 constexpr int kCorrCols = 2;       // spectrum columns (m) per CTA of the correlation kernel
 constexpr int kCorrNSlots = 8;     // N-side (shifted) sequence planes per correlation job: slots 0..7
 constexpr int kCorrZero = 8;       // slot of the all-zero plane (absent M-side rows, absent lag-0 columns)

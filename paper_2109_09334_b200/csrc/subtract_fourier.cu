@@ -475,6 +475,7 @@ cudaError_t launch_subtract_fourier(sfft_plan *p, const double *d_coef, const do
         default: return cudaErrorInvalidValue;
     }
     if (e != cudaSuccess) return e;
+    prof_mark(p, 11);       // FIR done, inverse row transforms next
     switch (p->bsM) {
         case 0: break;
         case 2048: return launch_inv_bs<2048>(p, d_coef, dS, dD);

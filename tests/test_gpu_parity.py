@@ -861,3 +861,28 @@ def test_argument_and_state_errors(cuda_device):
     assert B.sfft_run_host_async(h2, x.data_ptr(), x.data_ptr(), 0, 0) == B.SFFT_ERR_WORKSPACE
     B.sfft_plan_destroy(h2)
     B.sfft_plan_destroy(h)
+
+
+def test_stage_profile_splits_the_fourier_route_subtract(cuda_device):
+    """sfft_plan_profile / sfft_plan_profile_read: every stage of a step gets a time; on the Fourier-route subtract
+    stage 7 is the sum of its two parts (8 FIR along x, 9 inverse rows + difference), on the direct route the two
+    parts read -1."""
+    import torch
+    for (H, W, L, fourier) in [(64, 1024, 9, True), (128, 128, 7, False)]:
+        p = synth.make_pair(2, H=H, W=W)
+        plan = B.Plan(H, W, L, 1, 1, "poly")
+        dR, dS = torch.from_numpy(p.R).cuda(), torch.from_numpy(p.S).cuda()
+        plan.profile(2)
+        for _ in range(2):
+            plan.build_system(dR, dS)
+            coef = plan.solve()
+            plan.subtract(coef, dR, dS)
+        ms = plan.profile_read(2)
+        plan.status()
+        assert ms.shape == (2, B.SFFT_NUM_STAGES) and len(B.STAGE_NAMES) == B.SFFT_NUM_STAGES
+        assert np.all(ms[:, :8] > 0.0)
+        if fourier:
+            assert np.all(ms[:, 8:] > 0.0) and np.allclose(ms[:, 8] + ms[:, 9], ms[:, 7], rtol=0.05, atol=2e-3)
+        else:
+            assert np.all(ms[:, 8:] == -1.0)
+        plan.close()
