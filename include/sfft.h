@@ -179,20 +179,22 @@ int sfft_mask_fill(sfft_plan *plan, const double *d_R, const double *d_S, double
  * fails, or falls outside the pool's accounting), and a loop that must never stall (cudaMalloc and cudaFree
  * synchronise the whole device).  sfft_plan_create uploads tables into memory it allocates and sfft_mask_fill wants a
  * lent workspace, so neither serves such a caller; this call takes the five images and nothing else.
- *   Its scratch (row-grown seed flags, one byte per pixel, plus 8 KiB of partial sums) lives in an array that is part
- *   of the library image: SFFT_STATIC_MAX_PIXELS + 8192 bytes (16 MiB + 8 KiB) of device memory on EVERY GPU on which
+ *   Its scratch (row-grown seed flags, one byte per pixel, plus 32 KiB of partial sums) lives in an array that is part
+ *   of the library image: SFFT_STATIC_MAX_PIXELS + 32768 bytes (16 MiB + 32 KiB) of device memory on EVERY GPU on which
  *   the process uses this library, held from the moment the library's device code is loaded there until the process
  *   exits, whether or not this call is ever made.
  *   Limits: 1 <= H, W <= 16384 and H*W <= SFFT_STATIC_MAX_PIXELS (4096 x 4096, which covers the 2046 x 4094 CCD
  *   frame); anything larger is refused with SFFT_ERR_INVALID_ARG and a message naming the limit
  *   (sfft_static_last_error).  rd, rb, sat_*, the pointer roles, aliasing and layout are those of sfft_mask_fill,
- *   and so is the result, bit for bit (the same kernels run).  Any H and W are accepted (indices wrap by modulo).
+ *   and so is the result, bit for bit (the same kernels run).  Any H and W are accepted (indices wrap by modulo);
+ *   with W even and the four images 16-byte aligned (the mask 2-byte aligned) the faster two-pixels-per-thread kernels
+ *   run, otherwise one-pixel-per-thread forms of them (same mask; the global-mean fallback may differ in its last bit).
  *   Set-up: the first call on each device looks up the device address of the scratch array (once per device, cached;
  *   the device that is current at the call is the one used, and d_* and cuda_stream must belong to it).  That
  *   look-up may make the CUDA runtime load the library's device code, so issue the first call on a device ahead of
  *   any stream capture and ahead of the section that must not stall.
  *   Sharing: every call on a device uses the same scratch, and the scratch keeps the previous call's contents.
- *   Nothing in it has to start at zero: each call writes every entry it later reads (H*W flags, 768 partial sums,
+ *   Nothing in it has to start at zero: each call writes every entry it later reads (H*W flags, 3552 partial sums,
  *   2 means) before reading it, so no clearing pass is run.  Two calls that can overlap on the GPU (different
  *   streams, or different host threads without ordering) race on it and both results are garbage: order them on one
  *   stream or with events.

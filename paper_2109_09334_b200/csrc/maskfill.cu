@@ -13,22 +13,173 @@
 namespace sfft {
 namespace {
 
-// t(x,y) = OR_{|dy| <= rd} seed(x, (y+dy) mod W)
-__global__ void k_mask_rows(const double *__restrict__ R, const double *__restrict__ S, unsigned char *__restrict__ t,
-                            int H, int W, int rd, double satR, double satS) {
-    const int y = blockIdx.x * blockDim.x + threadIdx.x, x = blockIdx.y, b = blockIdx.z;
-    if (y >= W) return;
+constexpr int kMfBlocks = 1184;      // CTAs of the unmasked-sum kernel (8 per SM); fixed, so the sums are reproducible
+
+// t(x,y) = OR_{|dy| <= rd} seed(x, (y+dy) mod W).  A thread owns 4 consecutive pixels of a row and slides along it,
+// keeping the distance to the last seed seen: 4 + 2 rd loads per image instead of 4 (2 rd + 1).
+__global__ void __launch_bounds__(256) k_mask_rows(const double *__restrict__ R, const double *__restrict__ S,
+                                                   unsigned char *__restrict__ t, int H, int W, int rd, double satR, double satS) {
+    const int y0 = 4 * (blockIdx.x * blockDim.x + threadIdx.x), x = blockIdx.y, b = blockIdx.z;
+    if (y0 >= W) return;
     const size_t row = ((size_t)b * H + x) * W;
-    int m = 0;
-    for (int dy = -rd; dy <= rd; ++dy) {
-        const int yy = wrap_index(y + dy, W, (W & (W - 1)) == 0 ? W - 1 : -1);
-        m |= (__ldg(&R[row + yy]) >= satR) | (__ldg(&S[row + yy]) >= satS);
+    const int wm = (W & (W - 1)) == 0 ? W - 1 : -1;
+    int since = 1 << 20;                                  // pixels since the last seed
+    for (int i = -rd; i < 4 + rd; ++i) {
+        const int yy = wrap_index(y0 + i, W, wm);
+        const bool seed = (__ldg(&R[row + yy]) >= satR) | (__ldg(&S[row + yy]) >= satS);
+        since = seed ? 0 : since + 1;
+        const int yc = y0 + i - rd;                       // its window [yc - rd, yc + rd] ends at the pixel just read
+        if (i >= rd && yc < W) t[row + yc] = (unsigned char)(since <= 2 * rd);
     }
-    t[row + y] = (unsigned char)m;
 }
 
+// mask(x,y) = OR_{|dx| <= rd} t((x+dx) mod H, y).  A thread owns two adjacent columns (one 16-bit word: W is even,
+// so every row starts on an even byte) and 16 consecutive rows, sliding down: 16 + 2 rd loads for 32 pixels.
+constexpr int kMfColRows = 16;
+__global__ void __launch_bounds__(128) k_mask_cols(const unsigned char *__restrict__ t, unsigned char *__restrict__ mask,
+                                                   int H, int W, int rd) {
+    const int yp = blockIdx.x * blockDim.x + threadIdx.x, x0 = blockIdx.y * kMfColRows, b = blockIdx.z;
+    if (2 * yp >= W) return;
+    const int hm = (H & (H - 1)) == 0 ? H - 1 : -1, W2 = W / 2;
+    const unsigned short *t2 = reinterpret_cast<const unsigned short *>(t) + (size_t)b * H * W2;
+    unsigned short *m2 = reinterpret_cast<unsigned short *>(mask) + (size_t)b * H * W2;
+    int since0 = 1 << 20, since1 = 1 << 20;               // rows since byte 0 / byte 1 of the pair was last set
+    for (int i = -rd; i < kMfColRows + rd; ++i) {
+        const int xx = x0 + i;
+        const unsigned short v = t2[(size_t)wrap_index(xx, H, hm) * W2 + yp];
+        since0 = (v & 0x00ff) ? 0 : since0 + 1;
+        since1 = (v & 0xff00) ? 0 : since1 + 1;
+        // row xc = xx - rd has its whole window [xc - rd, xc + rd] = [xx - 2 rd, xx] loaded once i >= rd
+        const int xc = xx - rd;
+        if (i >= rd && xc < H) {
+            const unsigned short o = (unsigned short)((since0 <= 2 * rd ? 1 : 0) | (since1 <= 2 * rd ? 0x100 : 0));
+            m2[(size_t)xc * W2 + yp] = o;
+        }
+    }
+}
+
+// partial sums of the unmasked pixels: part[b][blk] = (sum R, sum S, count), fixed order (deterministic).  Two pixels
+// per thread and step (P is even), loads issued whether or not the pixel is masked so that several are in flight.
+__global__ void __launch_bounds__(256) k_unmasked_partial(const double *__restrict__ R, const double *__restrict__ S,
+                                                          const unsigned char *__restrict__ mask, double *__restrict__ part,
+                                                          size_t P, int nblk) {
+    const int b = blockIdx.y, tid = threadIdx.x;
+    const size_t P2 = P / 2, chunk = (P2 + nblk - 1) / nblk, lo = (size_t)blockIdx.x * chunk, hi = lo + chunk < P2 ? lo + chunk : P2;
+    const double2 *R2 = reinterpret_cast<const double2 *>(R + (size_t)b * P), *S2 = reinterpret_cast<const double2 *>(S + (size_t)b * P);
+    const unsigned short *M2 = reinterpret_cast<const unsigned short *>(mask + (size_t)b * P);
+    double sr = 0.0, ss = 0.0;
+    int cnt = 0;
+    for (size_t i = lo + tid; i < hi; i += 4 * 256) {
+        double2 r[4], s[4];
+        unsigned short m[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const size_t q = i + 256 * u;
+            m[u] = 0x0101;
+            if (q < hi) { m[u] = M2[q]; r[u] = R2[q]; s[u] = S2[q]; }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (!(m[u] & 0x00ff)) { sr += r[u].x; ss += s[u].x; ++cnt; }
+            if (!(m[u] & 0xff00)) { sr += r[u].y; ss += s[u].y; ++cnt; }
+        }
+    }
+    __shared__ double red[3][256];
+    red[0][tid] = sr; red[1][tid] = ss; red[2][tid] = (double)cnt;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (tid < o) { red[0][tid] += red[0][tid + o]; red[1][tid] += red[1][tid + o]; red[2][tid] += red[2][tid + o]; }
+        __syncthreads();
+    }
+    if (tid < 3) part[((size_t)b * nblk + blockIdx.x) * 3 + tid] = red[tid][0];
+}
+
+// gmean[b] = (mean R, mean S) over the unmasked pixels: tree sum of the nblk partials by one CTA per batch entry
+__global__ void __launch_bounds__(256) k_unmasked_mean(const double *__restrict__ part, double *__restrict__ gmean, int nblk) {
+    const int b = blockIdx.x, tid = threadIdx.x;
+    double v[3] = {0.0, 0.0, 0.0};
+    for (int k = tid; k < nblk; k += 256)
+        for (int c = 0; c < 3; ++c) v[c] += part[((size_t)b * nblk + k) * 3 + c];
+    __shared__ double red[3][256];
+    for (int c = 0; c < 3; ++c) red[c][tid] = v[c];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (tid < o) for (int c = 0; c < 3; ++c) red[c][tid] += red[c][tid + o];
+        __syncthreads();
+    }
+    if (tid == 0) {
+        const double cnt = red[2][0];
+        gmean[2 * b] = cnt > 0.0 ? red[0][0] / cnt : 0.0;
+        gmean[2 * b + 1] = cnt > 0.0 ? red[1][0] / cnt : 0.0;
+    }
+}
+
+// Window mean of the unmasked pixels around masked pixel (x, y), by a whole warp: lane l takes the window positions
+// l, l + 32, ... (row-major in the (2 rb + 1)^2 window) and the partial sums are combined by a butterfly, which
+// leaves the same value in every lane (a + b = b + a exactly).  A single thread walking the window alone is a chain
+// of (2 rb + 1)^2 dependent loads: it set the run time of the whole kernel.  Falls back to the global mean.
+__device__ __forceinline__ void warp_fill_one(const double *R, const double *S, const unsigned char *__restrict__ mask,
+                                              const double *__restrict__ gmean, size_t img, int x, int y, int H, int W, int rb,
+                                              int b, double &outR, double &outS) {
+    const int lane = threadIdx.x & 31, side = 2 * rb + 1, n = side * side;
+    const int hm = (H & (H - 1)) == 0 ? H - 1 : -1, wm = (W & (W - 1)) == 0 ? W - 1 : -1;
+    double sr = 0.0, ss = 0.0;
+    int cnt = 0;
+    for (int i = lane; i < n; i += 32) {
+        const int dx = i / side - rb, dy = i % side - rb;
+        const size_t q = img + (size_t)wrap_index(x + dx, H, hm) * W + wrap_index(y + dy, W, wm);
+        if (!mask[q]) { sr += R[q]; ss += S[q]; ++cnt; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sr += __shfl_xor_sync(0xffffffffu, sr, o);
+        ss += __shfl_xor_sync(0xffffffffu, ss, o);
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    }
+    outR = cnt > 0 ? sr / cnt : gmean[2 * b];
+    outS = cnt > 0 ? ss / cnt : gmean[2 * b + 1];
+}
+
+// copy / fill, two adjacent pixels per thread (W even: 16-byte aligned pairs); the masked pixels of a warp are filled
+// one after the other by the whole warp.  Rm may alias R (and Sm alias S): only unmasked pixels are read from the
+// window and those are never modified.
+__global__ void __launch_bounds__(256) k_fill(const double *R, const double *S, const unsigned char *__restrict__ mask,
+                                              const double *__restrict__ gmean, double *Rm, double *Sm, int H, int W, int rb) {
+    const int y = 2 * (blockIdx.x * blockDim.x + threadIdx.x), x = blockIdx.y, b = blockIdx.z, lane = threadIdx.x & 31;
+    const bool live = y < W;                               // (no early exit: the fills below need all 32 lanes)
+    const size_t img = (size_t)b * H * W, p = img + (size_t)x * W + (live ? y : 0);
+    unsigned m = 0;
+    double2 r = make_double2(0.0, 0.0), s = r;
+    if (live) {
+        m = *reinterpret_cast<const unsigned short *>(&mask[p]);
+        r = *reinterpret_cast<const double2 *>(&R[p]);
+        s = *reinterpret_cast<const double2 *>(&S[p]);
+    }
+    unsigned todo = __ballot_sync(0xffffffffu, m != 0);
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const unsigned ms = __shfl_sync(0xffffffffu, m, src);
+        const int ys = __shfl_sync(0xffffffffu, y, src);
+        double fr, fs;
+        if (ms & 0x00ff) {
+            warp_fill_one(R, S, mask, gmean, img, x, ys, H, W, rb, b, fr, fs);
+            if (lane == src) { r.x = fr; s.x = fs; }
+        }
+        if (ms & 0xff00) {
+            warp_fill_one(R, S, mask, gmean, img, x, ys + 1, H, W, rb, b, fr, fs);
+            if (lane == src) { r.y = fr; s.y = fs; }
+        }
+    }
+    if (live) {
+        *reinterpret_cast<double2 *>(&Rm[p]) = r;
+        *reinterpret_cast<double2 *>(&Sm[p]) = s;
+    }
+}
+
+// ---- one-pixel-per-thread forms of the three kernels above, for odd W or image pointers that are not 16-byte aligned ----
 // mask(x,y) = OR_{|dx| <= rd} t((x+dx) mod H, y)
-__global__ void k_mask_cols(const unsigned char *__restrict__ t, unsigned char *__restrict__ mask, int H, int W, int rd) {
+__global__ void k_mask_cols_1(const unsigned char *__restrict__ t, unsigned char *__restrict__ mask, int H, int W, int rd) {
     const int y = blockIdx.x * blockDim.x + threadIdx.x, x = blockIdx.y, b = blockIdx.z;
     if (y >= W) return;
     const size_t img = (size_t)b * H * W;
@@ -38,7 +189,7 @@ __global__ void k_mask_cols(const unsigned char *__restrict__ t, unsigned char *
 }
 
 // partial sums of the unmasked pixels: part[b][blk] = (sum R, sum S, count), fixed order (deterministic)
-__global__ void __launch_bounds__(256) k_unmasked_partial(const double *__restrict__ R, const double *__restrict__ S,
+__global__ void __launch_bounds__(256) k_unmasked_partial_1(const double *__restrict__ R, const double *__restrict__ S,
                                                           const unsigned char *__restrict__ mask, double *__restrict__ part,
                                                           size_t P, int nblk) {
     const int b = blockIdx.y, tid = threadIdx.x;
@@ -58,18 +209,8 @@ __global__ void __launch_bounds__(256) k_unmasked_partial(const double *__restri
     if (tid < 3) part[((size_t)b * nblk + blockIdx.x) * 3 + tid] = red[tid][0];
 }
 
-// gmean[b] = (mean R, mean S) over the unmasked pixels
-__global__ void k_unmasked_mean(const double *__restrict__ part, double *__restrict__ gmean, int nblk) {
-    const int b = blockIdx.x;
-    if (threadIdx.x != 0) return;
-    double sr = 0.0, ss = 0.0, cnt = 0.0;
-    for (int k = 0; k < nblk; ++k) { sr += part[((size_t)b * nblk + k) * 3]; ss += part[((size_t)b * nblk + k) * 3 + 1]; cnt += part[((size_t)b * nblk + k) * 3 + 2]; }
-    gmean[2 * b] = cnt > 0.0 ? sr / cnt : 0.0;
-    gmean[2 * b + 1] = cnt > 0.0 ? ss / cnt : 0.0;
-}
-
 // copy / fill.  Rm may alias R (and Sm alias S): only unmasked pixels are read from the window and those are never modified.
-__global__ void k_fill(const double *R, const double *S, const unsigned char *__restrict__ mask,
+__global__ void k_fill_1(const double *R, const double *S, const unsigned char *__restrict__ mask,
                        const double *__restrict__ gmean, double *Rm, double *Sm, int H, int W, int rb) {
     const int y = blockIdx.x * blockDim.x + threadIdx.x, x = blockIdx.y, b = blockIdx.z;
     if (y >= W) return;
@@ -92,6 +233,27 @@ __global__ void k_fill(const double *R, const double *S, const unsigned char *__
     Sm[p] = cnt > 0 ? ss / cnt : gmean[2 * b + 1];
 }
 
+
+// launch sequence shared by the plan path and the static-scratch entry point
+inline cudaError_t mask_fill_launches(const double *dR, const double *dS, double satR, double satS, int rd, int rb, double *dRm,
+                                      double *dSm, unsigned char *dmask, int H, int W, int nb, unsigned char *t, double *part,
+                                      double *gmean, cudaStream_t st) {
+    const uintptr_t a16 = (uintptr_t)dR | (uintptr_t)dS | (uintptr_t)dRm | (uintptr_t)dSm;
+    const bool pairs = W % 2 == 0 && (a16 & 15) == 0 && ((uintptr_t)dmask & 1) == 0 && ((uintptr_t)t & 1) == 0;
+    k_mask_rows<<<dim3((W + 1023) / 1024, H, nb), 256, 0, st>>>(dR, dS, t, H, W, rd, satR, satS);
+    if (pairs) {
+        k_mask_cols<<<dim3((W / 2 + 127) / 128, (H + kMfColRows - 1) / kMfColRows, nb), 128, 0, st>>>(t, dmask, H, W, rd);
+        k_unmasked_partial<<<dim3(kMfBlocks, nb), 256, 0, st>>>(dR, dS, dmask, part, (size_t)H * W, kMfBlocks);
+    } else {
+        k_mask_cols_1<<<dim3((W + 255) / 256, H, nb), 256, 0, st>>>(t, dmask, H, W, rd);
+        k_unmasked_partial_1<<<dim3(kMfBlocks, nb), 256, 0, st>>>(dR, dS, dmask, part, (size_t)H * W, kMfBlocks);
+    }
+    k_unmasked_mean<<<nb, 256, 0, st>>>(part, gmean, kMfBlocks);
+    if (pairs) k_fill<<<dim3((W / 2 + 255) / 256, H, nb), 256, 0, st>>>(dR, dS, dmask, gmean, dRm, dSm, H, W, rb);
+    else k_fill_1<<<dim3((W + 255) / 256, H, nb), 256, 0, st>>>(dR, dS, dmask, gmean, dRm, dSm, H, W, rb);
+    return cudaGetLastError();
+}
+
 }  // namespace
 
 cudaError_t launch_mask_fill(sfft_plan *p, const double *dR, const double *dS, double satR, double satS, int rd, int rb,
@@ -100,17 +262,10 @@ cudaError_t launch_mask_fill(sfft_plan *p, const double *dR, const double *dS, d
     const size_t P = (size_t)H * W;
     // scratch in the spectrum-stack region of the workspace (rewritten by the next build): row-grown seeds, partial sums
     unsigned char *t = reinterpret_cast<unsigned char *>(p->rhat);
-    const int nblk = 256;
     double *part = reinterpret_cast<double *>(t + (((size_t)nb * P + 255) & ~(size_t)255));
-    double *gmean = part + (size_t)nb * nblk * 3;
-    dim3 grid((W + 255) / 256, H, nb);
-    k_mask_rows<<<grid, 256, 0, p->stream>>>(dR, dS, t, H, W, rd, satR, satS);
-    k_mask_cols<<<grid, 256, 0, p->stream>>>(t, dmask, H, W, rd);
-    k_unmasked_partial<<<dim3(nblk, nb), 256, 0, p->stream>>>(dR, dS, dmask, part, P, nblk);
-    k_unmasked_mean<<<nb, 32, 0, p->stream>>>(part, gmean, nblk);
-    k_fill<<<grid, 256, 0, p->stream>>>(dR, dS, dmask, gmean, dRm, dSm, H, W, rb);
+    double *gmean = part + (size_t)nb * kMfBlocks * 3;
     p->launches += 5;
-    return cudaGetLastError();
+    return mask_fill_launches(dR, dS, satR, satS, rd, rb, dRm, dSm, dmask, H, W, nb, t, part, gmean, p->stream);
 }
 
 }  // namespace sfft
@@ -119,7 +274,7 @@ cudaError_t launch_mask_fill(sfft_plan *p, const double *dR, const double *dS, d
 // For callers that cannot give the library device memory and must not have it allocate any (a process whose memory
 // all belongs to one pool, a loop that may not stall on cudaMalloc's device-wide synchronisation): no plan, no
 // workspace, no cudaMalloc / cudaFree.  The kernels are the ones launch_mask_fill runs; only the scratch differs.
-constexpr size_t kStaticHead = 8192;      // partial sums [256][3] doubles (6144 B) + the two means, rounded up
+constexpr size_t kStaticHead = 32768;     // partial sums [1184][3] doubles (28416 B) + the two means, rounded up
 constexpr int kStaticMaxDev = 64;
 
 // Scratch of sfft_mask_fill_static: [0, kStaticHead) partial sums and means, then one flag byte per pixel.  Shared by
@@ -175,16 +330,9 @@ extern "C" int sfft_mask_fill_static(const double *d_R, const double *d_S, int H
         scratch = g_static_ptr[dev];
     }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const int nblk = 256;
-    double *part = reinterpret_cast<double *>(scratch), *gmean = part + (size_t)nblk * 3;
+    double *part = reinterpret_cast<double *>(scratch), *gmean = part + (size_t)sfft::kMfBlocks * 3;
     unsigned char *t = scratch + kStaticHead;
-    const dim3 grid((W + 255) / 256, H, 1);
-    sfft::k_mask_rows<<<grid, 256, 0, st>>>(d_R, d_S, t, H, W, rd, sat_R, sat_S);
-    sfft::k_mask_cols<<<grid, 256, 0, st>>>(t, d_mask, H, W, rd);
-    sfft::k_unmasked_partial<<<dim3(nblk, 1), 256, 0, st>>>(d_R, d_S, d_mask, part, (size_t)H * W, nblk);
-    sfft::k_unmasked_mean<<<1, 32, 0, st>>>(part, gmean, nblk);
-    sfft::k_fill<<<grid, 256, 0, st>>>(d_R, d_S, d_mask, gmean, d_Rm, d_Sm, H, W, rb);
-    e = cudaGetLastError();
+    e = sfft::mask_fill_launches(d_R, d_S, sat_R, sat_S, rd, rb, d_Rm, d_Sm, d_mask, H, W, 1, t, part, gmean, st);
     if (e != cudaSuccess) return static_fail(SFFT_ERR_CUDA, std::string("sfft_mask_fill_static launch: ") + cudaGetErrorString(e));
     return SFFT_OK;
 }

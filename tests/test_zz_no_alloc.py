@@ -102,3 +102,38 @@ def test_mask_fill_static_at_its_largest_frame(cuda_device):
     assert int(mask0.sum()) >= 300 * 25 // 2
     assert torch.equal(mask, mask0) and bool(mask[H - 1, W - 1]) and bool(mask[0, 0])
     assert float((Rm - Rm0).abs().max()) <= 1e-12 * SAT and float((Sm - Sm0).abs().max()) <= 1e-12 * SAT
+
+
+@pytest.mark.gpu
+def test_mask_fill_static_odd_width_and_unaligned_images(cuda_device):
+    """Frames the plan path does not take (odd W) and images that start on an 8-byte but not a 16-byte boundary go
+    through the one-pixel-per-thread kernels: checked against the CPU oracle (mask bit for bit, fills to 1e-12 * sat),
+    and the unaligned call against the aligned one on the same pixels."""
+    import torch
+    import oracle
+    H, W, rd, rb = 97, 131, 2, 5
+    R, S = _saturated_pair(H, W, seed=5)
+    Rmo, Smo, mo = oracle.mask_fill(R, S, SAT, SAT, rd, rb)
+    dR, dS = torch.from_numpy(R).cuda(), torch.from_numpy(S).cuda()
+    Rm, Sm = torch.empty_like(dR), torch.empty_like(dS)
+    mask = torch.empty((H, W), dtype=torch.uint8, device=cuda_device)
+    B.mask_fill_static(dR, dS, SAT, SAT, rd, rb, Rm, Sm, mask)
+    assert mo.sum() > 0 and np.array_equal(mask.cpu().numpy(), mo)
+    assert np.max(np.abs(Rm.cpu().numpy() - Rmo)) <= 1e-12 * SAT and np.max(np.abs(Sm.cpu().numpy() - Smo)) <= 1e-12 * SAT
+    # even width, but every image shifted by one double (and the mask by one byte) inside a larger buffer
+    H, W = 64, 130
+    R, S = _saturated_pair(H, W, seed=6)
+    Rmo, Smo, mo = oracle.mask_fill(R, S, SAT, SAT, rd, rb)
+    bufs = [torch.zeros(H * W + 1, dtype=torch.float64, device=cuda_device) for _ in range(4)]
+    mbuf = torch.zeros(H * W + 1, dtype=torch.uint8, device=cuda_device)
+    uR, uS, uRm, uSm = [b[1:].view(H, W) for b in bufs]
+    umask = mbuf[1:].view(H, W)
+    assert uR.data_ptr() % 16 == 8 and umask.data_ptr() % 2 == 1
+    uR.copy_(torch.from_numpy(R)); uS.copy_(torch.from_numpy(S))
+    B.mask_fill_static(uR, uS, SAT, SAT, rd, rb, uRm, uSm, umask)
+    aR, aS = uR.clone(), uS.clone()
+    aRm, aSm, amask = torch.empty_like(aR), torch.empty_like(aS), torch.empty((H, W), dtype=torch.uint8, device=cuda_device)
+    B.mask_fill_static(aR, aS, SAT, SAT, rd, rb, aRm, aSm, amask)
+    for m_, r_, s_ in ((umask, uRm, uSm), (amask, aRm, aSm)):
+        assert np.array_equal(m_.cpu().numpy(), mo)
+        assert np.max(np.abs(r_.cpu().numpy() - Rmo)) <= 1e-12 * SAT and np.max(np.abs(s_.cpu().numpy() - Smo)) <= 1e-12 * SAT
