@@ -121,7 +121,7 @@ def workload_name(cfg_index):
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
-    def __init__(self, index=0, period=0.002):
+    def __init__(self, index=0, period=0.005):
         super().__init__(daemon=True)
         self.index, self.period, self.stop_flag = index, period, False
         self.sm, self.reasons, self.sm_max, self.ok = [], set(), None, False
