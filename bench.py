@@ -34,10 +34,11 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA/clk x
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's dominant kernel at config 4, from the
 # committed `ncu --set full` capture named in NCU_TRAFFIC_SOURCE (bytes).  Not measured by this run: the line
 # carries the source beside the number.
-NCU_TRAFFIC_CFG4 = {"rowfft": 268.5e6 + 481.8e6, "subtract": 468.2e6 + 114.4e6, "corr": 539.4e6 + 27.7e6}
-_R02B = "profiles/r02_b_end_of_round.md (capture at commit 13137ef)"
-_R02C = "profiles/r02_c_final.md (capture at commit 6820580)"
-NCU_TRAFFIC_SOURCE = {"rowfft": _R02C, "subtract": _R02B + " (k_fir_x)", "corr": _R02C + " (k_corr_os)"}
+NCU_TRAFFIC_CFG4 = {"rowfft": 268.5e6 + 480.8e6, "subtract": 468.1e6 + 114.5e6, "corr": 539.5e6 + 27.5e6,
+                    "subtract_inverse": 268.6e6 + 104.5e6}
+_R03 = "profiles/r03_final.md (ncu --set full capture at commit c0f72b4)"
+NCU_TRAFFIC_SOURCE = {"rowfft": _R03, "subtract": _R03 + " (k_fir_x)", "corr": _R03 + " (k_corr_os)",
+                      "subtract_inverse": _R03 + " (k_rowfft_inverse_sub)"}
 REFERENCE_BUDGET_S = 200.0      # wall-clock cap of the --impl reference arm (the oracle is slow by construction)
 
 
