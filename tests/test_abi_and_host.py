@@ -126,3 +126,18 @@ def test_two_rank_gloo_sharding():
     for p, (o, e) in zip(procs, outs):
         assert p.returncode == 0, e[-2000:]
         assert o.startswith("ok")
+
+
+def test_bench_configs_and_stage_names_agree_with_the_header():
+    """bench.py --config accepts 1..5 and `decam` (the paper's 2046 x 4094 CCD frame, on the config-3
+    recipe and model); the binding's stage list has the length include/sfft.h declares."""
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2109_09334_b200 import binding as B
+    assert bench.parse_config("decam") == bench.DECAM and bench.parse_config("4") == 4
+    d, c3 = bench.CONFIGS[bench.DECAM], bench.CONFIGS[3]
+    assert (d["H"], d["W"]) == (2046, 4094) and all(d[k] == c3[k] for k in ("L", "DK", "DB", "basis", "batch"))
+    assert bench.config_dict(bench.DECAM)["unknowns"] == 1356 and "2046x4094" in bench.workload_name(bench.DECAM)
+    text = open(os.path.join(ROOT, "include", "sfft.h")).read()
+    assert int(re.search(r"#define SFFT_NUM_STAGES (\d+)", text).group(1)) == B.SFFT_NUM_STAGES == len(B.STAGE_NAMES)
+    assert int(eval(re.search(r"#define SFFT_STATIC_MAX_PIXELS \((.*)\)", text).group(1).replace("L", ""))) == B.SFFT_STATIC_MAX_PIXELS
